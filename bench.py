@@ -1,0 +1,315 @@
+"""bench.py -- events/s and digis/s of the Clusters chain on B200, with its HBM roofline fraction.
+
+    python bench.py --gpus 1 --steps 10 --warmup 3            # this repo's CUDA path
+    python bench.py --impl reference --steps 3 --warmup 1     # the oracle on the host cores (the reference arm)
+
+A step = one pass of the whole hot path (init, unpack+calibrate+boundaries, classify, cluster x4 size classes,
+finalize) over one batch of synthetic events: BASELINE.json configs[2], 1000 PU50-like events (config[1]'s
+generator, seeds 0..999), through pix_process_batch.  `value` is timed with the inputs resident in HBM; `e2e`
+goes through pix_process_batch_host with pinned HOST buffers, host<->device copies inside the timed region.
+Under torchrun (N > 1) every rank runs its own 1000 events (seeds rank*1000 ..): weak scaling, no collective
+on the data path; the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import pixgen  # noqa: E402
+
+PARAMS = dict(pixgen.DEFAULT_PARAMS)
+WORKLOAD = "cfg2: 1000 PU50-like events (1856 modules, ~60.6k words/event), pix_process_batch"
+
+
+def peak_hbm():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def generate(n_events: int, rank: int):
+    det = pixgen.detector("full")
+    batch = pixgen.events(det, "pu50", rank * 1000 + np.arange(n_events), cap_words_per_event=1 << 17)
+    return det, batch
+
+
+def algorithmic_bytes(W, K, M, E):
+    """bytes(event) = 19 W + 22 K + 12 M + 68, summed over the batch."""
+    return 19 * W + 22 * K + (12 * M + 68) * E
+
+
+# ---------------------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """The oracle, as it stands, single-threaded on the host cores, on the same workload (bounded sample per step)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    n_sample = min(args.ref_events, args.events)
+    det, batch = generate(n_sample, 0)
+    sizes = np.diff(batch.event_offsets.astype(np.int64))
+
+    def step():
+        for e in range(n_sample):
+            oracle.process(det, *batch.event(e), PARAMS, max_clusters_per_event=int(sizes[e]))
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    v = n_sample / dt
+    line = {"impl": "reference", "metric": "events/s", "value": v, "unit": "events/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32+f32", "data": "synthetic",
+            "digis_per_s": float(sizes.sum()) / dt,
+            "config": {"workload": WORKLOAD, "sample": f"first {n_sample} events of the batch per step"},
+            "cpu_baseline": {"value": v, "unit": "events/s", "cores": 1, "kind": "oracle",
+                             "sample": f"first {n_sample} events of cfg2 per step, {args.steps} steps"},
+            "e2e": {"value": v, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------- this repo's arm
+def run_ours(args):
+    import torch
+    import paper_2104_06573_b200 as pix
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    E = args.events
+    det, batch = generate(E, rank)
+    M, F = det.n_modules, det.n_feds
+    sizes = np.diff(batch.event_offsets.astype(np.int64))
+    W = int(sizes.sum())
+    wmax = (int(sizes.max()) + 1023) // 1024 * 1024
+    kmax = args.max_clusters
+    params = pix.make_params(PARAMS, wmax, kmax, E, args.chunk_events)
+    h = pix.pix_create(det.cabling, F, M, det.gain, det.pedestal, params)
+
+    dev = torch.device("cuda", local)
+    pad = np.zeros(16, np.uint32)
+    words_h = torch.from_numpy(np.concatenate([batch.words, pad]).view(np.int32)).pin_memory()
+    evoff_h = torch.from_numpy(batch.event_offsets.view(np.int32).copy()).pin_memory()
+    fedoff_h = torch.from_numpy(batch.fed_offsets.view(np.int32).reshape(-1).copy()).pin_memory()
+    words, ev_off, fed_off = words_h.to(dev), evoff_h.to(dev), fedoff_h.to(dev)
+    digis, clusters = pix.alloc_outputs(W, E, M, kmax, dev)
+    stream = torch.cuda.Stream(dev)
+
+    def step():
+        pix.pix_process_batch(h, stream, E, words, W, ev_off, fed_off, digis, clusters)
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events on the launch stream.
+    # Inputs (242 MB) + outputs (~1.3 GB) per step exceed the 126 MB L2, so no explicit flush is needed.
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    n0 = pix.pix_kernel_launches(h)
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    clocks = sampler.stop() if sampler else None
+    launches = pix.pix_kernel_launches(h) - n0
+    if dist is not None:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- per-kernel device time (CUDA events between the kernels, on the launch stream), same steps again
+    pix.pix_set_profiling(h, True)
+    for _ in range(args.steps):
+        step()
+    prof, n_chunks = pix.pix_read_profile(h)
+    pix.pix_set_profiling(h, False)
+    prof = {k: v / args.steps for k, v in prof.items()}  # ms per step, summed over the step's chunks
+    chunks_per_step = n_chunks // args.steps
+
+    # ---- what the step produced (for the byte counts) + a parity spot check against the oracle (rank 0)
+    torch.cuda.synchronize()
+    summ = clusters["summary"].cpu().numpy().reshape(E, 16).astype(np.int64)
+    K = int(summ[:, 14].sum())
+    mf = clusters["module_first"].cpu().numpy().astype(np.int64)
+    me = clusters["module_end"].cpu().numpy().astype(np.int64)
+    cms = clusters["clus_module_start"].cpu().numpy().reshape(E, M + 1).astype(np.int64)
+    run_len = me - mf
+    run_clus = np.diff(cms, axis=1).reshape(-1)
+    bounds = (0, 128, 768, 4096, 1 << 30)
+    names = ("cluster_warp", "cluster_small", "cluster_large", "cluster_global")
+    kernel_bytes = {"unpack": 15 * W, "finalize": 42 * K + (4 * (M + 1) + 64 + 4 * M) * E,
+                    "init": 8 * M * E, "classify": (8 + 4 + 20) * M * E}
+    for q, nm in enumerate(names):
+        sel = (run_len > bounds[q]) & (run_len <= bounds[q + 1])
+        kernel_bytes[nm] = int(13 * run_len[sel].sum() + 20 * run_clus[sel].sum())
+    top = max(prof, key=prof.get)
+    peak, peak_src = peak_hbm()
+    top_launches = chunks_per_step
+    top_gbs = kernel_bytes[top] / (prof[top] * 1e-3) / 1e9 if prof[top] > 0 else 0.0
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(top)
+    chain_bytes = algorithmic_bytes(W, K, M, E)
+    chain_gbs = chain_bytes / (ms * 1e-3) / 1e9
+
+    parity = None
+    if rank == 0 and not args.no_check:
+        import oracle
+        bad = 0
+        for e in (0, E // 2, E - 1):
+            o = oracle.process(det, *batch.event(e), PARAMS, max_clusters_per_event=kmax)
+            a, b = int(batch.event_offsets[e]), int(batch.event_offsets[e + 1])
+            bad += int(not np.array_equal(o["summary"].astype(np.int64), summ[e]))
+            bad += int(not np.array_equal(o["clus"], digis["clus"][a:b].cpu().numpy()))
+            bad += int(not np.array_equal(o["status"], digis["status"][a:b].cpu().numpy()))
+            bad += int(not np.array_equal(o["c_charge"], clusters["charge"][e * kmax:e * kmax + len(o["c_charge"])].cpu().numpy()))
+        parity = "ok (3 events, summary/clus/status/cluster charge bit-exact)" if bad == 0 else f"MISMATCH x{bad}"
+
+    # ---- end to end: same metric through pix_process_batch_host, pinned host buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hd, hc = pix.alloc_outputs(W, E, M, kmax, "cpu", pinned=True)
+        hstep = lambda: pix.pix_process_batch_host(h, stream, E, words_h, W, evoff_h, fedoff_h, hd, hc)  # noqa: E731
+        hstep()
+        barrier()
+        n_e2e = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            hstep()  # synchronous: returns after the device->host copies have landed
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / n_e2e
+        if dist is not None:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        h2d = W * 4 + (E + 1) * 4 + E * (F + 1) * 4
+        d2h = W * 15 + E * kmax * 22 + E * (3 * M + 1 + 16) * 4
+        e2e = {"value": E * world / dt, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "ms_per_step": dt * 1e3, "steps": n_e2e}
+
+    # ---- the oracle on this box's host cores (rank 0, N = 1 only), bounded sample
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        ns = min(args.ref_events, E)
+        t0 = time.perf_counter()
+        for e in range(ns):
+            oracle.process(det, *batch.event(e), PARAMS, max_clusters_per_event=int(sizes[e]))
+        dt = time.perf_counter() - t0
+        cpu = {"value": ns / dt, "unit": "events/s", "cores": 1, "kind": "oracle",
+               "sample": f"first {ns} events of the same batch, single thread, {dt:.1f} s", "digis_per_s": float(sizes[:ns].sum()) / dt}
+
+    pix.pix_destroy(h)
+    if rank == 0:
+        line = {
+            "metric": "events/s", "value": E * world / (ms * 1e-3), "unit": "events/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32+f32", "data": "synthetic",
+            "digis_per_s": W * world / (ms * 1e-3),
+            "config": {"workload": WORKLOAD, "events_per_gpu": E, "words_per_step_per_gpu": W, "clusters_per_step_per_gpu": K,
+                       "chunk_events": h.params["chunk_events"] or "auto", "chunks_per_step": chunks_per_step,
+                       "l2": "inputs+outputs per step (~1.5 GB) exceed the 126 MB L2; no flush"},
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e,
+            "roofline": {"bound": "hbm", "kernel": top, "achieved": top_gbs, "peak": peak, "unit": "GB/s",
+                         "frac": top_gbs / peak, "traffic": traffic, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": kernel_bytes[top] / max(top_launches, 1),
+                         "avg_launch_ms": prof[top] / max(top_launches, 1), "launches_per_step": top_launches},
+            "roofline_chain": {"bound": "hbm", "achieved": chain_gbs, "peak": peak, "unit": "GB/s", "frac": chain_gbs / peak,
+                               "algorithmic_bytes_per_step": chain_bytes, "formula": "19 W + 22 K + (12 M + 68) E"},
+            "kernel_ms_per_step": prof, "kernel_algorithmic_bytes_per_step": kernel_bytes,
+            "cpu_baseline": cpu, "parity_spot_check": parity,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--events", type=int, default=1000, help="events per step per GPU (cfg2: 1000)")
+    ap.add_argument("--chunk-events", type=int, default=0, help="events per internal launch group (0 = library default)")
+    ap.add_argument("--max-clusters", type=int, default=20480, help="cluster record capacity per event")
+    ap.add_argument("--ref-events", type=int, default=1000, help="events of the oracle sample (cpu_baseline / reference arm)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-check", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

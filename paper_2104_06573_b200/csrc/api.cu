@@ -1,0 +1,352 @@
+// api.cu -- the C ABI of libpixclus.so (include/pixclus.h).  Host code only: argument checks, device tables,
+// workspace, the per-chunk launch sequence.  No step of the path runs here; there is no CPU fallback.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/pixclus.h"
+#include "pix_common.cuh"
+
+namespace {
+
+struct SharedTables {  // read-only device tables shared by clones
+  std::atomic<int> refs{1};
+  uint32_t* cab = nullptr;
+  float2* gp = nullptr;
+};
+
+struct HostStage {  // device staging of pix_process_batch_host, allocated on first use
+  bool ready = false;
+  uint32_t *words = nullptr, *ev_off = nullptr, *fed_off = nullptr;
+  uint16_t *d_module = nullptr, *d_row = nullptr, *d_col = nullptr; int32_t *d_charge = nullptr, *d_clus = nullptr;
+  uint8_t* d_status = nullptr;
+  uint16_t* c_module = nullptr; uint32_t *c_first = nullptr, *c_npix = nullptr, *c_charge = nullptr;
+  float *c_x = nullptr, *c_y = nullptr;
+  uint32_t *module_first = nullptr, *module_end = nullptr, *clus_module_start = nullptr, *summary = nullptr;
+  std::vector<void*> allocs;
+};
+
+}  // namespace
+
+struct pix_handle {
+  int device = 0, n_sm = 0;
+  uint32_t F = 0, M = 0;
+  pix_params p{};
+  uint32_t chunk_events = 0, cap_words = 0;
+  uint64_t cap_total = 0;
+  SharedTables* tables = nullptr;
+  void* ws = nullptr;  // one allocation, carved below
+  pix::Chunk proto{};  // tables, params and workspace pointers filled once
+  uint64_t launches = 0;
+  std::string err;
+  HostStage hs;
+  bool profiling = false;
+  std::vector<cudaEvent_t> prof_events;  // 9 per chunk, in launch order
+  size_t prof_used = 0;
+};
+
+namespace {
+
+int fail(pix_handle* h, int code, const char* msg) {
+  if (h) h->err = msg;
+  return code;
+}
+int fail_cuda(pix_handle* h, cudaError_t e, const char* where) {
+  if (h) h->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return PIX_ERR_CUDA;
+}
+
+size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+// workspace layout; pass base == nullptr to get the size only
+size_t carve_workspace(pix_handle* h, unsigned char* base) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { unsigned char* p = base ? base + off : nullptr; off += align_up(bytes); return p; };
+  const size_t Ec = h->chunk_events, M = h->M, F = h->F, W = h->cap_words;
+  pix::Chunk& c = h->proto;
+  c.segB = (uint32_t*)take((Ec * F + 1) * 4);
+  c.ev_cnt = (uint32_t*)take(Ec * pix::EC_STRIDE * 4);
+  c.ctl = (uint32_t*)take(16 * 4);
+  c.lists = (uint32_t*)take((size_t)pix::N_TIERS * Ec * M * 4);
+  c.list_stride = (uint32_t)(Ec * M);
+  c.n_clus = (uint32_t*)take(Ec * M * 4);
+  c.mod_cnt = (uint32_t*)take(Ec * M * pix::MC_STRIDE * 4);
+  c.t_first = (uint32_t*)take(W * 4); c.t_npix = (uint32_t*)take(W * 4); c.t_charge = (uint32_t*)take(W * 4);
+  c.t_x = (float*)take(W * 4); c.t_y = (float*)take(W * 4);
+  c.g_hash = (unsigned long long*)take(W * 16);
+  c.g_pos = (uint32_t*)take(W * 4); c.g_q = (uint32_t*)take(W * 4); c.g_npix = (uint32_t*)take(W * 4);
+  c.g_sx = (unsigned long long*)take(W * 8); c.g_sy = (unsigned long long*)take(W * 8);
+  return off;
+}
+
+int make_workspace(pix_handle* h) {
+  const size_t bytes = carve_workspace(h, nullptr);
+  cudaError_t e = cudaMalloc(&h->ws, bytes);
+  if (e != cudaSuccess) { h->ws = nullptr; cudaGetLastError(); return PIX_ERR_ALLOC; }
+  carve_workspace(h, (unsigned char*)h->ws);
+  return PIX_OK;
+}
+
+void release_tables(SharedTables* t) {
+  if (t && t->refs.fetch_sub(1) == 1) { cudaFree(t->cab); cudaFree(t->gp); delete t; }
+}
+
+bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+int check_outputs(pix_handle* h, const pix_digis* d, const pix_clusters* k) {
+  if (!d || !k) return fail(h, PIX_ERR_INVALID_ARG, "out_digis / out_clusters is NULL");
+  if (!d->module || !d->row || !d->col || !d->charge || !d->clus || !d->status)
+    return fail(h, PIX_ERR_INVALID_ARG, "a digi output array is NULL");
+  if (!k->module || !k->first_digi || !k->n_pix || !k->charge || !k->x_col || !k->y_row || !k->module_first ||
+      !k->module_end || !k->clus_module_start || !k->summary)
+    return fail(h, PIX_ERR_INVALID_ARG, "a cluster output array is NULL");
+  if (!aligned16(d->module) || !aligned16(d->row) || !aligned16(d->col) || !aligned16(d->charge) ||
+      !aligned16(d->clus) || !aligned16(d->status))
+    return fail(h, PIX_ERR_INVALID_ARG, "digi output arrays must be 16-byte aligned");
+  return PIX_OK;
+}
+
+void bind_outputs(pix::Chunk& c, const pix_digis* d, const pix_clusters* k) {
+  c.d_module = d->module; c.d_row = d->row; c.d_col = d->col; c.d_charge = d->charge; c.d_clus = d->clus;
+  c.d_status = d->status;
+  c.c_module = k->module; c.c_first = k->first_digi; c.c_npix = k->n_pix; c.c_charge = k->charge;
+  c.c_x = k->x_col; c.c_y = k->y_row;
+  c.module_first = k->module_first; c.module_end = k->module_end; c.clus_module_start = k->clus_module_start;
+  c.summary = k->summary;
+}
+
+// the launch sequence of one chunk
+int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t words_bound, cudaStream_t s) {
+  cudaEvent_t* ev = nullptr;
+  if (h->profiling) {
+    while (h->prof_events.size() < h->prof_used + 9) {
+      cudaEvent_t x;
+      if (cudaEventCreate(&x) != cudaSuccess) return fail(h, PIX_ERR_ALLOC, "cudaEventCreate");
+      h->prof_events.push_back(x);
+    }
+    ev = h->prof_events.data() + h->prof_used;
+    h->prof_used += 9;
+    cudaEventRecord(ev[0], s);
+  }
+  pix::launch_init(c, n_total, h->n_sm, s);
+  if (ev) cudaEventRecord(ev[1], s);
+  pix::launch_unpack(c, words_bound, h->n_sm, s);
+  if (ev) cudaEventRecord(ev[2], s);
+  pix::launch_classify(c, h->n_sm, s);
+  if (ev) cudaEventRecord(ev[3], s);
+  pix::launch_cluster(c, words_bound, h->n_sm, s, ev ? ev + 4 : nullptr);
+  pix::launch_finalize(c, h->n_sm, s);
+  if (ev) cudaEventRecord(ev[8], s);
+  h->launches += pix::LAUNCHES_PER_CHUNK;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
+  return PIX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, const pix_params* params, pix_handle** out) {
+  if (!cabling || !gains || !params || !out || !cabling->entry || !gains->gain || !gains->pedestal) return PIX_ERR_INVALID_ARG;
+  const uint32_t F = cabling->n_feds, M = cabling->n_modules;
+  if (F < 1 || F > 65535 || M < 1 || M > pix::MAX_MODULES || gains->n_modules != M) return PIX_ERR_INVALID_ARG;
+  if (params->pixel_threshold_e < 1 || params->max_electrons < 1 || params->max_electrons > 65535) return PIX_ERR_INVALID_ARG;
+  if (params->max_words_per_event < 1 || params->max_events_per_batch < 1 || params->max_clusters_per_event < 1)
+    return PIX_ERR_INVALID_ARG;
+  for (size_t i = 0; i < (size_t)F * 64 * 32; ++i)  // every mapped entry must name a module of the gain table
+    if ((cabling->entry[i] & 2u) && ((cabling->entry[i] >> 2) & 0xFFFFu) >= M) return PIX_ERR_INVALID_ARG;
+
+  pix_handle* h = new (std::nothrow) pix_handle;
+  if (!h) return PIX_ERR_ALLOC;
+  h->F = F; h->M = M; h->p = *params;
+  cudaError_t e = cudaGetDevice(&h->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
+  if (e == cudaSuccess) e = pix::configure_cluster_kernels();
+  if (e == cudaSuccess) e = pix::configure_finalize_kernel();
+  if (e != cudaSuccess) { delete h; cudaGetLastError(); return PIX_ERR_CUDA; }
+
+  // chunking: events per internal launch group; default keeps a chunk's digis within the L2-friendly few MB
+  uint64_t ce = params->chunk_events;
+  if (ce == 0) { ce = (4u << 20) / params->max_words_per_event; if (ce < 1) ce = 1; }
+  if (ce > params->max_events_per_batch) ce = params->max_events_per_batch;
+  if (ce > 65535) ce = 65535;
+  const uint64_t capw = ce * (uint64_t)params->max_words_per_event;
+  if (capw > 0x7FFFFFFFull || ce * (uint64_t)M > 0x7FFFFFFFull) { delete h; return PIX_ERR_INVALID_ARG; }
+  h->chunk_events = (uint32_t)ce; h->cap_words = (uint32_t)capw;
+  h->cap_total = (uint64_t)params->max_words_per_event * params->max_events_per_batch;
+  if (h->cap_total > 0xFFFFFFFFull) h->cap_total = 0xFFFFFFFFull;
+
+  // tables: cabling as given; (gain, pedestal) interleaved so that a digi costs one 8-byte gather
+  SharedTables* t = new (std::nothrow) SharedTables;
+  if (!t) { delete h; return PIX_ERR_ALLOC; }
+  h->tables = t;
+  const size_t ncab = (size_t)F * 64 * 32, ngp = (size_t)M * PIX_COLS;
+  std::vector<float2> gp(ngp);
+  for (size_t i = 0; i < ngp; ++i) gp[i] = make_float2(gains->gain[i], gains->pedestal[i]);
+  bool ok = cudaMalloc(&t->cab, ncab * 4) == cudaSuccess && cudaMalloc(&t->gp, ngp * sizeof(float2)) == cudaSuccess;
+  ok = ok && cudaMemcpy(t->cab, cabling->entry, ncab * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+  ok = ok && cudaMemcpy(t->gp, gp.data(), ngp * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess;
+  if (!ok) { cudaGetLastError(); release_tables(t); delete h; return PIX_ERR_ALLOC; }
+
+  pix::Chunk& c = h->proto;
+  c.F = F; c.M = M; c.cab = t->cab; c.gp = t->gp;
+  c.vcal_gain = params->vcal_gain; c.vcal_offset = params->vcal_offset; c.max_e_f = (float)params->max_electrons;
+  c.thr = params->pixel_threshold_e; c.cut = params->cluster_charge_cut_e;
+  c.cap_mod = params->max_clusters_per_module; c.cap_ev = params->max_clusters_per_event; c.cap_words = h->cap_words;
+  if (make_workspace(h) != PIX_OK) { release_tables(t); delete h; return PIX_ERR_ALLOC; }
+  *out = h;
+  return PIX_OK;
+}
+
+int pix_clone(const pix_handle* src, pix_handle** out) {
+  if (!src || !out) return PIX_ERR_INVALID_ARG;
+  pix_handle* h = new (std::nothrow) pix_handle;
+  if (!h) return PIX_ERR_ALLOC;
+  h->device = src->device; h->n_sm = src->n_sm; h->F = src->F; h->M = src->M; h->p = src->p;
+  h->chunk_events = src->chunk_events; h->cap_words = src->cap_words; h->cap_total = src->cap_total;
+  h->tables = src->tables; h->tables->refs.fetch_add(1);
+  h->proto = src->proto;
+  if (make_workspace(h) != PIX_OK) { release_tables(h->tables); delete h; return PIX_ERR_ALLOC; }
+  *out = h;
+  return PIX_OK;
+}
+
+int pix_destroy(pix_handle* h) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  cudaFree(h->ws);
+  for (void* p : h->hs.allocs) cudaFree(p);
+  for (cudaEvent_t x : h->prof_events) cudaEventDestroy(x);
+  release_tables(h->tables);
+  delete h;
+  return PIX_OK;
+}
+
+int pix_process(pix_handle* h, void* cuda_stream, const uint32_t* raw_words, const uint32_t* fed_offsets,
+                uint32_t n_words, const pix_digis* out_digis, const pix_clusters* out_clusters) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  h->err.clear();
+  if (n_words > 0 && !raw_words) return fail(h, PIX_ERR_INVALID_ARG, "raw_words is NULL");
+  if (!aligned16(raw_words)) return fail(h, PIX_ERR_INVALID_ARG, "raw_words must be 16-byte aligned");
+  if (h->F > 1 && !fed_offsets) return fail(h, PIX_ERR_INVALID_ARG, "fed_offsets is NULL but n_feds > 1");
+  if (int rc = check_outputs(h, out_digis, out_clusters)) return rc;
+  if (n_words > h->p.max_words_per_event || n_words > h->cap_words) return fail(h, PIX_ERR_CAPACITY, "n_words > max_words_per_event");
+  pix::Chunk c = h->proto;
+  c.words = raw_words; c.ev_off = nullptr; c.fed_off = h->F > 1 ? fed_offsets : nullptr; c.n_single = n_words;
+  c.e0 = 0; c.e1 = 1;
+  bind_outputs(c, out_digis, out_clusters);
+  return run_chunk(h, c, n_words, n_words, (cudaStream_t)cuda_stream);
+}
+
+int pix_process_batch(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* raw_words,
+                      uint32_t n_words_total, const uint32_t* event_word_offsets, const uint32_t* fed_offsets,
+                      const pix_digis* out_digis, const pix_clusters* out_clusters) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  h->err.clear();
+  if (n_events == 0) return PIX_OK;
+  if (!event_word_offsets) return fail(h, PIX_ERR_INVALID_ARG, "event_word_offsets is NULL");
+  if (n_words_total > 0 && !raw_words) return fail(h, PIX_ERR_INVALID_ARG, "raw_words is NULL");
+  if (!aligned16(raw_words)) return fail(h, PIX_ERR_INVALID_ARG, "raw_words must be 16-byte aligned");
+  if (h->F > 1 && !fed_offsets) return fail(h, PIX_ERR_INVALID_ARG, "fed_offsets is NULL but n_feds > 1");
+  if (int rc = check_outputs(h, out_digis, out_clusters)) return rc;
+  if (n_events > h->p.max_events_per_batch) return fail(h, PIX_ERR_CAPACITY, "n_events > max_events_per_batch");
+  if ((uint64_t)n_words_total > h->cap_total) return fail(h, PIX_ERR_CAPACITY, "n_words_total > max_words_per_event * max_events_per_batch");
+  pix::Chunk c = h->proto;
+  c.words = raw_words; c.ev_off = event_word_offsets; c.fed_off = h->F > 1 ? fed_offsets : nullptr; c.n_single = 0;
+  bind_outputs(c, out_digis, out_clusters);
+  const uint32_t bound = n_words_total < h->cap_words ? n_words_total : h->cap_words;
+  for (uint32_t e0 = 0; e0 < n_events; e0 += h->chunk_events) {
+    c.e0 = e0; c.e1 = (n_events - e0 > h->chunk_events) ? e0 + h->chunk_events : n_events;
+    if (int rc = run_chunk(h, c, n_words_total, bound, (cudaStream_t)cuda_stream)) return rc;
+  }
+  return PIX_OK;
+}
+
+int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* raw_words,
+                           uint32_t n_words_total, const uint32_t* event_word_offsets, const uint32_t* fed_offsets,
+                           const pix_digis* od, const pix_clusters* oc) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  h->err.clear();
+  if (n_events == 0) return PIX_OK;
+  if (!event_word_offsets || !od || !oc) return fail(h, PIX_ERR_INVALID_ARG, "NULL argument");
+  if (n_words_total > 0 && !raw_words) return fail(h, PIX_ERR_INVALID_ARG, "raw_words is NULL");
+  if (h->F > 1 && !fed_offsets) return fail(h, PIX_ERR_INVALID_ARG, "fed_offsets is NULL but n_feds > 1");
+  if (n_events > h->p.max_events_per_batch) return fail(h, PIX_ERR_CAPACITY, "n_events > max_events_per_batch");
+  if ((uint64_t)n_words_total > h->cap_total) return fail(h, PIX_ERR_CAPACITY, "n_words_total > capacity");
+  HostStage& s = h->hs;
+  const size_t E = h->p.max_events_per_batch, W = (size_t)h->cap_total, M = h->M, F = h->F, K = h->p.max_clusters_per_event;
+  if (!s.ready) {
+    bool ok = true;
+    auto dev = [&](size_t bytes) -> void* {
+      void* p = nullptr;
+      if (!ok) return p;
+      if (cudaMalloc(&p, bytes ? bytes : 16) != cudaSuccess) { ok = false; cudaGetLastError(); return (void*)nullptr; }
+      s.allocs.push_back(p);
+      return p;
+    };
+    s.words = (uint32_t*)dev(W * 4); s.ev_off = (uint32_t*)dev((E + 1) * 4); s.fed_off = (uint32_t*)dev(E * (F + 1) * 4);
+    s.d_module = (uint16_t*)dev(W * 2); s.d_row = (uint16_t*)dev(W * 2); s.d_col = (uint16_t*)dev(W * 2);
+    s.d_charge = (int32_t*)dev(W * 4); s.d_clus = (int32_t*)dev(W * 4); s.d_status = (uint8_t*)dev(W);
+    s.c_module = (uint16_t*)dev(E * K * 2); s.c_first = (uint32_t*)dev(E * K * 4); s.c_npix = (uint32_t*)dev(E * K * 4);
+    s.c_charge = (uint32_t*)dev(E * K * 4); s.c_x = (float*)dev(E * K * 4); s.c_y = (float*)dev(E * K * 4);
+    s.module_first = (uint32_t*)dev(E * M * 4); s.module_end = (uint32_t*)dev(E * M * 4);
+    s.clus_module_start = (uint32_t*)dev(E * (M + 1) * 4); s.summary = (uint32_t*)dev(E * 16 * 4);
+    if (!ok) { for (void* p : s.allocs) cudaFree(p); s.allocs.clear(); return fail(h, PIX_ERR_ALLOC, "staging allocation failed"); }
+    s.ready = true;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t n = n_words_total, Ev = n_events;
+  cudaError_t e = cudaSuccess;
+  auto h2d = [&](void* d, const void* src, size_t bytes) { if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st); };
+  auto d2h = [&](void* dst, const void* d, size_t bytes) { if (e == cudaSuccess && dst && bytes) e = cudaMemcpyAsync(dst, d, bytes, cudaMemcpyDeviceToHost, st); };
+  h2d(s.words, raw_words, n * 4); h2d(s.ev_off, event_word_offsets, (Ev + 1) * 4);
+  if (F > 1) h2d(s.fed_off, fed_offsets, Ev * (F + 1) * 4);
+  if (e != cudaSuccess) return fail_cuda(h, e, "host->device copy");
+  pix_digis dd{s.d_module, s.d_row, s.d_col, s.d_charge, s.d_clus, s.d_status};
+  pix_clusters dc{s.c_module, s.c_first, s.c_npix, s.c_charge, s.c_x, s.c_y, s.module_first, s.module_end, s.clus_module_start, s.summary};
+  if (int rc = pix_process_batch(h, cuda_stream, n_events, s.words, n_words_total, s.ev_off, F > 1 ? s.fed_off : nullptr, &dd, &dc)) return rc;
+  d2h(od->module, s.d_module, n * 2); d2h(od->row, s.d_row, n * 2); d2h(od->col, s.d_col, n * 2);
+  d2h(od->charge, s.d_charge, n * 4); d2h(od->clus, s.d_clus, n * 4); d2h(od->status, s.d_status, n);
+  d2h(oc->module, s.c_module, Ev * K * 2); d2h(oc->first_digi, s.c_first, Ev * K * 4); d2h(oc->n_pix, s.c_npix, Ev * K * 4);
+  d2h(oc->charge, s.c_charge, Ev * K * 4); d2h(oc->x_col, s.c_x, Ev * K * 4); d2h(oc->y_row, s.c_y, Ev * K * 4);
+  d2h(oc->module_first, s.module_first, Ev * M * 4); d2h(oc->module_end, s.module_end, Ev * M * 4);
+  d2h(oc->clus_module_start, s.clus_module_start, Ev * (M + 1) * 4); d2h(oc->summary, s.summary, Ev * 16 * 4);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail_cuda(h, e, "device->host copy");
+  return PIX_OK;
+}
+
+int pix_set_profiling(pix_handle* h, int enable) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  h->profiling = enable != 0;
+  h->prof_used = 0;
+  return PIX_OK;
+}
+
+int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out) {
+  if (!h || !ms_out) return PIX_ERR_INVALID_ARG;
+  for (int k = 0; k < 8; ++k) ms_out[k] = 0.0f;
+  const size_t nch = h->prof_used / 9;
+  for (size_t q = 0; q < nch; ++q) {
+    cudaEvent_t* ev = h->prof_events.data() + q * 9;
+    cudaError_t e = cudaEventSynchronize(ev[8]);
+    for (int k = 0; k < 8 && e == cudaSuccess; ++k) {
+      float ms = 0.0f;
+      e = cudaEventElapsedTime(&ms, ev[k], ev[k + 1]);
+      ms_out[k] += ms;
+    }
+    if (e != cudaSuccess) return fail_cuda(h, e, "pix_read_profile");
+  }
+  if (n_chunks_out) *n_chunks_out = (uint32_t)nch;
+  h->prof_used = 0;
+  return PIX_OK;
+}
+
+uint64_t pix_kernel_launches(const pix_handle* h) { return h ? h->launches : 0; }
+
+const char* pix_last_error(const pix_handle* h) { return h ? h->err.c_str() : "invalid handle"; }
+
+}  // extern "C"

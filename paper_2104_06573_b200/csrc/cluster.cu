@@ -1,0 +1,407 @@
+// cluster.cu -- a4 findClus fused with a5 (cluster sums, charge cut, renumber, temp records).
+//
+// "clusters the pixels on each detector module".  The connectivity rule, the duplicate rule,
+// the canonical numbering and the charge cut are DESIGN.md readings S9, S10, S13, S14, S18.
+//
+// One task = one (event, module) run [first, end) of digis.  Per task:
+//   0  clear the position hash (2n slots)
+//   1  stage (position, charge) of every digi; insert decodable digis into the hash keyed by
+//      row*416+col; equal keys keep the MIN digi index (S10: first index wins)
+//   2  a digi that is not the owner of its position is a DUPLICATE
+//   3  every live digi (owner, charge >= threshold) looks up its 4 forward neighbours
+//      (r,c+1) (r+1,c-1) (r+1,c) (r+1,c+1) and unites with live owners: lock-free union-find,
+//      larger root hooked under smaller root with atomicMin => the root is the component's min digi index
+//   4  flatten labels; add charge, pixel count and charge-weighted col/row into the root's accumulators
+//   5  roots in digi order: Q >= cut survives and takes the next local id (ballot/popc scan); the root
+//      writes the temp record at (run first + id)
+//   6  per digi: final status and clus; per task: counts
+// Four size classes share this code: the group is a warp or a block, the tables sit in shared or global memory.
+#include "pix_common.cuh"
+
+namespace pix {
+
+namespace {
+
+constexpr uint32_t LIVE = 0x80000000u, KEYMASK = 0x0001FFFFu, NOPOS = 0xFFFFFFFFu;
+constexpr uint32_t HASH_MUL = 0x9E3779B1u;
+
+// ------------------------------------------------------------------ hash slots
+template <typename SlotT> struct SlotOps;
+template <> struct SlotOps<uint32_t> {  // key 17 bits | index 15 bits  (n <= 32767)
+  static constexpr uint32_t EMPTY = 0xFFFFFFFFu;
+  static __device__ __forceinline__ uint32_t pack(uint32_t key, uint32_t k) { return (key << 15) | k; }
+  static __device__ __forceinline__ uint32_t key(uint32_t v) { return v >> 15; }
+  static __device__ __forceinline__ uint32_t idx(uint32_t v) { return v & 0x7FFFu; }
+};
+template <> struct SlotOps<unsigned long long> {
+  static constexpr unsigned long long EMPTY = ~0ull;
+  static __device__ __forceinline__ unsigned long long pack(uint32_t key, uint32_t k) {
+    return ((unsigned long long)key << 32) | k;
+  }
+  static __device__ __forceinline__ uint32_t key(unsigned long long v) { return (uint32_t)(v >> 32); }
+  static __device__ __forceinline__ uint32_t idx(unsigned long long v) { return (uint32_t)v; }
+};
+
+__device__ __forceinline__ uint32_t hash_slot(uint32_t key, uint32_t size) { return __umulhi(key * HASH_MUL, size); }
+
+template <typename SlotT>
+__device__ __forceinline__ void hash_insert(SlotT* tab, uint32_t size, uint32_t key, uint32_t k) {
+  using O = SlotOps<SlotT>;
+  const SlotT mine = O::pack(key, k);
+  uint32_t s = hash_slot(key, size);
+  while (true) {
+    const SlotT old = atomicCAS(tab + s, O::EMPTY, mine);
+    if (old == O::EMPTY) return;
+    if (O::key(old) == key) { atomicMin(tab + s, mine); return; }  // same position: min index owns it (S10)
+    if (++s == size) s = 0;
+  }
+}
+
+// owner index of position `key`, or NO_INDEX
+template <typename SlotT>
+__device__ __forceinline__ uint32_t hash_find(const SlotT* tab, uint32_t size, uint32_t key) {
+  using O = SlotOps<SlotT>;
+  uint32_t s = hash_slot(key, size);
+  while (true) {
+    const SlotT v = tab[s];
+    if (v == O::EMPTY) return NO_INDEX;
+    if (O::key(v) == key) return O::idx(v);
+    if (++s == size) s = 0;
+  }
+}
+
+// ------------------------------------------------------------------ union-find (labels strictly decrease along parents)
+__device__ __forceinline__ uint32_t uf_find(volatile uint32_t* L, uint32_t x) {
+  uint32_t p = L[x];
+  while (p != x) {
+    const uint32_t gp = L[p];
+    if (gp != p) L[x] = gp;  // path halving; a racing hook only ever lowers a parent inside the same component
+    x = p; p = gp;
+  }
+  return x;
+}
+// read-only walk to the root (step 4: own entries are being flattened concurrently, nobody else's may be written)
+__device__ __forceinline__ uint32_t uf_root(const volatile uint32_t* L, uint32_t x) {
+  uint32_t p = L[x];
+  while (p != x) { x = p; p = L[x]; }
+  return x;
+}
+__device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
+  while (true) {
+    a = uf_find(L, a); b = uf_find(L, b);
+    if (a == b) return;
+    if (a < b) { const uint32_t t = a; a = b; b = t; }
+    const uint32_t old = atomicMin(L + a, b);  // hook the larger root under the smaller
+    if (old == a) return;
+    a = old;                                   // a was no longer a root: keep merging its parent with b
+  }
+}
+
+// ------------------------------------------------------------------ groups
+struct WarpGroup {
+  uint32_t lane;
+  __device__ __forceinline__ uint32_t rank() const { return lane; }
+  __device__ __forceinline__ uint32_t size() const { return 32u; }
+  __device__ __forceinline__ void sync() const { __syncwarp(); }
+  // exclusive scan of a flag over the group + total
+  __device__ __forceinline__ uint32_t scan_flag(bool f, uint32_t& total) const {
+    const uint32_t b = __ballot_sync(0xFFFFFFFFu, f);
+    total = __popc(b);
+    return __popc(b & ((1u << lane) - 1u));
+  }
+  __device__ __forceinline__ uint32_t sum(uint32_t v) const { return __reduce_add_sync(0xFFFFFFFFu, v); }
+};
+
+template <int THREADS>
+struct BlockGroup {
+  uint32_t* s_scan;  // [THREADS/32 + 1] shared scratch
+  __device__ __forceinline__ uint32_t rank() const { return threadIdx.x; }
+  __device__ __forceinline__ uint32_t size() const { return THREADS; }
+  __device__ __forceinline__ void sync() const { __syncthreads(); }
+  __device__ __forceinline__ uint32_t scan_flag(bool f, uint32_t& total) const {
+    const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    const uint32_t b = __ballot_sync(0xFFFFFFFFu, f);
+    __syncthreads();  // previous use of s_scan is over
+    if (lane == 0) s_scan[w] = __popc(b);
+    __syncthreads();
+    uint32_t base = 0, tot = 0;
+#pragma unroll
+    for (int q = 0; q < THREADS / 32; ++q) { const uint32_t v = s_scan[q]; if (q < (int)w) base += v; tot += v; }
+    total = tot;
+    return base + __popc(b & ((1u << lane) - 1u));
+  }
+  __device__ __forceinline__ uint32_t sum(uint32_t v) const {
+    const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    v = __reduce_add_sync(0xFFFFFFFFu, v);
+    __syncthreads();
+    if (lane == 0) s_scan[w] = v;
+    __syncthreads();
+    uint32_t tot = 0;
+#pragma unroll
+    for (int q = 0; q < THREADS / 32; ++q) tot += s_scan[q];
+    return tot;
+  }
+};
+
+// tables of one task
+template <typename SlotT>
+struct Tables {
+  SlotT* tab;                 // [2n]
+  uint32_t* pos;              // [n] key | LIVE, or NOPOS for undecodable words
+  int32_t* chg;               // [n]
+  uint32_t* label;            // [n]
+  uint32_t* q;                // [n] charge sum of the root; after step 5: local id or NO_INDEX
+  uint32_t* npix;             // [n]
+  unsigned long long* sx;     // [n] sum charge*col
+  unsigned long long* sy;     // [n] sum charge*row
+};
+
+// ------------------------------------------------------------------ the task
+template <typename G, typename SlotT, bool STAGE_CHARGE>
+__device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const Tables<SlotT>& T, uint32_t task) {
+  using O = SlotOps<SlotT>;
+  const uint32_t er = task / c.M, m = task - er * c.M;
+  const size_t mo = (size_t)(c.e0 + er) * c.M + m;
+  const uint32_t first = c.module_first[mo], n = c.module_end[mo] - first;
+  const uint32_t ebase = c.segB[er * c.F];           // global index of the event's word 0
+  const size_t gb = (size_t)ebase + first;           // global index of the run's digi 0
+  const uint32_t rb = ebase - c.segB[0] + first;     // chunk-relative index of the run's digi 0
+  const uint32_t size = 2u * n;
+  const uint32_t rk = g.rank(), gs = g.size();
+
+  // 0: clear
+  for (uint32_t s = rk; s < size; s += gs) T.tab[s] = O::EMPTY;
+  g.sync();
+  // 1: stage + insert
+  for (uint32_t k = rk; k < n; k += gs) {
+    const uint32_t row = c.d_row[gb + k], col = c.d_col[gb + k];
+    const int32_t e = c.d_charge[gb + k];
+    uint32_t p = NOPOS;
+    if (row != 0xFFFFu) {
+      const uint32_t key = row * COLS + col;
+      p = key | (e >= c.thr ? LIVE : 0u);
+      hash_insert(T.tab, size, key, k);
+    }
+    T.pos[k] = p;
+    if (STAGE_CHARGE) T.chg[k] = e;
+    T.label[k] = k; T.q[k] = 0u; T.npix[k] = 0u; T.sx[k] = 0ull; T.sy[k] = 0ull;
+  }
+  g.sync();
+  // 2: duplicates
+  uint32_t n_dup = 0, n_below = 0;
+  for (uint32_t k = rk; k < n; k += gs) {
+    const uint32_t p = T.pos[k];
+    if (p == NOPOS) continue;
+    if (hash_find(T.tab, size, p & KEYMASK) != k) { T.pos[k] = (p & KEYMASK) | 0x40000000u; ++n_dup; }  // not live
+    else if (!(p & LIVE)) ++n_below;
+  }
+  g.sync();
+  // 3: unions over forward neighbours (S13: max(|drow|,|dcol|) == 1, no wrap)
+  for (uint32_t k = rk; k < n; k += gs) {
+    const uint32_t p = T.pos[k];
+    if (p == NOPOS || !(p & LIVE)) continue;
+    const uint32_t key = p & KEYMASK;
+    const uint32_t row = key / COLS, col = key - row * COLS;
+    const bool right = col + 1u < COLS, left = col > 0u, down = row + 1u < ROWS;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const bool ok = q == 0 ? right : (q == 1 ? (down && left) : (q == 2 ? down : (down && right)));
+      if (!ok) continue;
+      const uint32_t nkey = q == 0 ? key + 1u : key + COLS + (uint32_t)(q - 2);
+      const uint32_t j = hash_find(T.tab, size, nkey);
+      if (j == NO_INDEX) continue;
+      if (!(((volatile uint32_t*)T.pos)[j] & LIVE)) continue;
+      uf_unite(T.label, k, j);
+    }
+  }
+  g.sync();
+  // 4: flatten + accumulate
+  for (uint32_t k = rk; k < n; k += gs) {
+    const uint32_t p = T.pos[k];
+    if (p == NOPOS || !(p & LIVE)) continue;
+    const uint32_t r = uf_root(T.label, k);
+    T.label[k] = r;
+    const uint32_t key = p & KEYMASK;
+    const uint32_t row = key / COLS, col = key - row * COLS;
+    const uint32_t e = (uint32_t)(STAGE_CHARGE ? T.chg[k] : c.d_charge[gb + k]);
+    atomicAdd(T.q + r, e);
+    atomicAdd(T.npix + r, 1u);
+    atomicAdd(T.sx + r, (unsigned long long)e * col);
+    atomicAdd(T.sy + r, (unsigned long long)e * row);
+  }
+  g.sync();
+  // 5: roots in digi order -> local ids (S14), temp records (S18)
+  uint32_t n_pre = 0, n_post = 0;
+  for (uint32_t k0 = 0; k0 < n; k0 += gs) {
+    const uint32_t k = k0 + rk;
+    bool root = false, surv = false;
+    uint32_t Q = 0;
+    if (k < n) {
+      const uint32_t p = T.pos[k];
+      root = p != NOPOS && (p & LIVE) && T.label[k] == k;
+      if (root) { Q = T.q[k]; surv = (long long)Q >= (long long)c.cut; }  // S9: equality keeps
+    }
+    uint32_t tot_pre, tot_post;
+    (void)g.scan_flag(root, tot_pre);
+    const uint32_t id = n_post + g.scan_flag(surv, tot_post);
+    if (root) {
+      if (surv) {
+        const uint32_t o = rb + id;
+        c.t_first[o] = first + k; c.t_npix[o] = T.npix[k]; c.t_charge[o] = Q;
+        c.t_x[o] = (float)((double)T.sx[k] / (double)Q);
+        c.t_y[o] = (float)((double)T.sy[k] / (double)Q);
+      }
+      T.q[k] = surv ? id : NO_INDEX;
+    }
+    n_pre += tot_pre; n_post += tot_post;
+  }
+  g.sync();
+  // 6: final status and clus of every decodable digi (undecodable ones were finished by unpack)
+  uint32_t n_ok = 0, n_cut = 0;
+  for (uint32_t k = rk; k < n; k += gs) {
+    const uint32_t p = T.pos[k];
+    if (p == NOPOS) {
+      if (!STAGE_CHARGE) c.d_clus[gb + k] = -1;  // global class: the labels lived in clus, restore unpack's -1
+      continue;
+    }
+    int32_t clus = -1;
+    uint8_t st;
+    if (p & LIVE) {
+      const uint32_t id = T.q[T.label[k]];
+      if (id != NO_INDEX) { clus = (int32_t)id; st = ST_OK; ++n_ok; } else { st = ST_CUT; ++n_cut; }
+    } else {
+      st = (p & 0x40000000u) ? ST_DUP : ST_BELOW;
+    }
+    c.d_clus[gb + k] = clus;
+    c.d_status[gb + k] = st;
+  }
+  n_dup = g.sum(n_dup); n_below = g.sum(n_below); n_ok = g.sum(n_ok); n_cut = g.sum(n_cut);
+  if (rk == 0) {
+    c.n_clus[task] = n_post;
+    uint32_t* mc = c.mod_cnt + (size_t)task * MC_STRIDE;
+    mc[MC_PRECUT] = n_pre; mc[MC_DUP] = n_dup; mc[MC_BELOW] = n_below; mc[MC_OK] = n_ok; mc[MC_CUT] = n_cut;
+  }
+}
+
+template <typename SlotT>
+__device__ __forceinline__ Tables<SlotT> carve(unsigned char* base, uint32_t cap) {
+  Tables<SlotT> T;
+  T.sx = reinterpret_cast<unsigned long long*>(base); base += (size_t)cap * 8;
+  T.sy = reinterpret_cast<unsigned long long*>(base); base += (size_t)cap * 8;
+  T.tab = reinterpret_cast<SlotT*>(base); base += (size_t)cap * 2 * sizeof(SlotT);
+  T.pos = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
+  T.chg = reinterpret_cast<int32_t*>(base); base += (size_t)cap * 4;
+  T.label = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
+  T.q = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
+  T.npix = reinterpret_cast<uint32_t*>(base);
+  return T;
+}
+constexpr size_t smem_per_digi = 8 + 8 + 2 * 4 + 4 * 5;  // 44 bytes
+
+// ------------------------------------------------------------------ kernels
+constexpr int WARP_TIER_THREADS = 256;
+__global__ void __launch_bounds__(WARP_TIER_THREADS) cluster_warp_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const Tables<uint32_t> T = carve<uint32_t>(smem + (size_t)warp * TIER_WARP_MAX * smem_per_digi, TIER_WARP_MAX);
+  const WarpGroup g{lane};
+  const uint32_t count = c.ctl[0];
+  const uint32_t* list = c.lists;
+  while (true) {
+    uint32_t t = 0;
+    if (lane == 0) t = atomicAdd(c.ctl + 4, 1u);
+    t = __shfl_sync(0xFFFFFFFFu, t, 0);
+    if (t >= count) break;
+    cluster_task<WarpGroup, uint32_t, true>(c, g, T, list[t]);
+    __syncwarp();
+  }
+}
+
+template <int THREADS, int TIER, uint32_t CAP>
+__global__ void __launch_bounds__(THREADS) cluster_block_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ uint32_t s_scan[THREADS / 32 + 1];
+  __shared__ uint32_t s_task;
+  const Tables<uint32_t> T = carve<uint32_t>(smem, CAP);
+  const BlockGroup<THREADS> g{s_scan};
+  const uint32_t count = c.ctl[TIER];
+  const uint32_t* list = c.lists + (size_t)TIER * c.list_stride;
+  while (true) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + 4 + TIER, 1u);
+    __syncthreads();
+    const uint32_t t = s_task;
+    if (t >= count) break;
+    cluster_task<BlockGroup<THREADS>, uint32_t, true>(c, g, T, list[t]);
+  }
+}
+
+constexpr int GLOBAL_TIER_THREADS = 512;
+__global__ void __launch_bounds__(GLOBAL_TIER_THREADS) cluster_global_kernel(const __grid_constant__ Chunk c) {
+  __shared__ uint32_t s_scan[GLOBAL_TIER_THREADS / 32 + 1];
+  __shared__ uint32_t s_task;
+  const BlockGroup<GLOBAL_TIER_THREADS> g{s_scan};
+  const uint32_t count = c.ctl[3];
+  const uint32_t* list = c.lists + (size_t)3 * c.list_stride;
+  while (true) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + 7, 1u);
+    __syncthreads();
+    const uint32_t t = s_task;
+    if (t >= count) break;
+    const uint32_t task = list[t];
+    const uint32_t er = task / c.M, m = task - er * c.M;
+    const uint32_t first = c.module_first[(size_t)(c.e0 + er) * c.M + m];
+    const uint32_t ebase = c.segB[er * c.F];
+    const uint32_t rb = ebase - c.segB[0] + first;
+    Tables<unsigned long long> T;
+    T.tab = c.g_hash + 2 * (size_t)rb;
+    T.pos = c.g_pos + rb; T.chg = nullptr;
+    T.label = reinterpret_cast<uint32_t*>(c.d_clus + (size_t)ebase + first);  // clus is written last, per digi
+    T.q = c.g_q + rb; T.npix = c.g_npix + rb; T.sx = c.g_sx + rb; T.sy = c.g_sy + rb;
+    cluster_task<BlockGroup<GLOBAL_TIER_THREADS>, unsigned long long, false>(c, g, T, task);
+  }
+}
+
+constexpr int SMALL_THREADS = 128, LARGE_THREADS = 512;
+constexpr size_t SMEM_WARP = (size_t)(WARP_TIER_THREADS / 32) * TIER_WARP_MAX * smem_per_digi;
+constexpr size_t SMEM_SMALL = (size_t)TIER_SMALL_MAX * smem_per_digi;
+constexpr size_t SMEM_LARGE = (size_t)TIER_LARGE_MAX * smem_per_digi;
+
+}  // namespace
+
+cudaError_t configure_cluster_kernels() {
+  cudaError_t e;
+  e = cudaFuncSetAttribute(cluster_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_WARP);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(cluster_block_kernel<SMALL_THREADS, 1, TIER_SMALL_MAX>,
+                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_SMALL);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(cluster_block_kernel<LARGE_THREADS, 2, TIER_LARGE_MAX>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LARGE);
+}
+
+static inline int clampi(uint64_t v, int lo, int hi) { return (int)(v < (uint64_t)lo ? lo : (v > (uint64_t)hi ? hi : v)); }
+
+// Persistent grids: every block pulls tasks from its class's list with an atomic ticket; the list lengths
+// live in device memory, so the grid is sized from host-side bounds only (legal during stream capture).
+void launch_cluster(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream, cudaEvent_t* ev) {
+  const uint64_t n_tasks = (uint64_t)(c.e1 - c.e0) * c.M;
+  const uint64_t wb = words_bound ? words_bound : 1;
+  // a class-q task has more than TIER_(q-1)_MAX words, so at most words/TIER_(q-1)_MAX tasks exist
+  const uint64_t bound1 = wb / TIER_WARP_MAX + 1, bound2 = wb / TIER_SMALL_MAX + 1, bound3 = wb / TIER_LARGE_MAX + 1;
+  const int g0 = clampi((n_tasks + 7) / 8, 1, n_sm * 5);
+  const int g1 = clampi(bound1 < n_tasks ? bound1 : n_tasks, 1, n_sm * 6);
+  const int g2 = clampi(bound2 < n_tasks ? bound2 : n_tasks, 1, n_sm);
+  const int g3 = clampi(bound3 < n_tasks ? bound3 : n_tasks, 1, n_sm * 2);
+  cluster_global_kernel<<<g3, GLOBAL_TIER_THREADS, 0, stream>>>(c);
+  if (ev) cudaEventRecord(ev[0], stream);
+  cluster_block_kernel<LARGE_THREADS, 2, TIER_LARGE_MAX><<<g2, LARGE_THREADS, SMEM_LARGE, stream>>>(c);
+  if (ev) cudaEventRecord(ev[1], stream);
+  cluster_block_kernel<SMALL_THREADS, 1, TIER_SMALL_MAX><<<g1, SMALL_THREADS, SMEM_SMALL, stream>>>(c);
+  if (ev) cudaEventRecord(ev[2], stream);
+  cluster_warp_kernel<<<g0, WARP_TIER_THREADS, SMEM_WARP, stream>>>(c);
+  if (ev) cudaEventRecord(ev[3], stream);
+}
+
+}  // namespace pix

@@ -1,0 +1,126 @@
+// finalize.cu -- a6 cluster offsets (Fig. 3, lines 76-81: moduleStart[i+1] = min(maxHitsInModule(),
+// cluStart[i]), followed by the prefix sum the figure leaves implicit, S19), the scatter of the temp
+// cluster records to their final place clus_module_start[module] + local id (S14), and the summary (S20).
+//
+// Grid (NB, events of the chunk).  Every block of an event recomputes the event's M-entry scan in shared
+// memory (warp-shuffle scan; a few KB), then copies a slice of the records: one thread per output record,
+// module found by binary search in the shared offsets.  Block 0 also writes the offsets and the summary.
+#include "pix_common.cuh"
+
+namespace pix {
+
+namespace {
+
+constexpr int FIN_THREADS = 256;
+
+__device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, uint32_t lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, v, d);
+    if (lane >= (uint32_t)d) v += t;
+  }
+  return v;
+}
+
+__global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ uint32_t s_start[];  // [M+1]
+  __shared__ uint32_t s_warp[FIN_THREADS / 32];
+  __shared__ uint32_t s_red[8];
+  const uint32_t er = blockIdx.y, e = c.e0 + er, M = c.M;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t flags = c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS];
+  const bool skip = (flags & FLAG_NONCONTIGUOUS) != 0;  // S11: clustering is not defined for such an event
+  const uint32_t* n_clus = c.n_clus + (size_t)er * M;
+
+  // ---- Fig. 3 clamp + exclusive prefix sum over the M modules
+  const uint32_t ipt = (M + FIN_THREADS - 1) / FIN_THREADS;
+  const uint32_t m0 = tid * ipt, m1 = (m0 + ipt < M) ? m0 + ipt : M;
+  uint32_t local = 0;
+  for (uint32_t m = m0; m < m1; ++m) {
+    const uint32_t n = skip ? 0u : n_clus[m];
+    local += n < c.cap_mod ? n : c.cap_mod;
+  }
+  const uint32_t incl = warp_inclusive_scan(local, lane);
+  if (lane == 31) s_warp[warp] = incl;
+  if (tid < 8) s_red[tid] = 0u;
+  __syncthreads();
+  uint32_t base = incl - local;
+  for (uint32_t w = 0; w < warp; ++w) base += s_warp[w];
+  for (uint32_t m = m0; m < m1; ++m) {
+    s_start[m] = base;
+    const uint32_t n = skip ? 0u : n_clus[m];
+    base += n < c.cap_mod ? n : c.cap_mod;
+  }
+  if (m0 < M && m1 == M) s_start[M] = base;
+  __syncthreads();
+  const uint32_t total = s_start[M];
+  const uint32_t n_emit = total < c.cap_ev ? total : c.cap_ev;
+  const uint32_t ebase = c.segB[er * c.F];
+  const uint32_t n_words = c.segB[(er + 1u) * c.F] - ebase;
+
+  // ---- block 0: offsets + summary
+  if (blockIdx.x == 0) {
+    uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
+    for (uint32_t m = tid; m <= M; m += FIN_THREADS) cms[m] = s_start[m];
+    uint32_t acc[7] = {0, 0, 0, 0, 0, 0, 0};  // present, n_clusters, precut, dup, below, ok, cut
+    for (uint32_t m = tid; m < M; m += FIN_THREADS) {
+      acc[0] += c.module_end[(size_t)e * M + m] > 0u ? 1u : 0u;
+      acc[1] += skip ? 0u : n_clus[m];
+      const uint32_t* mc = c.mod_cnt + ((size_t)er * M + m) * MC_STRIDE;
+#pragma unroll
+      for (int k = 0; k < MC_STRIDE; ++k) acc[2 + k] += mc[k];
+    }
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+      const uint32_t v = __reduce_add_sync(0xFFFFFFFFu, acc[k]);
+      if (lane == 0 && v) atomicAdd(s_red + k, v);
+    }
+    __syncthreads();
+    if (tid == 0) {
+      const uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
+      uint32_t* s = c.summary + (size_t)e * 16;
+      const uint32_t bad = ec[EC_EMPTY] + ec[EC_ERR_LINK] + ec[EC_ERR_ROC] + ec[EC_ERR_DCOL] + ec[EC_ERR_PXID];
+      s[0] = n_words; s[1] = n_words - bad; s[2] = ec[EC_EMPTY];
+      s[3] = ec[EC_ERR_LINK]; s[4] = ec[EC_ERR_ROC]; s[5] = ec[EC_ERR_DCOL]; s[6] = ec[EC_ERR_PXID];
+      s[7] = s_red[3]; s[8] = s_red[4]; s[9] = s_red[5]; s[10] = s_red[6];
+      s[11] = s_red[0]; s[12] = s_red[2]; s[13] = s_red[1]; s[14] = n_emit;
+      s[15] = flags | (total > c.cap_ev ? FLAG_CAPACITY : 0u);
+    }
+  }
+
+  // ---- records: output record g of the event <- temp record (run first + local id)
+  const uint32_t rel = ebase - c.segB[0];
+  for (uint32_t g = blockIdx.x * FIN_THREADS + tid; g < n_emit; g += gridDim.x * FIN_THREADS) {
+    uint32_t lo = 0, hi = M;  // last m with s_start[m] <= g
+    while (lo < hi) {
+      const uint32_t mid = (lo + hi + 1u) >> 1;
+      if (s_start[mid] <= g) lo = mid; else hi = mid - 1u;
+    }
+    const uint32_t src = rel + c.module_first[(size_t)e * M + lo] + (g - s_start[lo]);
+    const size_t o = (size_t)e * c.cap_ev + g;
+    c.c_module[o] = (uint16_t)lo;
+    c.c_first[o] = c.t_first[src]; c.c_npix[o] = c.t_npix[src]; c.c_charge[o] = c.t_charge[src];
+    c.c_x[o] = c.t_x[src]; c.c_y[o] = c.t_y[src];
+  }
+
+  // ---- an event whose modules are not contiguous was not clustered: define clus for its decodable words
+  if (skip) {
+    for (uint32_t i = blockIdx.x * FIN_THREADS + tid; i < n_words; i += gridDim.x * FIN_THREADS)
+      c.d_clus[(size_t)ebase + i] = -1;
+  }
+}
+
+}  // namespace
+
+cudaError_t configure_finalize_kernel() {
+  return cudaFuncSetAttribute(finalize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
+}
+
+void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream) {
+  const uint32_t Ec = c.e1 - c.e0;
+  uint32_t nb = (uint32_t)(n_sm * 4) / Ec;
+  nb = nb < 1u ? 1u : (nb > 16u ? 16u : nb);
+  finalize_kernel<<<dim3(nb, Ec), FIN_THREADS, (size_t)(c.M + 1) * sizeof(uint32_t), stream>>>(c);
+}
+
+}  // namespace pix

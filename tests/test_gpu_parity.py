@@ -1,0 +1,85 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, element by element.  Needs a B200."""
+import numpy as np
+import pytest
+
+import pixgen
+from helpers import P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import gpu_util
+    return gpu_util
+
+
+@pytest.fixture(scope="module")
+def full():
+    return pixgen.detector("full")
+
+
+def check(gu, det, batch, params=P, kmax=None, **kw):
+    got = gu.run_batch(det, batch, params, kmax=kmax, **kw)
+    exp = gu.oracle_events(det, batch, params, kmax=kmax)
+    assert len(got) == len(exp)
+    for e, (g, o) in enumerate(zip(got, exp)):
+        gu.assert_event_equal(g, o, tag=f"event {e}")
+    return got, exp
+
+
+@pytest.mark.parametrize("mode", ["batch", "single", "host"])
+def test_cfg0_tiny(gu, mode):
+    det, b = pixgen.config("cfg0")
+    check(gu, det, b, mode=mode)
+
+
+@pytest.mark.parametrize("mode", ["batch", "single"])
+def test_cfg1_pu50_event(gu, full, mode):
+    b = pixgen.events(full, "pu50", [0])
+    got, _ = check(gu, full, b, mode=mode)
+    assert 55000 < int(got[0]["summary"][0]) < 66000
+
+
+def test_cfg2_batch_ragged_chunks(gu, full):
+    """24 PU50-like events in chunks of 5 (last chunk ragged): chunk boundaries fall inside vectors and tiles."""
+    b = pixgen.events(full, "pu50", np.arange(24))
+    check(gu, full, b, chunk_events=5)
+
+
+def test_cfg2_one_chunk(gu, full):
+    b = pixgen.events(full, "pu50", np.arange(100, 112))
+    check(gu, full, b)
+
+
+def test_cfg3_pu200(gu, full):
+    b = pixgen.events(full, "pu200", np.arange(3))
+    got, _ = check(gu, full, b, chunk_events=2)
+    assert max(int(g["c_n_pix"].max()) for g in got) >= 50
+
+
+def test_cfg4_edge_mix(gu, full):
+    """5 events of each class: dense, duplicates, invalid words, edges, degenerate (empty, one word, all bad, ...)."""
+    _, b = pixgen.config("cfg4", n_events=25)
+    got, _ = check(gu, full, b, chunk_events=4)
+    tally = b.tally.astype(np.int64)
+    for e, g in enumerate(got):
+        s = g["summary"].astype(np.int64)
+        assert np.all(s[2:7] >= tally[e])  # injected invalid words are counted exactly (>=: degenerate events add their own)
+    assert sum(int(g["summary"][7]) for g in got) > 1000     # duplicates seen
+    assert any(int(g["summary"][0]) == 0 for g in got)        # an empty event
+
+
+def test_cfg4_edge_mix_single_calls(gu, full):
+    _, b = pixgen.config("cfg4", n_events=10)
+    check(gu, full, b, mode="single")
+
+
+def test_clamp_and_capacity(gu, full):
+    b = pixgen.events(full, "pu50", [3, 4])
+    check(gu, full, b, params=dict(P, max_clusters_per_module=8))
+    got, _ = check(gu, full, b, kmax=1000)
+    assert all(int(g["summary"][15]) & 2 for g in got)
