@@ -307,11 +307,10 @@ __global__ void __launch_bounds__(WARP_TIER_THREADS) cluster_warp_kernel(const _
   const WarpGroup g{lane};
   const uint32_t count = c.ctl[0];
   const uint32_t* list = c.lists;
-  while (true) {
-    uint32_t t = 0;
-    if (lane == 0) t = atomicAdd(c.ctl + 4, 1u);
-    t = __shfl_sync(0xFFFFFFFFu, t, 0);
-    if (t >= count) break;
+  // static striding: tasks of this class are all small, and one global ticket counter would serialise
+  // millions of atomics on a single address
+  const uint32_t n_warps = gridDim.x * (WARP_TIER_THREADS / 32);
+  for (uint32_t t = blockIdx.x * (WARP_TIER_THREADS / 32) + warp; t < count; t += n_warps) {
     cluster_task<WarpGroup, uint32_t, true>(c, g, T, list[t]);
     __syncwarp();
   }
@@ -326,7 +325,14 @@ __global__ void __launch_bounds__(THREADS) cluster_block_kernel(const __grid_con
   const BlockGroup<THREADS> g{s_scan};
   const uint32_t count = c.ctl[TIER];
   const uint32_t* list = c.lists + (size_t)TIER * c.list_stride;
-  while (true) {
+  if (TIER == 1) {  // many similar tasks: static striding, no ticket traffic
+    for (uint32_t t = blockIdx.x; t < count; t += gridDim.x) {
+      __syncthreads();
+      cluster_task<BlockGroup<THREADS>, uint32_t, true>(c, g, T, list[t]);
+    }
+    return;
+  }
+  while (true) {  // few, uneven tasks: atomic ticket
     __syncthreads();
     if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + 4 + TIER, 1u);
     __syncthreads();

@@ -14,7 +14,7 @@ constexpr uint32_t TILE = UNPACK_THREADS * 4;  // one 128-bit load of 4 words pe
 constexpr uint32_t NOKEY = 0xFFFFFFFFu;
 
 // ------------------------------------------------------------------ init
-// One thread per event of the chunk builds the clamped, monotone segment table
+// One warp per event of the chunk builds the clamped, monotone segment table
 //   segB[e_rel*F + f] = global word index where FED f of event e starts,  segB[Ec*F] = end of chunk.
 // Offsets are clamped into [lo, hi] (lo = start of chunk, hi = min(n_total, lo + cap_words)) so that
 // whatever the caller's offset arrays hold, every index derived later stays inside the buffers.
@@ -27,24 +27,31 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk
   const uint32_t room = n_total - lo;
   const uint32_t hi = lo + (room < c.cap_words ? room : c.cap_words);
   if (tid < 16) c.ctl[tid] = 0;
-  for (uint32_t er = tid; er < Ec; er += nth) {
+  // one warp per event: lanes take FEDs, the running max over the clamped offsets is a warp max-scan
+  const uint32_t lane = threadIdx.x & 31u, wid = tid >> 5, nwarp = nth >> 5;
+  for (uint32_t er = wid; er < Ec; er += nwarp) {
     const uint32_t e = c.e0 + er;
-    uint32_t rb = ev_offset(c, e), re = ev_offset(c, e + 1);
-    uint32_t b = rb < lo ? lo : (rb > hi ? hi : rb);
-    uint32_t en = re < b ? b : (re > hi ? hi : re);
+    const uint32_t rb = ev_offset(c, e), re = ev_offset(c, e + 1);
+    const uint32_t b = rb < lo ? lo : (rb > hi ? hi : rb);
+    const uint32_t en = re < b ? b : (re > hi ? hi : re);
     const uint32_t nw = en - b;
-    uint32_t flags = (re > hi || rb > hi || re < rb || rb < lo) ? FLAG_TOO_LARGE : 0u;
-    uint32_t run = 0;
-    for (uint32_t f = 0; f < c.F; ++f) {
-      uint32_t fo = (f == 0 || !c.fed_off) ? 0u : c.fed_off[(size_t)e * (c.F + 1) + f];
+    const uint32_t flags = (re > hi || rb > hi || re < rb || rb < lo) ? FLAG_TOO_LARGE : 0u;
+    uint32_t carry = 0;
+    for (uint32_t f0 = 0; f0 < c.F; f0 += 32u) {
+      const uint32_t f = f0 + lane;
+      uint32_t fo = (f == 0 || f >= c.F || !c.fed_off) ? 0u : c.fed_off[(size_t)e * (c.F + 1) + f];
       fo = fo > nw ? nw : fo;
-      run = fo > run ? fo : run;  // running max keeps the table monotone
-      c.segB[er * c.F + f] = b + run;
-    }
-    if (er == Ec - 1) c.segB[Ec * c.F] = en;
-    uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
+      fo = fo > carry ? fo : carry;
 #pragma unroll
-    for (int k = 0; k < EC_STRIDE; ++k) ec[k] = (k == EC_FLAGS) ? flags : 0u;
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, fo, d);
+        if (lane >= (uint32_t)d && o > fo) fo = o;
+      }
+      if (f < c.F) c.segB[er * c.F + f] = b + fo;  // monotone by construction
+      carry = __shfl_sync(0xFFFFFFFFu, fo, 31);
+    }
+    if (er == Ec - 1 && lane == 0) c.segB[Ec * c.F] = en;
+    if (lane < EC_STRIDE) c.ev_cnt[(size_t)er * EC_STRIDE + lane] = (lane == EC_FLAGS) ? flags : 0u;
   }
   const uint32_t nmod = Ec * c.M;
   uint32_t* mf = c.module_first + (size_t)c.e0 * c.M;
