@@ -3,8 +3,8 @@
     python bench.py --gpus 1 --steps 10 --warmup 3            # this repo's CUDA path
     python bench.py --impl reference --steps 3 --warmup 1     # the oracle on the host cores (the reference arm)
 
-A step = one pass of the whole hot path (init, unpack+calibrate+boundaries, classify, cluster x4 size classes,
-finalize) over one batch of synthetic events: BASELINE.json configs[2], 1000 PU50-like events (config[1]'s
+A step = one pass of the whole hot path (init, the fused unpack+calibrate+boundaries+cluster kernel, the overflow
+kernel, finalize) over one batch of synthetic events: BASELINE.json configs[2], 1000 PU50-like events (config[1]'s
 generator, seeds 0..999), through pix_process_batch.  `value` is timed with the inputs resident in HBM; `e2e`
 goes through pix_process_batch_host with pinned HOST buffers, host<->device copies inside the timed region.
 Under torchrun (N > 1) every rank runs its own 1000 events (seeds rank*1000 ..): weak scaling, no collective
@@ -196,18 +196,10 @@ def run_ours(args):
     torch.cuda.synchronize()
     summ = clusters["summary"].cpu().numpy().reshape(E, 16).astype(np.int64)
     K = int(summ[:, 14].sum())
-    mf = clusters["module_first"].cpu().numpy().astype(np.int64)
-    me = clusters["module_end"].cpu().numpy().astype(np.int64)
-    cms = clusters["clus_module_start"].cpu().numpy().reshape(E, M + 1).astype(np.int64)
-    run_len = me - mf
-    run_clus = np.diff(cms, axis=1).reshape(-1)
-    bounds = (0, 128, 768, 4096, 1 << 30)
-    names = ("cluster_warp", "cluster_small", "cluster_large", "cluster_global")
-    kernel_bytes = {"unpack": 15 * W, "finalize": 42 * K + (4 * (M + 1) + 64 + 4 * M) * E,
-                    "init": 8 * M * E, "classify": (8 + 4 + 20) * M * E}
-    for q, nm in enumerate(names):
-        sel = (run_len > bounds[q]) & (run_len <= bounds[q + 1])
-        kernel_bytes[nm] = int(13 * run_len[sel].sum() + 20 * run_clus[sel].sum())
+    # algorithmic bytes per kernel: fused reads the raw word and writes the 15 B digi and the
+    # 20 B temp record; finalize moves the records (20 B in, 22 B out) and writes the per-event arrays
+    kernel_bytes = {"init": 12 * M * E, "fused": 19 * W + 20 * K, "overflow": 0,
+                    "finalize": 42 * K + (4 * (M + 1) + 64 + 4 * M) * E}
     top = max(prof, key=prof.get)
     peak, peak_src = peak_hbm()
     top_launches = chunks_per_step

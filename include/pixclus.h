@@ -150,10 +150,14 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
 /* Number of CUDA kernels this handle has launched so far (for launch accounting). */
 uint64_t pix_kernel_launches(const pix_handle* h);
 
+/* Diagnostic: module runs the LAST internal chunk of the last call left to the overflow kernel (runs longer than the
+ * fused kernel's window, pathological charge sums).  Synchronises the device; not for the hot path. */
+int pix_overflow_runs(pix_handle* h, uint32_t* out);
+
 /* Optional per-kernel timing for benchmarks (not legal during stream capture).  While enabled, every chunk
  * records CUDA events between its kernels on the caller's stream.  pix_read_profile waits for them and adds up
- * the device time per kernel family since the last read: ms_out[8] = {init, unpack, classify, cluster_global,
- * cluster_large, cluster_small, cluster_warp, finalize}; *n_chunks_out = chunks covered. */
+ * the device time per kernel since the last read: ms_out[8] = {init, fused, overflow, finalize, 0, 0, 0, 0};
+ * *n_chunks_out = chunks covered. */
 int pix_set_profiling(pix_handle* h, int enable);
 int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out);
 

@@ -24,7 +24,7 @@ SUMMARY = ("n_words", "n_decoded", "n_empty", "n_err_link", "n_err_roc", "n_err_
            "n_clusters_emitted", "flags")
 FLAG_NONCONTIGUOUS, FLAG_CLUSTER_CAPACITY_OVERFLOW, FLAG_EVENT_TOO_LARGE = 1, 2, 4
 EXPORTS = ("pix_create", "pix_clone", "pix_destroy", "pix_process", "pix_process_batch", "pix_process_batch_host",
-           "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile")
+           "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile", "pix_overflow_runs")
 
 _vp, _u32 = ctypes.c_void_p, ctypes.c_uint32
 
@@ -81,6 +81,8 @@ def load() -> ctypes.CDLL:
         lib.pix_set_profiling.restype = ctypes.c_int
         lib.pix_read_profile.argtypes = [_vp, pp(ctypes.c_float), pp(_u32)]
         lib.pix_read_profile.restype = ctypes.c_int
+        lib.pix_overflow_runs.argtypes = [_vp, pp(_u32)]
+        lib.pix_overflow_runs.restype = ctypes.c_int
         lib.pix_last_error.argtypes = [_vp]
         lib.pix_last_error.restype = ctypes.c_char_p
         _lib = lib
@@ -164,8 +166,16 @@ def pix_kernel_launches(h: Handle) -> int:
     return int(load().pix_kernel_launches(h.ptr))
 
 
-KERNEL_FAMILIES = ("init", "unpack", "classify", "cluster_global", "cluster_large", "cluster_small", "cluster_warp",
-                   "finalize")
+def pix_overflow_runs(h: Handle) -> int:
+    """Diagnostic: runs the last internal chunk left to the overflow kernel (synchronises the device)."""
+    n = (_u32 * 8)()
+    rc = load().pix_overflow_runs(h.ptr, ctypes.cast(n, ctypes.POINTER(_u32)))
+    if rc != PIX_OK:
+        raise PixError(rc, pix_last_error(h))
+    return list(n)
+
+
+KERNEL_FAMILIES = ("init", "fused", "overflow", "finalize")
 
 
 def pix_set_profiling(h: Handle, enable: bool) -> None:

@@ -14,7 +14,7 @@ namespace {
 
 struct SharedTables {  // read-only device tables shared by clones
   std::atomic<int> refs{1};
-  uint32_t* cab = nullptr;
+  pix::CabEntry* cab = nullptr;
   float2* gp = nullptr;
 };
 
@@ -44,7 +44,7 @@ struct pix_handle {
   std::string err;
   HostStage hs;
   bool profiling = false;
-  std::vector<cudaEvent_t> prof_events;  // 9 per chunk, in launch order
+  std::vector<cudaEvent_t> prof_events;  // LAUNCHES_PER_CHUNK + 1 per chunk, in launch order
   size_t prof_used = 0;
 };
 
@@ -69,11 +69,10 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   pix::Chunk& c = h->proto;
   c.segB = (uint32_t*)take((Ec * F + 1) * 4);
   c.ev_cnt = (uint32_t*)take(Ec * pix::EC_STRIDE * 4);
-  c.ctl = (uint32_t*)take(16 * 4);
-  c.lists = (uint32_t*)take((size_t)pix::N_TIERS * Ec * M * 4);
-  c.list_stride = (uint32_t)(Ec * M);
+  c.ctl = (uint32_t*)take(pix::CTL_WORDS * 4);
+  c.ovf_list = (uint32_t*)take(Ec * M * 4);
+  c.ovf_cap = (uint32_t)(Ec * M);
   c.n_clus = (uint32_t*)take(Ec * M * 4);
-  c.mod_cnt = (uint32_t*)take(Ec * M * pix::MC_STRIDE * 4);
   c.t_first = (uint32_t*)take(W * 4); c.t_npix = (uint32_t*)take(W * 4); c.t_charge = (uint32_t*)take(W * 4);
   c.t_x = (float*)take(W * 4); c.t_y = (float*)take(W * 4);
   c.g_hash = (unsigned long long*)take(W * 16);
@@ -119,27 +118,27 @@ void bind_outputs(pix::Chunk& c, const pix_digis* d, const pix_clusters* k) {
 }
 
 // the launch sequence of one chunk
+constexpr int PROF_EVENTS = pix::LAUNCHES_PER_CHUNK + 1;
 int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t words_bound, cudaStream_t s) {
   cudaEvent_t* ev = nullptr;
   if (h->profiling) {
-    while (h->prof_events.size() < h->prof_used + 9) {
+    while (h->prof_events.size() < h->prof_used + PROF_EVENTS) {
       cudaEvent_t x;
       if (cudaEventCreate(&x) != cudaSuccess) return fail(h, PIX_ERR_ALLOC, "cudaEventCreate");
       h->prof_events.push_back(x);
     }
     ev = h->prof_events.data() + h->prof_used;
-    h->prof_used += 9;
+    h->prof_used += PROF_EVENTS;
     cudaEventRecord(ev[0], s);
   }
   pix::launch_init(c, n_total, h->n_sm, s);
   if (ev) cudaEventRecord(ev[1], s);
-  pix::launch_unpack(c, words_bound, h->n_sm, s);
+  pix::launch_fused(c, words_bound, h->n_sm, s);
   if (ev) cudaEventRecord(ev[2], s);
-  pix::launch_classify(c, h->n_sm, s);
+  pix::launch_overflow(c, h->n_sm, s);
   if (ev) cudaEventRecord(ev[3], s);
-  pix::launch_cluster(c, words_bound, h->n_sm, s, ev ? ev + 4 : nullptr);
   pix::launch_finalize(c, h->n_sm, s);
-  if (ev) cudaEventRecord(ev[8], s);
+  if (ev) cudaEventRecord(ev[4], s);
   h->launches += pix::LAUNCHES_PER_CHUNK;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
@@ -165,7 +164,7 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   h->F = F; h->M = M; h->p = *params;
   cudaError_t e = cudaGetDevice(&h->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
-  if (e == cudaSuccess) e = pix::configure_cluster_kernels();
+  if (e == cudaSuccess) e = pix::configure_fused_kernel();
   if (e == cudaSuccess) e = pix::configure_finalize_kernel();
   if (e != cudaSuccess) { delete h; cudaGetLastError(); return PIX_ERR_CUDA; }
 
@@ -187,8 +186,18 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   const size_t ncab = (size_t)F * 64 * 32, ngp = (size_t)M * PIX_COLS;
   std::vector<float2> gp(ngp);
   for (size_t i = 0; i < ngp; ++i) gp[i] = make_float2(gains->gain[i], gains->pedestal[i]);
-  bool ok = cudaMalloc(&t->cab, ncab * 4) == cudaSuccess && cudaMalloc(&t->gp, ngp * sizeof(float2)) == cudaSuccess;
-  ok = ok && cudaMemcpy(t->cab, cabling->entry, ncab * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+  // cabling re-laid out so that a decode is one 8-byte gather and two multiply-adds (pix_common.cuh; reading S3)
+  std::vector<pix::CabEntry> cab(ncab);
+  for (size_t i = 0; i < ncab; ++i) {
+    const uint32_t e = cabling->entry[i];
+    const uint32_t bad = !(e & 1u) ? PIX_ST_ERR_LINK : (!(e & 2u) ? PIX_ST_ERR_ROC : 0u);
+    const uint32_t rocx = (e >> 18) & 7u, rocy = (e >> 21) & 1u, flip_r = (e >> 22) & 1u, flip_c = (e >> 23) & 1u;
+    const uint32_t row0 = rocy * 80u + (flip_r ? 79u : 0u), col0 = rocx * 52u + (flip_c ? 51u : 0u);
+    cab[i].x = ((e >> 2) & 0xFFFFu) | (bad << 16) | ((flip_c ? 0xFFu : 0x01u) << 24);
+    cab[i].y = row0 | (col0 << 8) | ((flip_r ? 0xFFu : 0x01u) << 24);
+  }
+  bool ok = cudaMalloc(&t->cab, ncab * sizeof(pix::CabEntry)) == cudaSuccess && cudaMalloc(&t->gp, ngp * sizeof(float2)) == cudaSuccess;
+  ok = ok && cudaMemcpy(t->cab, cab.data(), ncab * sizeof(pix::CabEntry), cudaMemcpyHostToDevice) == cudaSuccess;
   ok = ok && cudaMemcpy(t->gp, gp.data(), ngp * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess;
   if (!ok) { cudaGetLastError(); release_tables(t); delete h; return PIX_ERR_ALLOC; }
 
@@ -329,11 +338,11 @@ int pix_set_profiling(pix_handle* h, int enable) {
 int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out) {
   if (!h || !ms_out) return PIX_ERR_INVALID_ARG;
   for (int k = 0; k < 8; ++k) ms_out[k] = 0.0f;
-  const size_t nch = h->prof_used / 9;
+  const size_t nch = h->prof_used / PROF_EVENTS;
   for (size_t q = 0; q < nch; ++q) {
-    cudaEvent_t* ev = h->prof_events.data() + q * 9;
-    cudaError_t e = cudaEventSynchronize(ev[8]);
-    for (int k = 0; k < 8 && e == cudaSuccess; ++k) {
+    cudaEvent_t* ev = h->prof_events.data() + q * PROF_EVENTS;
+    cudaError_t e = cudaEventSynchronize(ev[PROF_EVENTS - 1]);
+    for (int k = 0; k < PROF_EVENTS - 1 && e == cudaSuccess; ++k) {
       float ms = 0.0f;
       e = cudaEventElapsedTime(&ms, ev[k], ev[k + 1]);
       ms_out[k] += ms;
@@ -346,6 +355,14 @@ int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out) {
 }
 
 uint64_t pix_kernel_launches(const pix_handle* h) { return h ? h->launches : 0; }
+
+int pix_overflow_runs(pix_handle* h, uint32_t* out) {
+  if (!h || !out) return PIX_ERR_INVALID_ARG;
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaMemcpy(out, h->proto.ctl + pix::CTL_OVF_COUNT, 4 * 8, cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) return fail_cuda(h, e, "pix_overflow_runs");
+  return PIX_OK;
+}
 
 const char* pix_last_error(const pix_handle* h) { return h ? h->err.c_str() : "invalid handle"; }
 

@@ -1,4 +1,6 @@
-// cluster.cu -- a4 findClus fused with a5 (cluster sums, charge cut, renumber, temp records).
+// cluster.cu -- the overflow kernel: a4 findClus fused with a5 (cluster sums, charge cut, renumber, temp records)
+// for the module runs the fused tile kernel (fused.cu) could not take: runs longer than its window, tiles with
+// too many runs, charge sums beyond 32 bits.  One block per run, tables in the global workspace, 64-bit sums.
 //
 // "clusters the pixels on each detector module".  The connectivity rule, the duplicate rule,
 // the canonical numbering and the charge cut are DESIGN.md readings S9, S10, S13, S14, S18.
@@ -15,7 +17,7 @@
 //   5  roots in digi order: Q >= cut survives and takes the next local id (ballot/popc scan); the root
 //      writes the temp record at (run first + id)
 //   6  per digi: final status and clus; per task: counts
-// Four size classes share this code: the group is a warp or a block, the tables sit in shared or global memory.
+// The digi fields (row, col, charge) are read back from the output arrays the fused kernel has written.
 #include "pix_common.cuh"
 
 namespace pix {
@@ -27,12 +29,6 @@ constexpr uint32_t HASH_MUL = 0x9E3779B1u;
 
 // ------------------------------------------------------------------ hash slots
 template <typename SlotT> struct SlotOps;
-template <> struct SlotOps<uint32_t> {  // key 17 bits | index 15 bits  (n <= 32767)
-  static constexpr uint32_t EMPTY = 0xFFFFFFFFu;
-  static __device__ __forceinline__ uint32_t pack(uint32_t key, uint32_t k) { return (key << 15) | k; }
-  static __device__ __forceinline__ uint32_t key(uint32_t v) { return v >> 15; }
-  static __device__ __forceinline__ uint32_t idx(uint32_t v) { return v & 0x7FFFu; }
-};
 template <> struct SlotOps<unsigned long long> {
   static constexpr unsigned long long EMPTY = ~0ull;
   static __device__ __forceinline__ unsigned long long pack(uint32_t key, uint32_t k) {
@@ -98,20 +94,6 @@ __device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
 }
 
 // ------------------------------------------------------------------ groups
-struct WarpGroup {
-  uint32_t lane;
-  __device__ __forceinline__ uint32_t rank() const { return lane; }
-  __device__ __forceinline__ uint32_t size() const { return 32u; }
-  __device__ __forceinline__ void sync() const { __syncwarp(); }
-  // exclusive scan of a flag over the group + total
-  __device__ __forceinline__ uint32_t scan_flag(bool f, uint32_t& total) const {
-    const uint32_t b = __ballot_sync(0xFFFFFFFFu, f);
-    total = __popc(b);
-    return __popc(b & ((1u << lane) - 1u));
-  }
-  __device__ __forceinline__ uint32_t sum(uint32_t v) const { return __reduce_add_sync(0xFFFFFFFFu, v); }
-};
-
 template <int THREADS>
 struct BlockGroup {
   uint32_t* s_scan;  // [THREADS/32 + 1] shared scratch
@@ -256,12 +238,12 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     n_pre += tot_pre; n_post += tot_post;
   }
   g.sync();
-  // 6: final status and clus of every decodable digi (undecodable ones were finished by unpack)
+  // 6: final status and clus of every decodable digi (undecodable ones were finished by the fused kernel)
   uint32_t n_ok = 0, n_cut = 0;
   for (uint32_t k = rk; k < n; k += gs) {
     const uint32_t p = T.pos[k];
     if (p == NOPOS) {
-      if (!STAGE_CHARGE) c.d_clus[gb + k] = -1;  // global class: the labels lived in clus, restore unpack's -1
+      if (!STAGE_CHARGE) c.d_clus[gb + k] = -1;  // the labels lived in clus: restore the -1 of an undecodable word
       continue;
     }
     int32_t clus = -1;
@@ -278,85 +260,29 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
   n_dup = g.sum(n_dup); n_below = g.sum(n_below); n_ok = g.sum(n_ok); n_cut = g.sum(n_cut);
   if (rk == 0) {
     c.n_clus[task] = n_post;
-    uint32_t* mc = c.mod_cnt + (size_t)task * MC_STRIDE;
-    mc[MC_PRECUT] = n_pre; mc[MC_DUP] = n_dup; mc[MC_BELOW] = n_below; mc[MC_OK] = n_ok; mc[MC_CUT] = n_cut;
+    uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
+    atomicAdd(ec + EC_PRECUT, n_pre); atomicAdd(ec + EC_DUP, n_dup); atomicAdd(ec + EC_BELOW, n_below);
+    atomicAdd(ec + EC_OK, n_ok); atomicAdd(ec + EC_CUT, n_cut);
   }
 }
 
-template <typename SlotT>
-__device__ __forceinline__ Tables<SlotT> carve(unsigned char* base, uint32_t cap) {
-  Tables<SlotT> T;
-  T.sx = reinterpret_cast<unsigned long long*>(base); base += (size_t)cap * 8;
-  T.sy = reinterpret_cast<unsigned long long*>(base); base += (size_t)cap * 8;
-  T.tab = reinterpret_cast<SlotT*>(base); base += (size_t)cap * 2 * sizeof(SlotT);
-  T.pos = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
-  T.chg = reinterpret_cast<int32_t*>(base); base += (size_t)cap * 4;
-  T.label = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
-  T.q = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
-  T.npix = reinterpret_cast<uint32_t*>(base);
-  return T;
-}
-constexpr size_t smem_per_digi = 8 + 8 + 2 * 4 + 4 * 5;  // 44 bytes
-
-// ------------------------------------------------------------------ kernels
-constexpr int WARP_TIER_THREADS = 256;
-__global__ void __launch_bounds__(WARP_TIER_THREADS) cluster_warp_kernel(const __grid_constant__ Chunk c) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  const Tables<uint32_t> T = carve<uint32_t>(smem + (size_t)warp * TIER_WARP_MAX * smem_per_digi, TIER_WARP_MAX);
-  const WarpGroup g{lane};
-  const uint32_t count = c.ctl[0];
-  const uint32_t* list = c.lists;
-  // static striding: tasks of this class are all small, and one global ticket counter would serialise
-  // millions of atomics on a single address
-  const uint32_t n_warps = gridDim.x * (WARP_TIER_THREADS / 32);
-  for (uint32_t t = blockIdx.x * (WARP_TIER_THREADS / 32) + warp; t < count; t += n_warps) {
-    cluster_task<WarpGroup, uint32_t, true>(c, g, T, list[t]);
-    __syncwarp();
-  }
-}
-
-template <int THREADS, int TIER, uint32_t CAP>
-__global__ void __launch_bounds__(THREADS) cluster_block_kernel(const __grid_constant__ Chunk c) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ uint32_t s_scan[THREADS / 32 + 1];
+// ------------------------------------------------------------------ kernel
+constexpr int OVF_THREADS = 512;
+__global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_constant__ Chunk c) {
+  __shared__ uint32_t s_scan[OVF_THREADS / 32 + 1];
   __shared__ uint32_t s_task;
-  const Tables<uint32_t> T = carve<uint32_t>(smem, CAP);
-  const BlockGroup<THREADS> g{s_scan};
-  const uint32_t count = c.ctl[TIER];
-  const uint32_t* list = c.lists + (size_t)TIER * c.list_stride;
-  if (TIER == 1) {  // many similar tasks: static striding, no ticket traffic
-    for (uint32_t t = blockIdx.x; t < count; t += gridDim.x) {
-      __syncthreads();
-      cluster_task<BlockGroup<THREADS>, uint32_t, true>(c, g, T, list[t]);
-    }
-    return;
-  }
-  while (true) {  // few, uneven tasks: atomic ticket
-    __syncthreads();
-    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + 4 + TIER, 1u);
-    __syncthreads();
-    const uint32_t t = s_task;
-    if (t >= count) break;
-    cluster_task<BlockGroup<THREADS>, uint32_t, true>(c, g, T, list[t]);
-  }
-}
-
-constexpr int GLOBAL_TIER_THREADS = 512;
-__global__ void __launch_bounds__(GLOBAL_TIER_THREADS) cluster_global_kernel(const __grid_constant__ Chunk c) {
-  __shared__ uint32_t s_scan[GLOBAL_TIER_THREADS / 32 + 1];
-  __shared__ uint32_t s_task;
-  const BlockGroup<GLOBAL_TIER_THREADS> g{s_scan};
-  const uint32_t count = c.ctl[3];
-  const uint32_t* list = c.lists + (size_t)3 * c.list_stride;
+  const BlockGroup<OVF_THREADS> g{s_scan};
+  uint32_t count = c.ctl[CTL_OVF_COUNT];
+  count = count < c.ovf_cap ? count : c.ovf_cap;
   while (true) {
     __syncthreads();
-    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + 7, 1u);
+    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + CTL_OVF_TICKET, 1u);
     __syncthreads();
     const uint32_t t = s_task;
     if (t >= count) break;
-    const uint32_t task = list[t];
+    const uint32_t task = c.ovf_list[t];
     const uint32_t er = task / c.M, m = task - er * c.M;
+    if (c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] & FLAG_NONCONTIGUOUS) continue;  // S11: not clustered
     const uint32_t first = c.module_first[(size_t)(c.e0 + er) * c.M + m];
     const uint32_t ebase = c.segB[er * c.F];
     const uint32_t rb = ebase - c.segB[0] + first;
@@ -365,49 +291,14 @@ __global__ void __launch_bounds__(GLOBAL_TIER_THREADS) cluster_global_kernel(con
     T.pos = c.g_pos + rb; T.chg = nullptr;
     T.label = reinterpret_cast<uint32_t*>(c.d_clus + (size_t)ebase + first);  // clus is written last, per digi
     T.q = c.g_q + rb; T.npix = c.g_npix + rb; T.sx = c.g_sx + rb; T.sy = c.g_sy + rb;
-    cluster_task<BlockGroup<GLOBAL_TIER_THREADS>, unsigned long long, false>(c, g, T, task);
+    cluster_task<BlockGroup<OVF_THREADS>, unsigned long long, false>(c, g, T, task);
   }
 }
 
-constexpr int SMALL_THREADS = 128, LARGE_THREADS = 512;
-constexpr size_t SMEM_WARP = (size_t)(WARP_TIER_THREADS / 32) * TIER_WARP_MAX * smem_per_digi;
-constexpr size_t SMEM_SMALL = (size_t)TIER_SMALL_MAX * smem_per_digi;
-constexpr size_t SMEM_LARGE = (size_t)TIER_LARGE_MAX * smem_per_digi;
-
 }  // namespace
 
-cudaError_t configure_cluster_kernels() {
-  cudaError_t e;
-  e = cudaFuncSetAttribute(cluster_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_WARP);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(cluster_block_kernel<SMALL_THREADS, 1, TIER_SMALL_MAX>,
-                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_SMALL);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(cluster_block_kernel<LARGE_THREADS, 2, TIER_LARGE_MAX>,
-                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LARGE);
-}
-
-static inline int clampi(uint64_t v, int lo, int hi) { return (int)(v < (uint64_t)lo ? lo : (v > (uint64_t)hi ? hi : v)); }
-
-// Persistent grids: every block pulls tasks from its class's list with an atomic ticket; the list lengths
-// live in device memory, so the grid is sized from host-side bounds only (legal during stream capture).
-void launch_cluster(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream, cudaEvent_t* ev) {
-  const uint64_t n_tasks = (uint64_t)(c.e1 - c.e0) * c.M;
-  const uint64_t wb = words_bound ? words_bound : 1;
-  // a class-q task has more than TIER_(q-1)_MAX words, so at most words/TIER_(q-1)_MAX tasks exist
-  const uint64_t bound1 = wb / TIER_WARP_MAX + 1, bound2 = wb / TIER_SMALL_MAX + 1, bound3 = wb / TIER_LARGE_MAX + 1;
-  const int g0 = clampi((n_tasks + 7) / 8, 1, n_sm * 5);
-  const int g1 = clampi(bound1 < n_tasks ? bound1 : n_tasks, 1, n_sm * 6);
-  const int g2 = clampi(bound2 < n_tasks ? bound2 : n_tasks, 1, n_sm);
-  const int g3 = clampi(bound3 < n_tasks ? bound3 : n_tasks, 1, n_sm * 2);
-  cluster_global_kernel<<<g3, GLOBAL_TIER_THREADS, 0, stream>>>(c);
-  if (ev) cudaEventRecord(ev[0], stream);
-  cluster_block_kernel<LARGE_THREADS, 2, TIER_LARGE_MAX><<<g2, LARGE_THREADS, SMEM_LARGE, stream>>>(c);
-  if (ev) cudaEventRecord(ev[1], stream);
-  cluster_block_kernel<SMALL_THREADS, 1, TIER_SMALL_MAX><<<g1, SMALL_THREADS, SMEM_SMALL, stream>>>(c);
-  if (ev) cudaEventRecord(ev[2], stream);
-  cluster_warp_kernel<<<g0, WARP_TIER_THREADS, SMEM_WARP, stream>>>(c);
-  if (ev) cudaEventRecord(ev[3], stream);
+void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
+  overflow_kernel<<<n_sm, OVF_THREADS, 0, stream>>>(c);
 }
 
 }  // namespace pix

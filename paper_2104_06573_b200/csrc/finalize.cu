@@ -62,16 +62,15 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
   if (blockIdx.x == 0) {
     uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
     for (uint32_t m = tid; m <= M; m += FIN_THREADS) cms[m] = s_start[m];
-    uint32_t acc[7] = {0, 0, 0, 0, 0, 0, 0};  // present, n_clusters, precut, dup, below, ok, cut
+    uint32_t acc[2] = {0, 0};  // modules present, clusters surviving the cut
     for (uint32_t m = tid; m < M; m += FIN_THREADS) {
-      acc[0] += c.module_end[(size_t)e * M + m] > 0u ? 1u : 0u;
+      const bool present = c.module_end[(size_t)e * M + m] > 0u;
+      if (!present) c.module_first[(size_t)e * M + m] = 0u;  // S12: absent -> 0,0 (init left the atomicMin sentinel)
+      acc[0] += present ? 1u : 0u;
       acc[1] += skip ? 0u : n_clus[m];
-      const uint32_t* mc = c.mod_cnt + ((size_t)er * M + m) * MC_STRIDE;
-#pragma unroll
-      for (int k = 0; k < MC_STRIDE; ++k) acc[2 + k] += mc[k];
     }
 #pragma unroll
-    for (int k = 0; k < 7; ++k) {
+    for (int k = 0; k < 2; ++k) {
       const uint32_t v = __reduce_add_sync(0xFFFFFFFFu, acc[k]);
       if (lane == 0 && v) atomicAdd(s_red + k, v);
     }
@@ -82,8 +81,8 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
       const uint32_t bad = ec[EC_EMPTY] + ec[EC_ERR_LINK] + ec[EC_ERR_ROC] + ec[EC_ERR_DCOL] + ec[EC_ERR_PXID];
       s[0] = n_words; s[1] = n_words - bad; s[2] = ec[EC_EMPTY];
       s[3] = ec[EC_ERR_LINK]; s[4] = ec[EC_ERR_ROC]; s[5] = ec[EC_ERR_DCOL]; s[6] = ec[EC_ERR_PXID];
-      s[7] = s_red[3]; s[8] = s_red[4]; s[9] = s_red[5]; s[10] = s_red[6];
-      s[11] = s_red[0]; s[12] = s_red[2]; s[13] = s_red[1]; s[14] = n_emit;
+      s[7] = ec[EC_DUP]; s[8] = ec[EC_BELOW]; s[9] = ec[EC_OK]; s[10] = ec[EC_CUT];
+      s[11] = s_red[0]; s[12] = ec[EC_PRECUT]; s[13] = s_red[1]; s[14] = n_emit;
       s[15] = flags | (total > c.cap_ev ? FLAG_CAPACITY : 0u);
     }
   }

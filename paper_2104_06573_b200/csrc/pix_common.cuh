@@ -4,12 +4,12 @@
 // clusters the pixels on each detector module", plus the per-module offset table of PAPER.md Fig. 3
 // (lines 76-81).  Readings S1..S24 of DESIGN.md fix what the paper leaves open.
 //
-// Kernel chain for one chunk of events (DESIGN.md section 5):
+// Kernel chain for one chunk of events (DESIGN.md section 6):
 //   init      -> segment table, range sentinels, zeroed counters
-//   unpack    -> a1 decode + a2 calibrate + a3 run boundaries (ballot/shuffle last-valid scan)
-//   classify  -> per (event, module) task: absent-module fix-up, size class lists
-//   cluster   -> a4 findClus (position hash + min-index union-find) fused with a5 (sums, cut, renumber)
-//                in four size classes: warp / small block / large block (all shared memory) / global
+//   fused     -> a1 decode + a2 calibrate + a3 run boundaries + a4 findClus + a5 sums/cut/renumber for every
+//                module run that fits a block's 2048-word window (tile of 1024 words + look-ahead)
+//   overflow  -> a4 + a5 for the runs the fused kernel could not take (longer than the window, pathological
+//                charge sums): generic block-per-run kernel, tables in global workspace
 //   finalize  -> a6 clamp + prefix scan (Fig. 3), record scatter, summary
 // Nothing here is shared with oracle/.
 #pragma once
@@ -29,17 +29,17 @@ enum : uint8_t { ST_OK = 0, ST_CUT = 1, ST_BELOW = 2, ST_DUP = 3, ST_EMPTY = 4, 
 constexpr uint32_t FLAG_NONCONTIGUOUS = 1u, FLAG_CAPACITY = 2u, FLAG_TOO_LARGE = 4u;
 constexpr uint32_t NO_INDEX = 0xFFFFFFFFu;
 
-// size classes of the cluster step, by run length n = module_end - module_first
-constexpr int N_TIERS = 4;
-constexpr uint32_t TIER_WARP_MAX = 128;    // one warp per module, <= 4 digis per lane
-constexpr uint32_t TIER_SMALL_MAX = 768;   // 128-thread block, shared memory
-constexpr uint32_t TIER_LARGE_MAX = 4096;  // 512-thread block, shared memory
-                                           // beyond: 512-thread block, tables in global workspace
+// per-event counters (integer atomics only), one row of EC_STRIDE per event of the chunk
+enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
+       EC_PRECUT, EC_STRIDE = 16 };
+// ctl words
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_WORDS = 16 };
 
-// per-event counters produced by unpack (the rest of the summary comes from per-module counts)
-enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_STRIDE = 8 };
-// per-(event,module) counts produced by cluster
-enum { MC_PRECUT = 0, MC_DUP, MC_BELOW, MC_OK, MC_CUT, MC_STRIDE = 5 };
+// Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
+//   x = module | bad << 16 | scol << 24     bad: 0, ST_ERR_LINK or ST_ERR_ROC; scol = +1 / -1 (int8)
+//   y = row0 | col0 << 8 | srow << 24       row0 = rocy*80 + (flip_r ? 79 : 0), col0 = rocx*52 + (flip_c ? 51 : 0)
+// so that row = row0 + srow * (pxid >> 1), col = col0 + scol * (2*dcol + (pxid & 1)).
+typedef uint2 CabEntry;
 
 // Everything a kernel needs for one chunk of events [e0, e1).  Passed by value (__grid_constant__).
 struct Chunk {
@@ -51,7 +51,7 @@ struct Chunk {
   uint32_t e0, e1;          // event range of this chunk
   uint32_t F, M;
   // ---- tables (device, owned by the handle)
-  const uint32_t* cab;      // [F*64*32]
+  const CabEntry* cab;      // [F*64*32]
   const float2* gp;         // [M*416] (gain, pedestal) interleaved
   // ---- parameters
   float vcal_gain, vcal_offset, max_e_f;
@@ -66,14 +66,13 @@ struct Chunk {
   // ---- workspace (device, owned by the handle), indexed by chunk-relative event / word
   uint32_t* segB;           // [(e1-e0)*F + 1] global word index where segment (event, fed) starts
   uint32_t* ev_cnt;         // [(e1-e0)*EC_STRIDE]
-  uint32_t* ctl;            // [16]: 0..3 list counts, 4..7 tickets, 8 chunk skip flag
-  uint32_t* lists;          // [N_TIERS][(e1-e0)*M] task ids (event_rel*M + module)
-  uint32_t list_stride;
+  uint32_t* ctl;            // [CTL_WORDS]
+  uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
+  uint32_t ovf_cap;
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
-  uint32_t* mod_cnt;        // [(e1-e0)*M*MC_STRIDE]
   // temp cluster records, indexed by chunk-relative word index (run first + local id)
   uint32_t* t_first; uint32_t* t_npix; uint32_t* t_charge; float* t_x; float* t_y;
-  // global-tier scratch, indexed by chunk-relative word index
+  // overflow-kernel scratch, indexed by chunk-relative word index
   unsigned long long* g_hash;  // [2*cap_words]
   uint32_t* g_pos; uint32_t* g_q; uint32_t* g_npix; unsigned long long* g_sx; unsigned long long* g_sy;
 };
@@ -82,16 +81,14 @@ __device__ __forceinline__ uint32_t ev_offset(const Chunk& c, uint32_t e) {
   return c.ev_off ? c.ev_off[e] : (e ? c.n_single : 0u);
 }
 
-// launchers (host), one per kernel family; all asynchronous on `stream`
+// launchers (host), one per kernel; all asynchronous on `stream`
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream);
-void launch_unpack(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
-void launch_classify(const Chunk& c, int n_sm, cudaStream_t stream);
-// ev (optional): 4 events, recorded after each of the four class kernels (global, large, small, warp)
-void launch_cluster(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream, cudaEvent_t* ev = nullptr);
+void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
+void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);
-cudaError_t configure_cluster_kernels();
+cudaError_t configure_fused_kernel();
 cudaError_t configure_finalize_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 8;  // init, unpack, classify, cluster x4, finalize
+constexpr int LAUNCHES_PER_CHUNK = 4;    // init, fused, overflow, finalize
 
 }  // namespace pix
