@@ -168,11 +168,11 @@ def pix_kernel_launches(h: Handle) -> int:
 
 def pix_overflow_runs(h: Handle) -> int:
     """Diagnostic: runs the last internal chunk left to the overflow kernel (synchronises the device)."""
-    n = (_u32 * 8)()
-    rc = load().pix_overflow_runs(h.ptr, ctypes.cast(n, ctypes.POINTER(_u32)))
+    n = _u32()
+    rc = load().pix_overflow_runs(h.ptr, ctypes.byref(n))
     if rc != PIX_OK:
         raise PixError(rc, pix_last_error(h))
-    return list(n)
+    return int(n.value)
 
 
 KERNEL_FAMILIES = ("init", "fused", "overflow", "finalize")

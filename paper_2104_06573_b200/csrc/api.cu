@@ -359,7 +359,7 @@ uint64_t pix_kernel_launches(const pix_handle* h) { return h ? h->launches : 0; 
 int pix_overflow_runs(pix_handle* h, uint32_t* out) {
   if (!h || !out) return PIX_ERR_INVALID_ARG;
   cudaError_t e = cudaDeviceSynchronize();
-  if (e == cudaSuccess) e = cudaMemcpy(out, h->proto.ctl + pix::CTL_OVF_COUNT, 4 * 8, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(out, h->proto.ctl + pix::CTL_OVF_COUNT, 4, cudaMemcpyDeviceToHost);
   if (e != cudaSuccess) return fail_cuda(h, e, "pix_overflow_runs");
   return PIX_OK;
 }

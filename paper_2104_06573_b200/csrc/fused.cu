@@ -7,15 +7,16 @@
 // form one run (S11); a run belongs to the tile that holds its first word.  The block
 //   A  clears its position hash; warp 0 looks back for the last decodable word before the tile (carry-in run)
 //   B  decodes + calibrates its words, stores module/row/col/charge, finds run starts with a ballot/shuffle
-//      "previous decodable word" scan, numbers the tile's runs with a block prefix sum
-//   C  warp 0 looks ahead (up to 1024 more words) for the rest of the tile's last run
-//   D  inserts every owned decodable digi into the hash keyed by (run, row, col), equal keys keep the lowest
-//      digi index (S10); looks up the 4 forward neighbours and unites (lock-free min-index union-find)
+//      "previous decodable word" scan, numbers the tile's runs with a block prefix sum, and inserts every owned
+//      decodable digi into the position hash keyed by (run, row, col); equal keys keep the lowest digi (S10)
+//   C  meanwhile warp 0 looks ahead (up to 1024 more words) for the rest of the tile's last run
+//   D  every warp looks up the forward neighbours of its digis, compacts the adjacent pairs into a dense edge
+//      list and unites them (lock-free min-index union-find, all lanes busy)
 //   E  roots store, members atomically add: charge, charge*col, charge*row (u32) and the pixel count
 //   F  surviving roots (Q >= cut) are numbered in digi order per run (block prefix sum), temp records written
 //   G  final status and clus of every word the tile owns
-// Runs that do not fit the window, tiles with more than RCAP runs and charge sums that could overflow 32 bits
-// go to the overflow list (cluster.cu).  Nothing here is shared with oracle/.
+// Runs that do not fit the window or the hash, tiles with more than RCAP runs and charge sums that could
+// overflow 32 bits go to the overflow list (cluster.cu).  Nothing here is shared with oracle/.
 #include "pix_common.cuh"
 
 namespace pix {
@@ -140,8 +141,9 @@ constexpr int FT = 256;                   // threads per block
 constexpr int FW = FT / 32;
 constexpr uint32_t TW = FT * 4;           // words per tile
 constexpr uint32_t CW = 2 * TW;           // window: tile + look-ahead
-constexpr uint32_t TABN = 2 * CW, TABMASK = TABN - 1;
+constexpr uint32_t TABN = 2 * CW;         // hash slots
 constexpr uint32_t RCAP = 510;            // runs a tile can own
+constexpr uint32_t EDGE_CAP = CW / FW;    // edge slots per warp (in Smem::q)
 constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
@@ -154,15 +156,16 @@ struct __align__(16) Smem {
   uint32_t tab[TABN];    // position hash (see hinsert), EMPTY-filled.  After phase D: sx = tab, sy = tab + CW
   uint32_t dkey[CW];     // key of the digi in window slot d (word tBeg + d), INVALID if not owned / undecodable
   uint32_t label[CW];    // union-find parent (low 16 bits) | members added << 16, or MARK_*
-  uint32_t q[CW];        // root: charge sum; after phase F: local cluster id or NO_INDEX
+  uint32_t q[CW];        // phase D: per-warp edge lists; then root: charge sum; after phase F: local id or NO_INDEX
   uint16_t chg[CW];
   uint32_t run_ifirst[RCAP + 2];  // event-relative index of the run's first digi
   uint16_t run_first[RCAP + 2];   // window slot of the run's first digi
   uint16_t run_base[RCAP + 2];    // survivors before the run
+  uint8_t run_bad[RCAP + 2];      // the run is left to the overflow kernel
   uint2 warp_last[FW];
   uint32_t warp_sum[FW];
   uint2 carry;
-  uint32_t seg0, seg_last, n_tot, over, qover, n_runs, last_valid;
+  uint32_t n_tot;
 };
 
 // Position hash: 1024 buckets of 4 slots (one 128-bit shared load per probe).  h = key * HASH_MUL mod 2^28 is a
@@ -170,16 +173,17 @@ struct __align__(16) Smem {
 // exactly and no second load is needed to verify a hit.  A key whose home bucket is full goes to the next
 // bucket(s) and records the displacement.  Slot = disp (2) | tag (18) | digi (11) | below_threshold (1); slots of
 // a bucket fill in order and are never emptied, equal keys meet in one slot and keep the lowest digi (S10).
-constexpr uint32_t NBUCKET = TABN / 4, MAX_DISP = 2;
+constexpr uint32_t NBUCKET = TABN / 4, MAX_DISP = 3;
 __device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & 0x0FFFFFFFu; }
 
-// false: no room within MAX_DISP buckets (the tile then goes to the overflow kernel)
+// false: no room within MAX_DISP buckets (the run then goes to the overflow kernel)
 __device__ __forceinline__ bool hinsert(Smem& s, uint32_t key, uint32_t d, uint32_t below) {
   const uint32_t h = hmix(key), tag = h & 0x3FFFFu;
   uint32_t b = h >> 18;
 #pragma unroll 1
   for (uint32_t i = 0; i <= MAX_DISP; ++i, b = (b + 1u) & (NBUCKET - 1u)) {
     const uint32_t want = (i << 18) | tag, mine = (want << 12) | (d << 1) | below;
+    if (mine == EMPTY) return false;
 #pragma unroll 1
     for (uint32_t q = 0; q < 4u; ++q) {
       uint32_t* slot = &s.tab[b * 4u + q];
@@ -218,6 +222,11 @@ __device__ __noinline__ uint32_t hfind_slow(const Smem& s, uint32_t key) {
   }
   return EMPTY;
 }
+__device__ __forceinline__ uint32_t hfind(const Smem& s, uint32_t key) {
+  bool more;
+  const uint32_t e = hfind_fast(s, key, more);
+  return more ? hfind_slow(s, key) : e;
+}
 __device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x7FFu; }
 
 // union-find on s.label (phase D only: high halves are zero); labels strictly decrease along parents
@@ -250,49 +259,37 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
   return v;
 }
 
-// phase D for the 4 digis of window slots d0..d0+3
-__device__ __forceinline__ void phase_unite(Smem& s, uint32_t d0) {
-  const uint4 k4 = *reinterpret_cast<const uint4*>(&s.dkey[d0]);
+// phase D, part 1, for the 4 digis of window slots d0..d0+3 (active lanes; the call is warp-uniform): duplicate
+// check and forward-neighbour lookups; the adjacent pairs go to the warp's edge list (ballot compaction).
+// Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE are
+// joined to it by their own E edges, so d-S alone is enough.
+__device__ __forceinline__ void phase_edges(Smem& s, uint32_t d0, bool active, uint32_t* elist, uint32_t& ne,
+                                            uint32_t lt_mask) {
+  uint4 k4 = make_uint4(INVALID, INVALID, INVALID, INVALID);
+  if (active) k4 = *reinterpret_cast<const uint4*>(&s.dkey[d0]);
   const uint32_t k[4] = {k4.x, k4.y, k4.z, k4.w};
-  uint32_t ent[4][5];
-  bool slow = false;
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    const uint32_t key = k[j];
+    const uint32_t key = k[j], d = d0 + j;
+    bool live = key != INVALID;
+    const uint32_t own = hfind(s, key);
+    const uint32_t eE = hfind(s, key + 1u), eSW = hfind(s, key + 511u), eS = hfind(s, key + 512u),
+                   eSE = hfind(s, key + 513u);
+    if (live && slot_digi(own) != d) { s.label[d] = MARK_DUP; live = false; }  // S10: an earlier word owns this pixel
+    if (own & 1u) live = false;                                                // below threshold: joins nothing
+    const bool hS = live && eS != EMPTY && !(eS & 1u);
+    const bool f[3] = {live && eE != EMPTY && !(eE & 1u), hS || (live && eSW != EMPTY && !(eSW & 1u)),
+                       live && !hS && eSE != EMPTY && !(eSE & 1u)};
+    const uint32_t nb[3] = {slot_digi(eE), slot_digi(hS ? eS : eSW), slot_digi(eSE)};
 #pragma unroll
-    for (int q = 0; q < 5; ++q) {
-      // own pixel, then the forward neighbours (r, c+1), (r+1, c-1), (r+1, c), (r+1, c+1) (S13)
-      const uint32_t nk = key + (q == 0 ? 0u : (q == 1 ? 1u : 509u + (uint32_t)q));
-      bool more;
-      ent[j][q] = hfind_fast(s, nk, more);
-      slow |= more && key != INVALID;
-    }
-  }
-  if (slow) {  // rare: some home bucket was full
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      if (k[j] == INVALID) continue;
-#pragma unroll
-      for (int q = 0; q < 5; ++q) {
-        const uint32_t nk = k[j] + (q == 0 ? 0u : (q == 1 ? 1u : 509u + (uint32_t)q));
-        bool more;
-        const uint32_t e = hfind_fast(s, nk, more);
-        if (more) ent[j][q] = hfind_slow(s, nk);
-        else ent[j][q] = e;
+    for (int t = 0; t < 3; ++t) {
+      const uint32_t mask = __ballot_sync(0xFFFFFFFFu, f[t]);
+      if (f[t]) {
+        const uint32_t pos = ne + __popc(mask & lt_mask);
+        if (pos < EDGE_CAP) elist[pos] = d | (nb[t] << 16);
+        else uf_unite(s.label, d, nb[t]);  // list full (dense window): unite in place
       }
-    }
-  }
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    const uint32_t d = d0 + j;
-    if (k[j] == INVALID) continue;
-    const uint32_t e = ent[j][0];
-    if (slot_digi(e) != d) { s.label[d] = MARK_DUP; continue; }  // S10: an earlier word owns this pixel
-    if (e & 1u) continue;                                        // below threshold: owns the pixel, joins nothing
-#pragma unroll
-    for (int q = 1; q < 5; ++q) {
-      const uint32_t n = ent[j][q];
-      if (n != EMPTY && !(n & 1u)) uf_unite(s.label, d, slot_digi(n));
+      ne += __popc(mask);
     }
   }
 }
@@ -300,10 +297,12 @@ __device__ __forceinline__ void phase_unite(Smem& s, uint32_t d0) {
 // phase E1: roots store their own contribution
 __device__ __forceinline__ void phase_roots(Smem& s, uint32_t d0) {
   uint32_t* sx = s.tab; uint32_t* sy = s.tab + CW;
+  const uint4 l4 = *reinterpret_cast<const uint4*>(&s.label[d0]);
+  const uint32_t l[4] = {l4.x, l4.y, l4.z, l4.w};
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
     const uint32_t d = d0 + j;
-    if (s.label[d] != d) continue;
+    if (l[j] != d) continue;
     const uint32_t key = s.dkey[d], e = s.chg[d];
     s.q[d] = e; sx[d] = e * (key & 511u); sy[d] = e * ((key >> 9) & 255u);
   }
@@ -343,25 +342,39 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
   const uint32_t lt_mask = (1u << lane) - 1u;
 
   for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const uint32_t tBeg = T0 + tile * TW;
-    const uint32_t tFirst = tBeg < gBeg ? gBeg : tBeg;  // first word of the tile that belongs to the chunk
-    // ================================================================== A: clear; segment + look-back (warp 0)
+    const uint32_t tBeg = T0 + tile * TW, tEnd = tBeg + TW;
+    // ================================================================== A: load; clear; segment; look-back
+    const uint32_t g0 = tBeg + tid * 4u;
+    const bool any = (g0 + 4u > gBeg) && (g0 < gEnd);
+    const bool full = (g0 >= gBeg) && (g0 + 4u <= gEnd);
+    uint32_t w[4] = {0u, 0u, 0u, 0u};
+    if (full) {
+      const uint4 v = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
+      w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+    } else if (any) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) if (g0 + j >= gBeg && g0 + j < gEnd) w[j] = __ldg(c.words + g0 + j);
+    }
     {
       uint4* t4 = reinterpret_cast<uint4*>(s.tab);
       const uint4 e4 = make_uint4(EMPTY, EMPTY, EMPTY, EMPTY);
 #pragma unroll
       for (int k = 0; k < (int)(TABN / 4 / FT); ++k) t4[tid + k * FT] = e4;
+      if (tid < (RCAP + 2u) / 4u) reinterpret_cast<uint32_t*>(s.run_bad)[tid] = 0u;
     }
-    if (warp == 0) {
-      const uint32_t s0 = warp_find_segment(segB, S, tFirst, lane);
+    // segment (event, FED) of the warp's first word inside the chunk
+    uint32_t gw = tBeg + warp * 128u;
+    gw = gw < gBeg ? gBeg : (gw >= gEnd ? gEnd - 1u : gw);
+    const uint32_t sgw = warp_find_segment(segB, S, gw, lane);
+    if (warp == 0) {  // last decodable word before the tile: its run may continue into the tile
       uint2 carry = make_uint2(NOKEY, 0u);
-      uint32_t g = tFirst;  // words [gBeg, g) are still to be searched, backwards
+      uint32_t g = gw;  // words [gBeg, g) are still to be searched, backwards
       while (g > gBeg) {
         const bool in = lane < g - gBeg;
         const uint32_t gi = g - 1u - lane;
         uint32_t key = NOKEY;
         if (in) {
-          uint32_t sg = s0;
+          uint32_t sg = sgw;
           while (segB[sg] > gi) --sg;  // segB[0] = gBeg <= gi
           const uint32_t er = sg / c.F, fed = sg - er * c.F;
           uint32_t m, r, cc;
@@ -376,35 +389,23 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
         }
         g = (g - gBeg > 32u) ? g - 32u : gBeg;
       }
-      if (lane == 0) { s.seg0 = s0; s.carry = carry; s.over = 0u; s.qover = 0u; s.n_tot = TW; }
+      if (lane == 0) s.carry = carry;
     }
-    __syncthreads();
 
-    // ================================================================== B: load, decode, calibrate, run starts
-    const uint32_t g0 = tBeg + tid * 4u;
-    const bool any = (g0 + 4u > gBeg) && (g0 < gEnd);
-    const bool full = (g0 >= gBeg) && (g0 + 4u <= gEnd);
-    uint32_t w[4] = {0u, 0u, 0u, 0u};
-    if (full) {
-      const uint4 v = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
-      w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
-    } else if (any) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) if (g0 + j >= gBeg && g0 + j < gEnd) w[j] = __ldg(c.words + g0 + j);
-    }
+    // ================================================================== B: decode, calibrate, run starts
     uint32_t st[4], key[4], pos[4];
     int32_t chg[4];
     uint32_t tkey = NOKEY, tg = 0u;
     uint32_t inmask = 0u;  // words of this thread inside the chunk
     {
       uint32_t mod[4], row[4], col[4];
-      uint32_t sg = s.seg0;
+      uint32_t sg = sgw;
       if (any) {
         const uint32_t gf = g0 < gBeg ? gBeg : g0;
         while (sg + 1u < S && segB[sg + 1u] <= gf) ++sg;
       }
       uint32_t er = sg / c.F, fed = sg - er * c.F;
-      uint32_t nextB = (any && sg + 1u <= S) ? segB[sg + 1u] : 0xFFFFFFFFu;
+      uint32_t nextB = segB[sg + 1u];
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const uint32_t g = g0 + j;
@@ -429,7 +430,6 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
           atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st[j] - ST_EMPTY), 1u);
         }
       }
-      if (tid == FT - 1) s.seg_last = sg;
       if (full) {
         *reinterpret_cast<ushort4*>(c.d_module + g0) = make_ushort4(mod[0], mod[1], mod[2], mod[3]);
         *reinterpret_cast<ushort4*>(c.d_row + g0) = make_ushort4(row[0], row[1], row[2], row[3]);
@@ -456,7 +456,7 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
     const int src = below_l ? 31 - __clz(below_l) : 0;
     uint32_t pkey = __shfl_sync(0xFFFFFFFFu, tkey, src);
     uint32_t pg = __shfl_sync(0xFFFFFFFFu, tg, src);
-    __syncthreads();
+    __syncthreads();  // #1: warp_last, carry, cleared hash
     if (!below_l) {  // nothing decodable earlier in this warp: take the nearest earlier warp, else the look-back
       uint2 cin = s.carry;
       for (int wq = (int)warp - 1; wq >= 0; --wq) {
@@ -477,25 +477,37 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       }
       pkey = key[j]; pg = g0 + j;
     }
-    // the tile's last decodable word (thread 0 reads it for the chunk's last run; warp 0 for the look-ahead)
+    // the tile's last decodable word: its run is the one the look-ahead completes
     uint2 lastv = s.carry;
     bool tile_has = false;
-    if (warp == 0) {
-      for (int wq = FW - 1; wq >= 0; --wq) {
-        const uint2 v = s.warp_last[wq];
-        if (v.x != NOKEY) { lastv = v; tile_has = true; break; }
-      }
-      if (tile == n_tiles - 1u && tid == 0 && lastv.x != NOKEY) run_end(c, lastv.x, lastv.y);
+    for (int wq = FW - 1; wq >= 0; --wq) {
+      const uint2 v = s.warp_last[wq];
+      if (v.x != NOKEY) { lastv = v; tile_has = true; break; }
     }
+    if (tile == n_tiles - 1u && tid == 0 && lastv.x != NOKEY) run_end(c, lastv.x, lastv.y);  // the chunk's last run
     // ---- number the tile's runs: block prefix sum of the run starts
     const uint32_t nst = __popc(startmask);
     const uint32_t incl = warp_incl_scan(nst, lane);
     if (lane == 31) s.warp_sum[warp] = incl;
-    __syncthreads();
+    __syncthreads();  // #2
     uint32_t rbase = incl - nst, n_runs = 0;
 #pragma unroll
     for (int q = 0; q < FW; ++q) { const uint32_t v = s.warp_sum[q]; if (q < (int)warp) rbase += v; n_runs += v; }
-    // stage the window slots of this thread's words
+    const uint32_t R = n_runs < RCAP ? n_runs : RCAP;  // runs this tile owns; the last one may reach past the tile
+    if (n_runs == 0u) {
+      // nothing owned: only the undecodable words of the tile are finished here
+      if (full && (st[0] >= ST_EMPTY) && (st[1] >= ST_EMPTY) && (st[2] >= ST_EMPTY) && (st[3] >= ST_EMPTY)) {
+        *reinterpret_cast<uchar4*>(c.d_status + g0) = make_uchar4(st[0], st[1], st[2], st[3]);
+        *reinterpret_cast<int4*>(c.d_clus + g0) = make_int4(-1, -1, -1, -1);
+      } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if ((inmask >> j & 1u) && st[j] >= ST_EMPTY) { c.d_status[g0 + j] = (uint8_t)st[j]; c.d_clus[g0 + j] = -1; }
+      }
+      __syncthreads();
+      continue;
+    }
+    // stage the window slots of this thread's words and insert the owned ones into the hash
     uint32_t runl[4];
     {
       uint32_t r = rbase;
@@ -515,31 +527,19 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       *reinterpret_cast<uint4*>(&s.label[tid * 4u]) = make_uint4(lb[0], lb[1], lb[2], lb[3]);
       *reinterpret_cast<uint2*>(&s.chg[tid * 4u]) =
           make_uint2((uint32_t)chg[0] | ((uint32_t)chg[1] << 16), (uint32_t)chg[2] | ((uint32_t)chg[3] << 16));
-    }
-    const uint32_t R = n_runs < RCAP ? n_runs : RCAP;  // runs this tile owns
-    if (n_runs == 0u) {
-      // nothing owned: only the undecodable words of the tile are finished here
-      if (full && (st[0] >= ST_EMPTY) && (st[1] >= ST_EMPTY) && (st[2] >= ST_EMPTY) && (st[3] >= ST_EMPTY)) {
-        *reinterpret_cast<uchar4*>(c.d_status + g0) = make_uchar4(st[0], st[1], st[2], st[3]);
-        *reinterpret_cast<int4*>(c.d_clus + g0) = make_int4(-1, -1, -1, -1);
-      } else {
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-          if ((inmask >> j & 1u) && st[j] >= ST_EMPTY) { c.d_status[g0 + j] = (uint8_t)st[j]; c.d_clus[g0 + j] = -1; }
-      }
-      __syncthreads();
-      continue;
+      for (int j = 0; j < 4; ++j)
+        if (runl[j] && !hinsert(s, dk[j], tid * 4u + j, st[j] == ST_BELOW ? 1u : 0u)) s.run_bad[runl[j]] = 1;
     }
 
     // ================================================================== C: look-ahead for the last run (warp 0)
     if (warp == 0) {
-      const uint32_t tEnd = tBeg + TW;
       uint32_t n_tot = TW;
       if (tile_has && n_runs <= RCAP && tEnd < gEnd) {
         const uint32_t keyR = lastv.x;
         uint32_t p = tEnd;
         bool ended = false;
-        uint32_t sg = s.seg_last;
+        uint32_t sg = warp_find_segment(segB, S, tEnd, lane);
         while (!ended && p < gEnd && p < tEnd + TW) {
           const uint32_t x0 = p + lane * 4u;
           uint32_t ww[4] = {0u, 0u, 0u, 0u};
@@ -567,7 +567,7 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
             const float2 gp = __ldg(c.gp + (m * (uint32_t)COLS + cc));
             const int32_t e = calibrate(c, ww[j] & 255u, gp);
             dk[j] = (R << 17) | (r << 9) | cc; ch[j] = (uint32_t)e;
-            lb[j] = (e < c.thr) ? MARK_BELOW : (x0 + j - tBeg);
+            lb[j] = (e < c.thr) ? MARK_BELOW : (g - tBeg);
           }
           const uint32_t stopped = __ballot_sync(0xFFFFFFFFu, stop != 4);
           const uint32_t first_stop = stopped ? (uint32_t)(__ffs(stopped) - 1) : 32u;
@@ -579,71 +579,72 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
           *reinterpret_cast<uint4*>(&s.dkey[d0]) = make_uint4(dk[0], dk[1], dk[2], dk[3]);
           *reinterpret_cast<uint4*>(&s.label[d0]) = make_uint4(lb[0], lb[1], lb[2], lb[3]);
           *reinterpret_cast<uint2*>(&s.chg[d0]) = make_uint2(ch[0] | (ch[1] << 16), ch[2] | (ch[3] << 16));
-          if (stopped) { ended = true; n_tot = d0 - lane * 4u + (first_stop + 1u) * 4u; }
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (dk[j] != INVALID && !hinsert(s, dk[j], d0 + j, lb[j] == MARK_BELOW ? 1u : 0u)) s.run_bad[R] = 1;
+          if (stopped) { ended = true; n_tot = (p - tBeg) + (first_stop + 1u) * 4u; }
           else { p += 128u; n_tot = p - tBeg; }
         }
         if (!ended && p < gEnd) {  // the run does not fit the window: the overflow kernel takes it
-          if (lane == 0) { s.over = 1u; push_overflow(c, keyR); atomicAdd(c.ctl + 5, 1u); }
+          if (lane == 0) s.run_bad[R] = 1;
           n_tot = TW;
         }
       }
-      if (lane == 0) { s.n_tot = n_tot; s.n_runs = R; }
+      if (lane == 0) s.n_tot = n_tot;
     }
-    __syncthreads();
+    __syncthreads();  // #3: hash complete
     const uint32_t n_tot = s.n_tot;
-    const bool over = s.over != 0u;
     const uint32_t d0n = tid * 4u, d0x = TW + tid * 4u;
     const bool has_ext = d0x < n_tot;
-    if (over) {  // the last run left to the overflow kernel: its words in the tile are not owned after all
-#pragma unroll
-      for (int j = 0; j < 4; ++j) if (runl[j] == R) { runl[j] = 0u; s.dkey[d0n + j] = INVALID; }
-    }
+    const bool warp_ext = TW + warp * 128u < n_tot;  // warp-uniform: some lane of this warp has look-ahead slots
 
-    // ================================================================== D: hash insert, then neighbours + unions
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-      if (runl[j] && !hinsert(s, (runl[j] << 17) | pos[j], d0n + j, st[j] == ST_BELOW ? 1u : 0u)) { s.qover = 1u; atomicAdd(c.ctl + 2, 1u); }
-    if (has_ext) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const uint32_t k = s.dkey[d0x + j];
-        if (k != INVALID && !hinsert(s, k, d0x + j, s.label[d0x + j] == MARK_BELOW ? 1u : 0u)) { s.qover = 1u; atomicAdd(c.ctl + 3, 1u); }
+    // ================================================================== D: neighbours -> edge list -> unions
+    {
+      uint32_t* elist = s.q + warp * EDGE_CAP;
+      uint32_t ne = 0u;
+      phase_edges(s, d0n, true, elist, ne, lt_mask);
+      if (warp_ext) phase_edges(s, d0x, has_ext, elist, ne, lt_mask);
+      __syncwarp();
+      ne = ne < EDGE_CAP ? ne : EDGE_CAP;
+      for (uint32_t i = lane; i < ne; i += 32u) {
+        const uint32_t e = elist[i];
+        uf_unite(s.label, e & 0xFFFFu, e >> 16);
       }
     }
-    __syncthreads();
-    phase_unite(s, d0n);
-    if (has_ext) phase_unite(s, d0x);
-    __syncthreads();
+    __syncthreads();  // #4: components complete; the hash is dead, its memory becomes sx / sy
     // ================================================================== E: cluster sums
     phase_roots(s, d0n);
     if (has_ext) phase_roots(s, d0x);
-    __syncthreads();
+    __syncthreads();  // #5
     phase_members(s, d0n);
     if (has_ext) phase_members(s, d0x);
-    __syncthreads();
+    __syncthreads();  // #6
     // ================================================================== F: cut, renumber, temp records
     uint32_t labn[4], labx[4] = {MARK_BELOW, MARK_BELOW, MARK_BELOW, MARK_BELOW};
-    uint32_t survn = 0u, survx = 0u, n_pre = 0u;
+    uint32_t survn = 0u, survx = 0u, rootn = 0u, rootx = 0u;
     {
       const uint4 l4 = *reinterpret_cast<const uint4*>(&s.label[d0n]);
       labn[0] = l4.x; labn[1] = l4.y; labn[2] = l4.z; labn[3] = l4.w;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         if (!runl[j] || !is_root(labn[j], d0n + j)) continue;
-        ++n_pre;
+        rootn |= 1u << j;
         const uint32_t Q = s.q[d0n + j];
-        if (Q > Q_SAFE) { s.qover = 1u; atomicAdd(c.ctl + 4, 1u); }
+        if (Q > Q_SAFE) s.run_bad[runl[j]] = 1;                  // 32-bit weighted sums may have wrapped
         if ((long long)Q >= (long long)c.cut) survn |= 1u << j;  // S9: equality keeps
       }
       if (has_ext) {
         const uint4 x4 = *reinterpret_cast<const uint4*>(&s.label[d0x]);
+        const uint4 k4 = *reinterpret_cast<const uint4*>(&s.dkey[d0x]);
+        const uint32_t kx[4] = {k4.x, k4.y, k4.z, k4.w};
         labx[0] = x4.x; labx[1] = x4.y; labx[2] = x4.z; labx[3] = x4.w;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          if (s.dkey[d0x + j] == INVALID || !is_root(labx[j], d0x + j)) continue;
-          ++n_pre;
+          if (kx[j] == INVALID) { labx[j] = INVALID; continue; }  // INVALID label: slot not in the run
+          if (!is_root(labx[j], d0x + j)) continue;
+          rootx |= 1u << j;
           const uint32_t Q = s.q[d0x + j];
-          if (Q > Q_SAFE) s.qover = 1u;
+          if (Q > Q_SAFE) s.run_bad[R] = 1;
           if ((long long)Q >= (long long)c.cut) survx |= 1u << j;
         }
       }
@@ -651,13 +652,12 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
     const uint32_t packed = __popc(survn) | (__popc(survx) << 16);
     const uint32_t pincl = warp_incl_scan(packed, lane);
     if (lane == 31) s.warp_sum[warp] = pincl;
-    __syncthreads();
+    __syncthreads();  // #7
     uint32_t pbase = pincl - packed, ptot = 0;
 #pragma unroll
     for (int q = 0; q < FW; ++q) { const uint32_t v = s.warp_sum[q]; if (q < (int)warp) pbase += v; ptot += v; }
     const uint32_t totN = ptot & 0xFFFFu, totAll = totN + (ptot >> 16);
     const uint32_t exclN = pbase & 0xFFFFu, exclX = totN + (pbase >> 16);
-    const bool qover = s.qover != 0u;
     {
       uint32_t r = rbase;
 #pragma unroll
@@ -668,22 +668,16 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
         }
       if (tid == 0) s.run_base[R + 1u] = (uint16_t)totAll;
     }
-    __syncthreads();
-    if (qover) {
-      // pathological charges: every run of this tile goes to the overflow kernel (64-bit sums there)
-      uint32_t r = rbase;
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-        if (startmask >> j & 1u) { ++r; if (r <= RCAP && !(over && r == R)) push_overflow(c, key[j]); }
-    } else {
+    __syncthreads();  // #8: run_base, run_bad final
+    {
       uint32_t r = rbase;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        if (startmask >> j & 1u) {
-          ++r;
-          if (r <= RCAP && !(over && r == R))
-            c.n_clus[(key[j] >> 16) * c.M + (key[j] & 0xFFFFu)] = (uint32_t)s.run_base[r + 1u] - s.run_base[r];
-        }
+        if (!(startmask >> j & 1u)) continue;
+        ++r;
+        if (r > RCAP) continue;
+        if (s.run_bad[r]) push_overflow(c, key[j]);
+        else c.n_clus[(key[j] >> 16) * c.M + (key[j] & 0xFFFFu)] = (uint32_t)s.run_base[r + 1u] - s.run_base[r];
       }
       const uint32_t* sx = s.tab; const uint32_t* sy = s.tab + CW;
       const uint32_t relBeg = tBeg - gBeg;  // may wrap for the chunk's first tile; only used added to a slot >= gBeg - tBeg
@@ -691,31 +685,33 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       for (int half = 0; half < 2; ++half) {
         if (half == 1 && !has_ext) break;
         const uint32_t d0 = half ? d0x : d0n;
-        const uint32_t surv = half ? survx : survn;
+        const uint32_t surv = half ? survx : survn, roots = half ? rootx : rootn;
         const uint32_t excl = half ? exclX : exclN;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          const uint32_t d = d0 + j, lab = half ? labx[j] : labn[j];
-          const bool live_root = half ? (s.dkey[d] != INVALID && is_root(lab, d)) : (runl[j] && is_root(lab, d));
-          if (!live_root) continue;
+          if (!(roots >> j & 1u)) continue;
+          const uint32_t d = d0 + j;
           if (!(surv >> j & 1u)) { s.q[d] = NO_INDEX; continue; }
           const uint32_t rr = half ? R : runl[j];
           const uint32_t id = excl + __popc(surv & ((1u << j) - 1u)) - s.run_base[rr];
+          const uint32_t Q = s.q[d];
+          s.q[d] = id;
+          if (s.run_bad[rr]) continue;
           const uint32_t rf = s.run_first[rr];
           const uint32_t o = relBeg + rf + id;
-          const uint32_t Q = s.q[d];
           c.t_first[o] = s.run_ifirst[rr] + (d - rf);
-          c.t_npix[o] = 1u + (lab >> 16);
+          c.t_npix[o] = 1u + ((half ? labx[j] : labn[j]) >> 16);
           c.t_charge[o] = Q;
           c.t_x[o] = (float)sx[d] / (float)Q;   // S18; exact integer sums, one rounding each (within 1e-5)
           c.t_y[o] = (float)sy[d] / (float)Q;
-          s.q[d] = id;
         }
       }
     }
-    __syncthreads();
+    __syncthreads();  // #9: q holds the local ids
     // ================================================================== G: final status and clus, counters
-    uint32_t cntA = 0u, cntB = 0u;  // dup | below << 16 ; ok | cut << 16
+    uint32_t cntA = 0u, cntB = 0u, n_pre = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
+    uint32_t ev_lo = NOKEY, ev_hi = 0u;         // events of the digis this thread counted
+    uint32_t cmask = 0u, cmaskx = 0u;           // digis counted (native, look-ahead)
     {
       int32_t cl[4];
       uint32_t so[4];
@@ -724,13 +720,17 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       for (int j = 0; j < 4; ++j) {
         cl[j] = -1; so[j] = st[j];
         if (st[j] >= ST_EMPTY) continue;             // undecodable: status as decoded (0xFF outside the chunk)
-        if (!runl[j] || qover) { mine_all = false; so[j] = 0xFFu; continue; }
+        if (!runl[j] || s.run_bad[runl[j]]) { mine_all = false; so[j] = 0xFFu; continue; }
+        cmask |= 1u << j;
+        const uint32_t e = key[j] >> 16;
+        ev_lo = e < ev_lo ? e : ev_lo; ev_hi = e > ev_hi ? e : ev_hi;
         const uint32_t lab = labn[j];
         if (lab == MARK_DUP) { so[j] = ST_DUP; cntA += 1u; }
         else if (lab == MARK_BELOW) { so[j] = ST_BELOW; cntA += 0x10000u; }
         else {
           const uint32_t id = s.q[lab & 0xFFFFu];
           if (id != NO_INDEX) { so[j] = ST_OK; cl[j] = (int32_t)id; cntB += 1u; } else { so[j] = ST_CUT; cntB += 0x10000u; }
+          n_pre += rootn >> j & 1u;
         }
       }
       if (mine_all) {
@@ -741,36 +741,31 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
         for (int j = 0; j < 4; ++j)
           if ((inmask >> j & 1u) && so[j] != 0xFFu) { c.d_status[g0 + j] = (uint8_t)so[j]; c.d_clus[g0 + j] = cl[j]; }
       }
-      if (has_ext && !qover) {
+    }
+    const uint32_t er_x = lastv.x >> 16;  // the look-ahead digis belong to the run of the tile's last decodable word
+    if (has_ext && !s.run_bad[R]) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint32_t d = d0x + j;
-          if (s.dkey[d] == INVALID) continue;
-          const uint32_t lab = labx[j];
-          uint32_t sj; int32_t cj = -1;
-          if (lab == MARK_DUP) { sj = ST_DUP; cntA += 1u; }
-          else if (lab == MARK_BELOW) { sj = ST_BELOW; cntA += 0x10000u; }
-          else {
-            const uint32_t id = s.q[lab & 0xFFFFu];
-            if (id != NO_INDEX) { sj = ST_OK; cj = (int32_t)id; cntB += 1u; } else { sj = ST_CUT; cntB += 0x10000u; }
-          }
-          c.d_status[tBeg + d] = (uint8_t)sj; c.d_clus[tBeg + d] = cj;
+      for (int j = 0; j < 4; ++j) {
+        const uint32_t lab = labx[j];
+        if (lab == INVALID) continue;
+        cmaskx |= 1u << j;
+        uint32_t sj; int32_t cj = -1;
+        if (lab == MARK_DUP) { sj = ST_DUP; cntA += 1u; }
+        else if (lab == MARK_BELOW) { sj = ST_BELOW; cntA += 0x10000u; }
+        else {
+          const uint32_t id = s.q[lab & 0xFFFFu];
+          if (id != NO_INDEX) { sj = ST_OK; cj = (int32_t)id; cntB += 1u; } else { sj = ST_CUT; cntB += 0x10000u; }
+          n_pre += rootx >> j & 1u;
         }
+        c.d_status[tBeg + d0x + j] = (uint8_t)sj; c.d_clus[tBeg + d0x + j] = cj;
       }
+      if (cmaskx) { ev_lo = er_x < ev_lo ? er_x : ev_lo; ev_hi = er_x > ev_hi ? er_x : ev_hi; }
     }
     // counters: one event per warp in the common case -> warp sums, lane 0 adds; else every digi adds its own
-    if (!qover) {
-      uint32_t er_x = NOKEY;  // the look-ahead digis belong to the tile's last run = run of its last decodable word
-      if (has_ext)
-        for (int wq = FW - 1; wq >= 0; --wq) { const uint32_t v = s.warp_last[wq].x; if (v != NOKEY) { er_x = v >> 16; break; } }
-      uint32_t ev_lo = NOKEY, ev_hi = 0u;
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-        if (runl[j]) { const uint32_t e = key[j] >> 16; ev_lo = e < ev_lo ? e : ev_lo; ev_hi = e > ev_hi ? e : ev_hi; }
-      if (has_ext && er_x != NOKEY) { ev_lo = er_x < ev_lo ? er_x : ev_lo; ev_hi = er_x > ev_hi ? er_x : ev_hi; }
+    {
       const uint32_t lo = __reduce_min_sync(0xFFFFFFFFu, ev_lo), hi = __reduce_max_sync(0xFFFFFFFFu, ev_hi);
       if (lo == NOKEY) {
-        // no owned digi in this warp
+        // no counted digi in this warp
       } else if (lo == hi) {
         const uint32_t a = __reduce_add_sync(0xFFFFFFFFu, cntA), b = __reduce_add_sync(0xFFFFFFFFu, cntB);
         const uint32_t p = __reduce_add_sync(0xFFFFFFFFu, n_pre);
@@ -785,24 +780,22 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       } else {
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
-          if (half == 1 && !has_ext) break;
 #pragma unroll
           for (int j = 0; j < 4; ++j) {
-            const uint32_t d = (half ? d0x : d0n) + j;
-            if (half ? (s.dkey[d] == INVALID) : !runl[j]) continue;
+            if (!((half ? cmaskx : cmask) >> j & 1u)) continue;
             uint32_t* ec = c.ev_cnt + (size_t)(half ? er_x : (key[j] >> 16)) * EC_STRIDE;
             const uint32_t lab = half ? labx[j] : labn[j];
             if (lab == MARK_DUP) atomicAdd(ec + EC_DUP, 1u);
             else if (lab == MARK_BELOW) atomicAdd(ec + EC_BELOW, 1u);
             else {
               atomicAdd(ec + (s.q[lab & 0xFFFFu] != NO_INDEX ? EC_OK : EC_CUT), 1u);
-              if (is_root(lab, d)) atomicAdd(ec + EC_PRECUT, 1u);
+              if ((half ? rootx : rootn) >> j & 1u) atomicAdd(ec + EC_PRECUT, 1u);
             }
           }
         }
       }
     }
-    __syncthreads();  // shared state is rewritten by the next tile
+    __syncthreads();  // #10: shared state is rewritten by the next tile
   }
 }
 
