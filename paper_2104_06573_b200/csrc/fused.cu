@@ -9,7 +9,7 @@
 //   B  decodes + calibrates its words, stores module/row/col/charge, finds run starts with a ballot/shuffle
 //      "previous decodable word" scan, numbers the tile's runs with a block prefix sum, and inserts every owned
 //      decodable digi into the position hash keyed by (run, row, col); equal keys keep the lowest digi (S10)
-//   C  meanwhile warp 0 looks ahead (up to 1024 more words) for the rest of the tile's last run
+//   C  meanwhile warp 0 looks ahead (up to 512 more words) for the rest of the tile's last run
 //   D  every warp looks up the forward neighbours of its digis, compacts the adjacent pairs into a dense edge
 //      list and unites them (lock-free min-index union-find, all lanes busy)
 //   E  roots store, members atomically add: charge, charge*col, charge*row (u32) and the pixel count
@@ -140,15 +140,16 @@ __device__ __forceinline__ void push_overflow(const Chunk& c, uint32_t key) {
 constexpr int FT = 256;                   // threads per block
 constexpr int FW = FT / 32;
 constexpr uint32_t TW = FT * 4;           // words per tile
-constexpr uint32_t CW = 2 * TW;           // window: tile + look-ahead
-constexpr uint32_t TABN = 2 * CW;         // hash slots
-constexpr uint32_t RCAP = 510;            // runs a tile can own
+constexpr uint32_t AHEAD = 512;           // look-ahead for the tile's last run
+constexpr uint32_t CW = TW + AHEAD;       // window
+constexpr uint32_t TABN = 8192;           // hash slots
+constexpr uint32_t RCAP = 254;            // runs a tile can own
 constexpr uint32_t EDGE_CAP = CW / FW;    // edge slots per warp (in Smem::q)
-constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
+constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu, NO_SLOT = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
 constexpr uint32_t HASH_MUL = 0x9E3779B1u;
-static_assert(TABN == 4096 && CW == 2048, "slot layout: 10-bit bucket, 11-bit digi");
+static_assert(TABN == 8192 && CW <= 2048 && 2 * CW <= TABN, "slot layout: 11-bit bucket, 17-bit tag, 11-bit digi");
 
 // digi key inside the window: run (11 bits) | row (8 bits) | col (9 bits).  Neighbour keys are key+1 (col+1)
 // and key+512-1, +512, +512+1 (row+1): col 416..511 and row 160..255 never occur, so no bounds checks (S13).
@@ -157,7 +158,7 @@ struct __align__(16) Smem {
   uint32_t dkey[CW];     // key of the digi in window slot d (word tBeg + d), INVALID if not owned / undecodable
   uint32_t label[CW];    // union-find parent (low 16 bits) | members added << 16, or MARK_*
   uint32_t q[CW];        // phase D: per-warp edge lists; then root: charge sum; after phase F: local id or NO_INDEX
-  uint16_t chg[CW];
+  uint16_t chg[CW];      // charge; after phase E: the list of surviving roots
   uint32_t run_ifirst[RCAP + 2];  // event-relative index of the run's first digi
   uint16_t run_first[RCAP + 2];   // window slot of the run's first digi
   uint16_t run_base[RCAP + 2];    // survivors before the run
@@ -168,64 +169,54 @@ struct __align__(16) Smem {
   uint32_t n_tot;
 };
 
-// Position hash: 1024 buckets of 4 slots (one 128-bit shared load per probe).  h = key * HASH_MUL mod 2^28 is a
-// bijection on the 28-bit keys; bucket = top 10 bits of h, tag = the other 18, so (bucket, tag) names the key
+// Position hash: 2048 buckets of 4 slots, one 128-bit shared load per lookup.  h = key * HASH_MUL mod 2^28 is a
+// bijection on the 28-bit keys; bucket = top 11 bits of h, tag = the other 17, so (bucket, tag) names the key
 // exactly and no second load is needed to verify a hit.  A key whose home bucket is full goes to the next
-// bucket(s) and records the displacement.  Slot = disp (2) | tag (18) | digi (11) | below_threshold (1); slots of
-// a bucket fill in order and are never emptied, equal keys meet in one slot and keep the lowest digi (S10).
-constexpr uint32_t NBUCKET = TABN / 4, MAX_DISP = 3;
+// bucket(s) and records the displacement.  Slot = 0 | disp (2) | tag (17) | digi (11) | below_threshold (1);
+// slots of a bucket fill in order and are never emptied, equal keys meet in one slot and keep the lowest digi (S10).
+constexpr uint32_t NBUCKET = TABN / 4, MAX_DISP = 3, TAG_BITS = 17, TAG_MASK = (1u << TAG_BITS) - 1u;
 __device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & 0x0FFFFFFFu; }
 
-// false: no room within MAX_DISP buckets (the run then goes to the overflow kernel)
-__device__ __forceinline__ bool hinsert(Smem& s, uint32_t key, uint32_t d, uint32_t below) {
-  const uint32_t h = hmix(key), tag = h & 0x3FFFFu;
-  uint32_t b = h >> 18;
+// returns the slot index, or NO_SLOT: no room within MAX_DISP buckets (the run then goes to the overflow kernel)
+__device__ __forceinline__ uint32_t hinsert(Smem& s, uint32_t key, uint32_t d, uint32_t below) {
+  const uint32_t h = hmix(key), tag = h & TAG_MASK;
+  uint32_t p = (h >> TAG_BITS) * 4u;
 #pragma unroll 1
-  for (uint32_t i = 0; i <= MAX_DISP; ++i, b = (b + 1u) & (NBUCKET - 1u)) {
-    const uint32_t want = (i << 18) | tag, mine = (want << 12) | (d << 1) | below;
-    if (mine == EMPTY) return false;
-#pragma unroll 1
-    for (uint32_t q = 0; q < 4u; ++q) {
-      uint32_t* slot = &s.tab[b * 4u + q];
-      uint32_t old = *reinterpret_cast<volatile uint32_t*>(slot);
-      if (old == EMPTY) old = atomicCAS(slot, EMPTY, mine);
-      if (old == EMPTY) return true;
-      if ((old >> 12) == want) { atomicMin(slot, mine); return true; }
-    }
+  for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u); ++i, p = (p + 1u) & (TABN - 1u)) {
+    const uint32_t want = ((i >> 2) << TAG_BITS) | tag, mine = (want << 12) | (d << 1) | below;
+    const uint32_t old = atomicCAS(&s.tab[p], EMPTY, mine);
+    if (old == EMPTY) return p;
+    if ((old >> 12) == want) { atomicMin(&s.tab[p], mine); return p; }  // same pixel: the lowest digi owns it
   }
-  return false;
+  return NO_SLOT;
 }
-// slot of `key` or EMPTY: first probe; more = the home bucket is full and holds no match (rare)
-__device__ __forceinline__ uint32_t hfind_fast(const Smem& s, uint32_t key, bool& more) {
-  const uint32_t h = hmix(key), want = h & 0x3FFFFu;
-  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> 18) * 4u]);
+__device__ __forceinline__ uint32_t half_match(const uint4& e, uint32_t want) {
   uint32_t r = EMPTY;
   if ((e.w >> 12) == want) r = e.w;
   if ((e.z >> 12) == want) r = e.z;
   if ((e.y >> 12) == want) r = e.y;
   if ((e.x >> 12) == want) r = e.x;
-  more = (r == EMPTY) && (e.w != EMPTY);
   return r;
 }
 __device__ __noinline__ uint32_t hfind_slow(const Smem& s, uint32_t key) {
-  const uint32_t h = hmix(key), tag = h & 0x3FFFFu;
-  uint32_t b = h >> 18;
-  for (uint32_t i = 1; i <= MAX_DISP; ++i) {
+  const uint32_t h = hmix(key), tag = h & TAG_MASK;
+  uint32_t b = h >> TAG_BITS;
+  for (uint32_t i = 1; i <= MAX_DISP; ++i) {  // the buckets after the (full) home bucket
     b = (b + 1u) & (NBUCKET - 1u);
-    const uint32_t want = (i << 18) | tag;
     const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[b * 4u]);
-    if ((e.x >> 12) == want) return e.x;
-    if ((e.y >> 12) == want) return e.y;
-    if ((e.z >> 12) == want) return e.z;
-    if ((e.w >> 12) == want) return e.w;
+    const uint32_t r = half_match(e, (i << TAG_BITS) | tag);
+    if (r != EMPTY) return r;
     if (e.w == EMPTY) return EMPTY;
   }
   return EMPTY;
 }
+// slot contents of `key`, or EMPTY
 __device__ __forceinline__ uint32_t hfind(const Smem& s, uint32_t key) {
-  bool more;
-  const uint32_t e = hfind_fast(s, key, more);
-  return more ? hfind_slow(s, key) : e;
+  const uint32_t h = hmix(key), want = h & TAG_MASK;
+  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> TAG_BITS) * 4u]);
+  uint32_t r = half_match(e, want);
+  if (r == EMPTY && e.w != EMPTY) r = hfind_slow(s, key);  // home bucket full, no match (rare): displaced keys
+  return r;
 }
 __device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x7FFu; }
 
@@ -263,8 +254,9 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
 // check and forward-neighbour lookups; the adjacent pairs go to the warp's edge list (ballot compaction).
 // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE are
 // joined to it by their own E edges, so d-S alone is enough.
-__device__ __forceinline__ void phase_edges(Smem& s, uint32_t d0, bool active, uint32_t* elist, uint32_t& ne,
-                                            uint32_t lt_mask) {
+template <bool NATIVE>
+__device__ __forceinline__ void phase_edges(Smem& s, uint32_t d0, bool active, const uint32_t (&slot)[4], uint32_t* elist,
+                                            uint32_t& ne, uint32_t lt_mask) {
   uint4 k4 = make_uint4(INVALID, INVALID, INVALID, INVALID);
   if (active) k4 = *reinterpret_cast<const uint4*>(&s.dkey[d0]);
   const uint32_t k[4] = {k4.x, k4.y, k4.z, k4.w};
@@ -272,7 +264,8 @@ __device__ __forceinline__ void phase_edges(Smem& s, uint32_t d0, bool active, u
   for (int j = 0; j < 4; ++j) {
     const uint32_t key = k[j], d = d0 + j;
     bool live = key != INVALID;
-    const uint32_t own = hfind(s, key);
+    // own pixel: a tile word remembers its slot; a look-ahead word (inserted by warp 0) looks itself up
+    const uint32_t own = NATIVE ? s.tab[slot[j] & (TABN - 1u)] : hfind(s, key);
     const uint32_t eE = hfind(s, key + 1u), eSW = hfind(s, key + 511u), eS = hfind(s, key + 512u),
                    eSE = hfind(s, key + 513u);
     if (live && slot_digi(own) != d) { s.label[d] = MARK_DUP; live = false; }  // S10: an earlier word owns this pixel
@@ -508,7 +501,7 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       continue;
     }
     // stage the window slots of this thread's words and insert the owned ones into the hash
-    uint32_t runl[4];
+    uint32_t runl[4], slot[4];
     {
       uint32_t r = rbase;
       uint32_t dk[4], lb[4];
@@ -528,8 +521,12 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
       *reinterpret_cast<uint2*>(&s.chg[tid * 4u]) =
           make_uint2((uint32_t)chg[0] | ((uint32_t)chg[1] << 16), (uint32_t)chg[2] | ((uint32_t)chg[3] << 16));
 #pragma unroll
-      for (int j = 0; j < 4; ++j)
-        if (runl[j] && !hinsert(s, dk[j], tid * 4u + j, st[j] == ST_BELOW ? 1u : 0u)) s.run_bad[runl[j]] = 1;
+      for (int j = 0; j < 4; ++j) {
+        slot[j] = 0u;
+        if (!runl[j]) continue;
+        slot[j] = hinsert(s, dk[j], tid * 4u + j, st[j] == ST_BELOW ? 1u : 0u);
+        if (slot[j] == NO_SLOT) s.run_bad[runl[j]] = 1;
+      }
     }
 
     // ================================================================== C: look-ahead for the last run (warp 0)
@@ -540,7 +537,7 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
         uint32_t p = tEnd;
         bool ended = false;
         uint32_t sg = warp_find_segment(segB, S, tEnd, lane);
-        while (!ended && p < gEnd && p < tEnd + TW) {
+        while (!ended && p < gEnd && p < tEnd + AHEAD) {
           const uint32_t x0 = p + lane * 4u;
           uint32_t ww[4] = {0u, 0u, 0u, 0u};
           if (x0 + 4u <= gEnd) {
@@ -581,7 +578,7 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
           *reinterpret_cast<uint2*>(&s.chg[d0]) = make_uint2(ch[0] | (ch[1] << 16), ch[2] | (ch[3] << 16));
 #pragma unroll
           for (int j = 0; j < 4; ++j)
-            if (dk[j] != INVALID && !hinsert(s, dk[j], d0 + j, lb[j] == MARK_BELOW ? 1u : 0u)) s.run_bad[R] = 1;
+            if (dk[j] != INVALID && hinsert(s, dk[j], d0 + j, lb[j] == MARK_BELOW ? 1u : 0u) == NO_SLOT) s.run_bad[R] = 1;
           if (stopped) { ended = true; n_tot = (p - tBeg) + (first_stop + 1u) * 4u; }
           else { p += 128u; n_tot = p - tBeg; }
         }
@@ -602,8 +599,8 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
     {
       uint32_t* elist = s.q + warp * EDGE_CAP;
       uint32_t ne = 0u;
-      phase_edges(s, d0n, true, elist, ne, lt_mask);
-      if (warp_ext) phase_edges(s, d0x, has_ext, elist, ne, lt_mask);
+      phase_edges<true>(s, d0n, true, slot, elist, ne, lt_mask);
+      if (warp_ext) phase_edges<false>(s, d0x, has_ext, slot, elist, ne, lt_mask);
       __syncwarp();
       ne = ne < EDGE_CAP ? ne : EDGE_CAP;
       for (uint32_t i = lane; i < ne; i += 32u) {
@@ -668,7 +665,20 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
         }
       if (tid == 0) s.run_base[R + 1u] = (uint16_t)totAll;
     }
-    __syncthreads();  // #8: run_base, run_bad final
+    // surviving roots, densely listed in digi order (the charge array is dead by now)
+    uint16_t* slist = s.chg;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (rootn >> j & 1u) {
+        if (survn >> j & 1u) slist[exclN + __popc(survn & ((1u << j) - 1u))] = (uint16_t)(d0n + j);
+        else s.q[d0n + j] = NO_INDEX;
+      }
+      if (rootx >> j & 1u) {
+        if (survx >> j & 1u) slist[exclX + __popc(survx & ((1u << j) - 1u))] = (uint16_t)(d0x + j);
+        else s.q[d0x + j] = NO_INDEX;
+      }
+    }
+    __syncthreads();  // #8: run_base, run_bad, survivor list final
     {
       uint32_t r = rbase;
 #pragma unroll
@@ -679,32 +689,23 @@ __global__ void __launch_bounds__(FT, 4) fused_kernel(const __grid_constant__ Ch
         if (s.run_bad[r]) push_overflow(c, key[j]);
         else c.n_clus[(key[j] >> 16) * c.M + (key[j] & 0xFFFFu)] = (uint32_t)s.run_base[r + 1u] - s.run_base[r];
       }
+      // one survivor per thread: local id (S14) and temp record (S18)
       const uint32_t* sx = s.tab; const uint32_t* sy = s.tab + CW;
       const uint32_t relBeg = tBeg - gBeg;  // may wrap for the chunk's first tile; only used added to a slot >= gBeg - tBeg
-#pragma unroll
-      for (int half = 0; half < 2; ++half) {
-        if (half == 1 && !has_ext) break;
-        const uint32_t d0 = half ? d0x : d0n;
-        const uint32_t surv = half ? survx : survn, roots = half ? rootx : rootn;
-        const uint32_t excl = half ? exclX : exclN;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          if (!(roots >> j & 1u)) continue;
-          const uint32_t d = d0 + j;
-          if (!(surv >> j & 1u)) { s.q[d] = NO_INDEX; continue; }
-          const uint32_t rr = half ? R : runl[j];
-          const uint32_t id = excl + __popc(surv & ((1u << j) - 1u)) - s.run_base[rr];
-          const uint32_t Q = s.q[d];
-          s.q[d] = id;
-          if (s.run_bad[rr]) continue;
-          const uint32_t rf = s.run_first[rr];
-          const uint32_t o = relBeg + rf + id;
-          c.t_first[o] = s.run_ifirst[rr] + (d - rf);
-          c.t_npix[o] = 1u + ((half ? labx[j] : labn[j]) >> 16);
-          c.t_charge[o] = Q;
-          c.t_x[o] = (float)sx[d] / (float)Q;   // S18; exact integer sums, one rounding each (within 1e-5)
-          c.t_y[o] = (float)sy[d] / (float)Q;
-        }
+      for (uint32_t i = tid; i < totAll; i += FT) {
+        const uint32_t d = slist[i];
+        const uint32_t rr = s.dkey[d] >> 17;
+        const uint32_t id = i - s.run_base[rr];
+        const uint32_t Q = s.q[d];
+        s.q[d] = id;
+        if (s.run_bad[rr]) continue;
+        const uint32_t rf = s.run_first[rr];
+        const uint32_t o = relBeg + rf + id;
+        c.t_first[o] = s.run_ifirst[rr] + (d - rf);
+        c.t_npix[o] = 1u + (s.label[d] >> 16);
+        c.t_charge[o] = Q;
+        c.t_x[o] = (float)sx[d] / (float)Q;   // S18; exact integer sums, one rounding each (within 1e-5)
+        c.t_y[o] = (float)sy[d] / (float)Q;
       }
     }
     __syncthreads();  // #9: q holds the local ids
