@@ -72,6 +72,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.ctl = (uint32_t*)take(pix::CTL_WORDS * 4);
   c.ovf_list = (uint32_t*)take(Ec * M * 4);
   c.ovf_cap = (uint32_t)(Ec * M);
+  c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.n_clus = (uint32_t*)take(Ec * M * 4);
   c.t_first = (uint32_t*)take(W * 4); c.t_npix = (uint32_t*)take(W * 4); c.t_charge = (uint32_t*)take(W * 4);
   c.t_x = (float*)take(W * 4); c.t_y = (float*)take(W * 4);
@@ -118,7 +119,7 @@ void bind_outputs(pix::Chunk& c, const pix_digis* d, const pix_clusters* k) {
 }
 
 // the launch sequence of one chunk
-constexpr int PROF_EVENTS = pix::LAUNCHES_PER_CHUNK + 1;
+constexpr int PROF_EVENTS = 5;  // families: init, fused, overflow, finalize (offsets + scatter)
 int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t words_bound, cudaStream_t s) {
   cudaEvent_t* ev = nullptr;
   if (h->profiling) {
@@ -154,7 +155,8 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   const uint32_t F = cabling->n_feds, M = cabling->n_modules;
   if (F < 1 || F > 65535 || M < 1 || M > pix::MAX_MODULES || gains->n_modules != M) return PIX_ERR_INVALID_ARG;
   if (params->pixel_threshold_e < 1 || params->max_electrons < 1 || params->max_electrons > 65535) return PIX_ERR_INVALID_ARG;
-  if (params->max_words_per_event < 1 || params->max_events_per_batch < 1 || params->max_clusters_per_event < 1)
+  if (params->max_words_per_event < 1 || params->max_events_per_batch < 1 || params->max_clusters_per_event < 1 ||
+      params->max_clusters_per_event > (1u << 26))
     return PIX_ERR_INVALID_ARG;
   for (size_t i = 0; i < (size_t)F * 64 * 32; ++i)  // every mapped entry must name a module of the gain table
     if ((cabling->entry[i] & 2u) && ((cabling->entry[i] >> 2) & 0xFFFFu) >= M) return PIX_ERR_INVALID_ARG;
@@ -166,11 +168,13 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
   if (e == cudaSuccess) e = pix::configure_fused_kernel();
   if (e == cudaSuccess) e = pix::configure_finalize_kernel();
+  if (e == cudaSuccess) e = pix::configure_overflow_kernel();
   if (e != cudaSuccess) { delete h; cudaGetLastError(); return PIX_ERR_CUDA; }
 
-  // chunking: events per internal launch group; default keeps a chunk's digis within the L2-friendly few MB
+  // chunking: events per internal launch group; default: up to 64 Mi words per group (the path is bound by
+  // instruction issue, not by HBM, so few large launches beat L2-sized ones)
   uint64_t ce = params->chunk_events;
-  if (ce == 0) { ce = (4u << 20) / params->max_words_per_event; if (ce < 1) ce = 1; }
+  if (ce == 0) { ce = (64u << 20) / params->max_words_per_event; if (ce < 1) ce = 1; }
   if (ce > params->max_events_per_batch) ce = params->max_events_per_batch;
   if (ce > 65535) ce = 65535;
   const uint64_t capw = ce * (uint64_t)params->max_words_per_event;

@@ -29,6 +29,12 @@ constexpr uint32_t HASH_MUL = 0x9E3779B1u;
 
 // ------------------------------------------------------------------ hash slots
 template <typename SlotT> struct SlotOps;
+template <> struct SlotOps<uint32_t> {  // key 17 bits | index 15 bits  (n <= 32767)
+  static constexpr uint32_t EMPTY = 0xFFFFFFFFu;
+  static __device__ __forceinline__ uint32_t pack(uint32_t key, uint32_t k) { return (key << 15) | k; }
+  static __device__ __forceinline__ uint32_t key(uint32_t v) { return v >> 15; }
+  static __device__ __forceinline__ uint32_t idx(uint32_t v) { return v & 0x7FFFu; }
+};
 template <> struct SlotOps<unsigned long long> {
   static constexpr unsigned long long EMPTY = ~0ull;
   static __device__ __forceinline__ unsigned long long pack(uint32_t key, uint32_t k) {
@@ -267,8 +273,27 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
 }
 
 // ------------------------------------------------------------------ kernel
-constexpr int OVF_THREADS = 512;
+// Runs of up to SMEM_CAP digis keep all their tables in shared memory; longer ones use the global workspace.
+constexpr int OVF_THREADS = 256;
+constexpr uint32_t SMEM_CAP = 1024;
+constexpr size_t SMEM_PER_DIGI = 8 + 8 + 2 * 4 + 4 * 5;  // sx, sy, 2 hash slots, pos, chg, label, q, npix
+constexpr size_t OVF_SMEM = SMEM_CAP * SMEM_PER_DIGI;
+
+__device__ __forceinline__ Tables<uint32_t> carve(unsigned char* base, uint32_t cap) {
+  Tables<uint32_t> T;
+  T.sx = reinterpret_cast<unsigned long long*>(base); base += (size_t)cap * 8;
+  T.sy = reinterpret_cast<unsigned long long*>(base); base += (size_t)cap * 8;
+  T.tab = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 2 * 4;
+  T.pos = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
+  T.chg = reinterpret_cast<int32_t*>(base); base += (size_t)cap * 4;
+  T.label = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
+  T.q = reinterpret_cast<uint32_t*>(base); base += (size_t)cap * 4;
+  T.npix = reinterpret_cast<uint32_t*>(base);
+  return T;
+}
+
 __global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ __align__(16) unsigned char ovf_smem[];
   __shared__ uint32_t s_scan[OVF_THREADS / 32 + 1];
   __shared__ uint32_t s_task;
   const BlockGroup<OVF_THREADS> g{s_scan};
@@ -284,6 +309,10 @@ __global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_cons
     const uint32_t er = task / c.M, m = task - er * c.M;
     if (c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] & FLAG_NONCONTIGUOUS) continue;  // S11: not clustered
     const uint32_t first = c.module_first[(size_t)(c.e0 + er) * c.M + m];
+    if (c.module_end[(size_t)(c.e0 + er) * c.M + m] - first <= SMEM_CAP) {
+      cluster_task<BlockGroup<OVF_THREADS>, uint32_t, true>(c, g, carve(ovf_smem, SMEM_CAP), task);
+      continue;
+    }
     const uint32_t ebase = c.segB[er * c.F];
     const uint32_t rb = ebase - c.segB[0] + first;
     Tables<unsigned long long> T;
@@ -297,8 +326,12 @@ __global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_cons
 
 }  // namespace
 
+cudaError_t configure_overflow_kernel() {
+  return cudaFuncSetAttribute(overflow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OVF_SMEM);
+}
+
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
-  overflow_kernel<<<n_sm, OVF_THREADS, 0, stream>>>(c);
+  overflow_kernel<<<n_sm * 4, OVF_THREADS, OVF_SMEM, stream>>>(c);
 }
 
 }  // namespace pix

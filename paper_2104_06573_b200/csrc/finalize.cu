@@ -2,9 +2,10 @@
 // cluStart[i]), followed by the prefix sum the figure leaves implicit, S19), the scatter of the temp
 // cluster records to their final place clus_module_start[module] + local id (S14), and the summary (S20).
 //
-// Grid (NB, events of the chunk).  Every block of an event recomputes the event's M-entry scan in shared
-// memory (warp-shuffle scan; a few KB), then copies a slice of the records: one thread per output record,
-// module found by binary search in the shared offsets.  Block 0 also writes the offsets and the summary.
+// Two kernels.  offsets: one block per event computes the event's M-entry scan (warp-shuffle scan), writes the
+// offsets and the summary, and appends the event's record slices (SLICE records each) to a work list.
+// scatter: a persistent grid takes slices from the list; a block stages the event's offsets in shared memory
+// and copies its records, one thread per output record, module found by binary search in the shared offsets.
 #include "pix_common.cuh"
 
 namespace pix {
@@ -22,11 +23,13 @@ __device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, uint32_t lan
   return v;
 }
 
-__global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_constant__ Chunk c) {
+constexpr uint32_t SLICE = 1024;  // records per scatter work item
+
+__global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ uint32_t s_start[];  // [M+1]
   __shared__ uint32_t s_warp[FIN_THREADS / 32];
   __shared__ uint32_t s_red[8];
-  const uint32_t er = blockIdx.y, e = c.e0 + er, M = c.M;
+  const uint32_t er = blockIdx.x, e = c.e0 + er, M = c.M;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t flags = c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS];
   const bool skip = (flags & FLAG_NONCONTIGUOUS) != 0;  // S11: clustering is not defined for such an event
@@ -58,68 +61,90 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
   const uint32_t ebase = c.segB[er * c.F];
   const uint32_t n_words = c.segB[(er + 1u) * c.F] - ebase;
 
-  // ---- block 0: offsets + summary
-  if (blockIdx.x == 0) {
-    uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
-    for (uint32_t m = tid; m <= M; m += FIN_THREADS) cms[m] = s_start[m];
-    uint32_t acc[2] = {0, 0};  // modules present, clusters surviving the cut
-    for (uint32_t m = tid; m < M; m += FIN_THREADS) {
-      const bool present = c.module_end[(size_t)e * M + m] > 0u;
-      if (!present) c.module_first[(size_t)e * M + m] = 0u;  // S12: absent -> 0,0 (init left the atomicMin sentinel)
-      acc[0] += present ? 1u : 0u;
-      acc[1] += skip ? 0u : n_clus[m];
-    }
+  // ---- offsets + summary + work items
+  uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
+  for (uint32_t m = tid; m <= M; m += FIN_THREADS) cms[m] = s_start[m];
+  uint32_t acc[2] = {0, 0};  // modules present, clusters surviving the cut
+  for (uint32_t m = tid; m < M; m += FIN_THREADS) {
+    const bool present = c.module_end[(size_t)e * M + m] > 0u;
+    if (!present) c.module_first[(size_t)e * M + m] = 0u;  // S12: absent -> 0,0 (init left the atomicMin sentinel)
+    acc[0] += present ? 1u : 0u;
+    acc[1] += skip ? 0u : n_clus[m];
+  }
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const uint32_t v = __reduce_add_sync(0xFFFFFFFFu, acc[k]);
-      if (lane == 0 && v) atomicAdd(s_red + k, v);
-    }
-    __syncthreads();
-    if (tid == 0) {
-      const uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
-      uint32_t* s = c.summary + (size_t)e * 16;
-      const uint32_t bad = ec[EC_EMPTY] + ec[EC_ERR_LINK] + ec[EC_ERR_ROC] + ec[EC_ERR_DCOL] + ec[EC_ERR_PXID];
-      s[0] = n_words; s[1] = n_words - bad; s[2] = ec[EC_EMPTY];
-      s[3] = ec[EC_ERR_LINK]; s[4] = ec[EC_ERR_ROC]; s[5] = ec[EC_ERR_DCOL]; s[6] = ec[EC_ERR_PXID];
-      s[7] = ec[EC_DUP]; s[8] = ec[EC_BELOW]; s[9] = ec[EC_OK]; s[10] = ec[EC_CUT];
-      s[11] = s_red[0]; s[12] = ec[EC_PRECUT]; s[13] = s_red[1]; s[14] = n_emit;
-      s[15] = flags | (total > c.cap_ev ? FLAG_CAPACITY : 0u);
+  for (int k = 0; k < 2; ++k) {
+    const uint32_t v = __reduce_add_sync(0xFFFFFFFFu, acc[k]);
+    if (lane == 0 && v) atomicAdd(s_red + k, v);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    const uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
+    uint32_t* s = c.summary + (size_t)e * 16;
+    const uint32_t bad = ec[EC_EMPTY] + ec[EC_ERR_LINK] + ec[EC_ERR_ROC] + ec[EC_ERR_DCOL] + ec[EC_ERR_PXID];
+    s[0] = n_words; s[1] = n_words - bad; s[2] = ec[EC_EMPTY];
+    s[3] = ec[EC_ERR_LINK]; s[4] = ec[EC_ERR_ROC]; s[5] = ec[EC_ERR_DCOL]; s[6] = ec[EC_ERR_PXID];
+    s[7] = ec[EC_DUP]; s[8] = ec[EC_BELOW]; s[9] = ec[EC_OK]; s[10] = ec[EC_CUT];
+    s[11] = s_red[0]; s[12] = ec[EC_PRECUT]; s[13] = s_red[1]; s[14] = n_emit;
+    s[15] = flags | (total > c.cap_ev ? FLAG_CAPACITY : 0u);
+    const uint32_t nsl = (n_emit + SLICE - 1u) / SLICE;
+    if (nsl) {
+      const uint32_t at = atomicAdd(c.ctl + CTL_SLICE_COUNT, nsl);
+      for (uint32_t q = 0; q < nsl; ++q) c.slice_list[at + q] = (er << 16) | q;  // cap_ev <= 2^26 records (pix_create)
     }
   }
-
-  // ---- records: output record g of the event <- temp record (run first + local id)
-  const uint32_t rel = ebase - c.segB[0];
-  for (uint32_t g = blockIdx.x * FIN_THREADS + tid; g < n_emit; g += gridDim.x * FIN_THREADS) {
-    uint32_t lo = 0, hi = M;  // last m with s_start[m] <= g
-    while (lo < hi) {
-      const uint32_t mid = (lo + hi + 1u) >> 1;
-      if (s_start[mid] <= g) lo = mid; else hi = mid - 1u;
-    }
-    const uint32_t src = rel + c.module_first[(size_t)e * M + lo] + (g - s_start[lo]);
-    const size_t o = (size_t)e * c.cap_ev + g;
-    c.c_module[o] = (uint16_t)lo;
-    c.c_first[o] = c.t_first[src]; c.c_npix[o] = c.t_npix[src]; c.c_charge[o] = c.t_charge[src];
-    c.c_x[o] = c.t_x[src]; c.c_y[o] = c.t_y[src];
-  }
-
   // ---- an event whose modules are not contiguous was not clustered: define clus for its decodable words
   if (skip) {
-    for (uint32_t i = blockIdx.x * FIN_THREADS + tid; i < n_words; i += gridDim.x * FIN_THREADS)
-      c.d_clus[(size_t)ebase + i] = -1;
+    for (uint32_t i = tid; i < n_words; i += FIN_THREADS) c.d_clus[(size_t)ebase + i] = -1;
+  }
+}
+
+// ---- records: output record g of the event <- temp record (run first + local id)
+__global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ uint32_t s_start[];  // [M+1]
+  const uint32_t M = c.M, tid = threadIdx.x;
+  const uint32_t count = c.ctl[CTL_SLICE_COUNT];
+  for (uint32_t it = blockIdx.x; it < count; it += gridDim.x) {
+    const uint32_t item = c.slice_list[it];
+    const uint32_t er = item >> 16, e = c.e0 + er, g0 = (item & 0xFFFFu) * SLICE;
+    const uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
+    __syncthreads();  // the previous item is done with s_start
+    for (uint32_t m = tid; m <= M; m += FIN_THREADS) s_start[m] = cms[m];
+    __syncthreads();
+    const uint32_t total = s_start[M];
+    const uint32_t n_emit = total < c.cap_ev ? total : c.cap_ev;
+    const uint32_t rel = c.segB[er * c.F] - c.segB[0];
+    const uint32_t* mfirst = c.module_first + (size_t)e * M;
+#pragma unroll
+    for (uint32_t j = 0; j < SLICE / FIN_THREADS; ++j) {
+      const uint32_t g = g0 + j * FIN_THREADS + tid;
+      if (g >= n_emit) continue;
+      uint32_t lo = 0, hi = M;  // last m with s_start[m] <= g
+      while (lo < hi) {
+        const uint32_t mid = (lo + hi + 1u) >> 1;
+        if (s_start[mid] <= g) lo = mid; else hi = mid - 1u;
+      }
+      const uint32_t src = rel + mfirst[lo] + (g - s_start[lo]);
+      const size_t o = (size_t)e * c.cap_ev + g;
+      c.c_module[o] = (uint16_t)lo;
+      c.c_first[o] = c.t_first[src]; c.c_npix[o] = c.t_npix[src]; c.c_charge[o] = c.t_charge[src];
+      c.c_x[o] = c.t_x[src]; c.c_y[o] = c.t_y[src];
+    }
   }
 }
 
 }  // namespace
 
 cudaError_t configure_finalize_kernel() {
-  return cudaFuncSetAttribute(finalize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
+  cudaError_t e = cudaFuncSetAttribute(offsets_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
 }
 
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream) {
   const uint32_t Ec = c.e1 - c.e0;
-  uint32_t nb = (uint32_t)(n_sm * 4) / Ec;
-  nb = nb < 1u ? 1u : (nb > 16u ? 16u : nb);
-  finalize_kernel<<<dim3(nb, Ec), FIN_THREADS, (size_t)(c.M + 1) * sizeof(uint32_t), stream>>>(c);
+  const size_t smem = (size_t)(c.M + 1) * sizeof(uint32_t);
+  offsets_kernel<<<Ec, FIN_THREADS, smem, stream>>>(c);
+  scatter_kernel<<<n_sm * 8, FIN_THREADS, smem, stream>>>(c);
 }
 
 }  // namespace pix

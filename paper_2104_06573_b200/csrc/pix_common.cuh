@@ -7,10 +7,11 @@
 // Kernel chain for one chunk of events:
 //   init      -> segment table, range sentinels, zeroed counters
 //   fused     -> a1 decode + a2 calibrate + a3 run boundaries + a4 findClus + a5 sums/cut/renumber for every
-//                module run that fits a block's 2048-word window (tile of 1024 words + look-ahead)
+//                module run that fits a warp's 256-word window (home chunk of 128 words + look-ahead)
 //   overflow  -> a4 + a5 for the runs the fused kernel could not take (longer than the window, pathological
 //                charge sums): generic block-per-run kernel, tables in global workspace
-//   finalize  -> a6 clamp + prefix scan (Fig. 3), record scatter, summary
+//   offsets   -> a6 clamp + prefix scan (Fig. 3), summary, scatter work list
+//   scatter   -> cluster records to their final place
 // Nothing here is shared with oracle/.
 #pragma once
 
@@ -33,7 +34,7 @@ constexpr uint32_t NO_INDEX = 0xFFFFFFFFu;
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
        EC_PRECUT, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_WORDS = 16 };
 
 // Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
 //   x = module | bad << 16 | scol << 24     bad: 0, ST_ERR_LINK or ST_ERR_ROC; scol = +1 / -1 (int8)
@@ -69,6 +70,7 @@ struct Chunk {
   uint32_t* ctl;            // [CTL_WORDS]
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
   uint32_t ovf_cap;
+  uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
   // temp cluster records, indexed by chunk-relative word index (run first + local id)
   uint32_t* t_first; uint32_t* t_npix; uint32_t* t_charge; float* t_x; float* t_y;
@@ -88,7 +90,8 @@ void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);
 cudaError_t configure_fused_kernel();
 cudaError_t configure_finalize_kernel();
+cudaError_t configure_overflow_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 4;    // init, fused, overflow, finalize
+constexpr int LAUNCHES_PER_CHUNK = 5;    // init, fused, overflow, offsets, scatter
 
 }  // namespace pix
