@@ -74,8 +74,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.ovf_cap = (uint32_t)(Ec * M);
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.n_clus = (uint32_t*)take(Ec * M * 4);
-  c.t_first = (uint32_t*)take(W * 4); c.t_npix = (uint32_t*)take(W * 4); c.t_charge = (uint32_t*)take(W * 4);
-  c.t_x = (float*)take(W * 4); c.t_y = (float*)take(W * 4);
+  c.t_rec = (pix::TempRec*)take(W * sizeof(pix::TempRec));
   c.g_hash = (unsigned long long*)take(W * 16);
   c.g_pos = (uint32_t*)take(W * 4); c.g_q = (uint32_t*)take(W * 4); c.g_npix = (uint32_t*)take(W * 4);
   c.g_sx = (unsigned long long*)take(W * 8); c.g_sy = (unsigned long long*)take(W * 8);

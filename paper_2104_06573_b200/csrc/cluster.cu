@@ -235,9 +235,8 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     if (root) {
       if (surv) {
         const uint32_t o = rb + id;
-        c.t_first[o] = first + k; c.t_npix[o] = T.npix[k]; c.t_charge[o] = Q;
-        c.t_x[o] = (float)((double)T.sx[k] / (double)Q);
-        c.t_y[o] = (float)((double)T.sy[k] / (double)Q);
+        put_temp(c.t_rec + o, first + k, T.npix[k], Q, (float)((double)T.sx[k] / (double)Q),
+                 (float)((double)T.sy[k] / (double)Q));
       }
       T.q[k] = surv ? id : NO_INDEX;
     }

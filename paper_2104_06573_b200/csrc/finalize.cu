@@ -126,8 +126,9 @@ __global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_const
       const uint32_t src = rel + mfirst[lo] + (g - s_start[lo]);
       const size_t o = (size_t)e * c.cap_ev + g;
       c.c_module[o] = (uint16_t)lo;
-      c.c_first[o] = c.t_first[src]; c.c_npix[o] = c.t_npix[src]; c.c_charge[o] = c.t_charge[src];
-      c.c_x[o] = c.t_x[src]; c.c_y[o] = c.t_y[src];
+      const uint4 a = c.t_rec[src].a;
+      const float y = c.t_rec[src].y;
+      c.c_first[o] = a.x; c.c_npix[o] = a.y; c.c_charge[o] = a.z; c.c_x[o] = __uint_as_float(a.w); c.c_y[o] = y;
     }
   }
 }

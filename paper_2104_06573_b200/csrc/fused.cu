@@ -139,41 +139,41 @@ __device__ __forceinline__ void push_overflow(const Chunk& c, uint32_t key) {
 }
 
 // ------------------------------------------------------------------ the fused warp kernel
-constexpr int WPB = 8;                    // warps per block (they share nothing but the block)
+constexpr int WPB = 4;                    // warps per block (they share nothing but the block)
 constexpr int FT = WPB * 32;
 constexpr uint32_t HC = 128;              // words of a home chunk (rounds 0-3)
 constexpr uint32_t MAXT = 256;            // window: home chunk + up to 4 extension rounds
-constexpr uint32_t WTAB = 1024;           // hash slots per warp
+constexpr uint32_t WTAB = 512;            // hash slots per warp
 constexpr uint32_t RC = 62;               // runs a warp can own
 constexpr uint32_t ECAP = 3 * MAXT;       // at most 3 forward edges per digi
 constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
 constexpr uint32_t HASH_MUL = 0x9E3779B1u;
-constexpr uint32_t KEY_BITS = 23, KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = 13, TAG_MASK = (1u << TAG_BITS) - 1u;
+constexpr uint32_t KEY_BITS = 23, KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = 14, TAG_MASK = (1u << TAG_BITS) - 1u;
 static_assert(((RC + 1u) << 17) <= (1u << KEY_BITS) && (1u << (KEY_BITS - TAG_BITS)) == WTAB && MAXT <= 256,
-              "key: run (6 bits) | row (8) | col (9); slot: disp (10) | tag (13) | digi (8) | below (1)");
+              "key: run (6 bits) | row (8) | col (9); slot: disp (9) | tag (14) | digi (8) | below (1)");
 
 // digi key inside the window: run (6 bits) | row (8 bits) | col (9 bits).  Neighbour keys are key+1 (col+1)
 // and key+512-1, +512, +512+1 (row+1): col 416..511 and row 160..255 never occur, so no bounds checks (S13).
 struct __align__(16) WarpSmem {
-  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D: qn = tab, sx = tab + 256, sy = tab + 512,
-                           // id = tab + 768
+  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D, tab + edge: qn = tab, sx = tab + 256, sy = tab + 512
+  uint16_t edge[ECAP];     // a | b << 8
   uint32_t dkey[MAXT];     // key of the digi in window slot t (word b + t), INVALID if not owned / undecodable
   uint32_t label[MAXT];    // union-find parent, or MARK_*
-  uint16_t chg[MAXT];      // charge
-  uint16_t edge[ECAP];     // a | b << 8
+  uint16_t chg[MAXT];      // charge; after phase E: local id of a root, or NO_ID
   uint32_t run_ifirst[RC + 2];  // event-relative index of the run's first digi
   uint32_t run_key[RC + 2];     // event_rel << 16 | module
   uint16_t run_first[RC + 2];   // window slot of the run's first digi
   uint16_t run_base[RC + 2];    // survivors before the run
   uint8_t run_bad[RC + 2];      // the run is left to the overflow kernel
 };
+static_assert(WTAB * 4 + ECAP * 2 >= 3 * MAXT * 4 + MAXT, "the sums and the root list fit in tab + edge");
 static_assert(sizeof(WarpSmem) % 16 == 0, "per-warp slices stay 16-byte aligned");
 
 // Position hash, open addressing, one word per slot.  h = key * HASH_MUL mod 2^23 is a bijection on the 23-bit
-// keys; home slot = top 10 bits of h, tag = the other 13, so (home, tag) names the key exactly.  A key stored
-// i slots after its home records the displacement: slot = disp (10) | tag (13) | digi (8) | below_threshold (1).
+// keys; home slot = top 9 bits of h, tag = the other 14, so (home, tag) names the key exactly.  A key stored
+// i slots after its home records the displacement: slot = disp (9) | tag (14) | digi (8) | below_threshold (1).
 // Slots are never emptied; equal keys meet in one slot and keep the lowest digi (S10).
 __device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
 
@@ -187,7 +187,7 @@ __device__ __forceinline__ bool hinsert(WarpSmem& s, uint32_t key, uint32_t t, u
     const uint32_t old = atomicCAS(&s.tab[p], EMPTY, mine);
     if (old == EMPTY) return false;
     if ((old >> 9) == want) { atomicMin(&s.tab[p], mine); return true; }  // same pixel: the lowest digi owns it
-    p = (p + 1u) & (WTAB - 1u); want += 1u << TAG_BITS;  // at most 256 of the 1024 slots are ever taken
+    p = (p + 1u) & (WTAB - 1u); want += 1u << TAG_BITS;  // at most 256 of the 512 slots are ever taken
   }
 }
 // slot contents of the key whose mixed value is h, or EMPTY
@@ -215,13 +215,16 @@ __device__ __forceinline__ uint32_t uf_find(volatile uint32_t* L, uint32_t x) {
   return x;
 }
 __device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
-  while (true) {
+  bool done = false;  // single exit: the lanes of a warp reconverge after the loop
+  while (!done) {
     a = uf_find(L, a); b = uf_find(L, b);
-    if (a == b) return;
-    if (a < b) { const uint32_t t = a; a = b; b = t; }
-    const uint32_t old = atomicMin(L + a, b);  // hook the larger root under the smaller
-    if (old == a) return;
-    a = old;                                   // a was no longer a root: keep merging its parent with b
+    if (a == b) { done = true; }
+    else {
+      if (a < b) { const uint32_t t = a; a = b; b = t; }
+      const uint32_t old = atomicMin(L + a, b);  // hook the larger root under the smaller
+      if (old == a) done = true;
+      else a = old;                            // a was no longer a root: keep merging its parent with b
+    }
   }
 }
 
@@ -236,7 +239,7 @@ __device__ __forceinline__ void seg_of(const uint32_t* __restrict__ segB, uint32
   }
 }
 
-__global__ void __launch_bounds__(FT, 3) fused_kernel(const __grid_constant__ Chunk c) {
+__global__ void __launch_bounds__(FT, 8) fused_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   WarpSmem& s = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
@@ -248,8 +251,11 @@ __global__ void __launch_bounds__(FT, 3) fused_kernel(const __grid_constant__ Ch
   const uint32_t n_chunks = (gEnd - T0 + HC - 1u) / HC;
   const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
   constexpr uint32_t FULL = 0xFFFFFFFFu;
-  uint32_t* const qn = s.tab; uint32_t* const sx = s.tab + MAXT; uint32_t* const sy = s.tab + 2 * MAXT;
-  uint32_t* const lid = s.tab + 3 * MAXT;
+  uint32_t* const w0 = reinterpret_cast<uint32_t*>(&s);  // tab + edge, reused after phase D
+  uint32_t* const qn = w0; uint32_t* const sx = w0 + MAXT; uint32_t* const sy = w0 + 2 * MAXT;
+  uint16_t* const lid = s.chg;
+  uint8_t* const rlist = reinterpret_cast<uint8_t*>(w0 + 3 * MAXT);  // roots in digi order (after phase D)
+  constexpr uint32_t NO_ID = 0xFFFFu;
 
   for (uint32_t ci = blockIdx.x * WPB + warp; ci < n_chunks; ci += gridDim.x * WPB) {
     const uint32_t b = T0 + ci * HC;
@@ -436,75 +442,88 @@ __global__ void __launch_bounds__(FT, 3) fused_kernel(const __grid_constant__ Ch
       ne += __popc(m2);
     }
     __syncwarp();
-    for (uint32_t i = lane; i < ne; i += 32u) {
-      const uint32_t e = s.edge[i];
-      uf_unite(s.label, e & 0xFFu, e >> 8);
+    for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
+      if (i0 + lane < ne) {
+        const uint32_t e = s.edge[i0 + lane];
+        uf_unite(s.label, e & 0xFFu, e >> 8);
+      }
+      __syncwarp();
     }
     __syncwarp();  // components complete; the hash is dead, its memory becomes qn / sx / sy / lid
 
-    // ================================================================== E: cluster sums
+    // ================================================================== E: cluster sums; dense list of the roots
     {
-      uint4* t4 = reinterpret_cast<uint4*>(s.tab);
+      uint4* t4 = reinterpret_cast<uint4*>(w0);
       const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
       for (int k = 0; k < (int)(3 * MAXT / 4 / 32); ++k) t4[lane + 32 * k] = z4;
     }
     __syncwarp();
+    uint32_t nr = 0u;  // roots so far
 #pragma unroll 1
     for (uint32_t k = k0; k < k1; ++k) {
       const uint32_t t = 32u * k + lane;
       volatile uint32_t* L = s.label;
       uint32_t r = L[t];
-      if (r >= MAXT) continue;  // MARK_*
-      while (true) { const uint32_t n = L[r]; if (n == r) break; r = n; }
-      L[t] = r;  // flatten: r is the root, so other walkers through t stay correct
-      const uint32_t key = s.dkey[t], e = s.chg[t];
-      atomicAdd(&qn[r], e | (1u << 24));  // charge sum (< 2^24: 256 * 65535) | pixel count (256 wraps to 0)
-      atomicAdd(&sx[r], e * (key & 511u));
-      atomicAdd(&sy[r], e * ((key >> 9) & 255u));
+      const bool live = r < MAXT;  // else MARK_*
+      if (live) {
+        while (true) { const uint32_t n = L[r]; if (n == r) break; r = n; }
+        L[t] = r;  // flatten: r is the root, so other walkers through t stay correct
+        const uint32_t key = s.dkey[t], e = s.chg[t];
+        atomicAdd(&qn[r], e | (1u << 24));  // charge sum (< 2^24: 256 * 65535) | pixel count (256 wraps to 0)
+        atomicAdd(&sx[r], e * (key & 511u));
+        atomicAdd(&sy[r], e * ((key >> 9) & 255u));
+      }
+      const bool root = live && r == t;
+      const uint32_t rm = __ballot_sync(FULL, root);
+      if (root) rlist[nr + __popc(rm & lt_mask)] = (uint8_t)t;  // digi order
+      nr += __popc(rm);
     }
     __syncwarp();
 
-    // ================================================================== F: cut, renumber, temp records
+    // ================================================================== F: cut, renumber, temp records (one root per lane)
     {
-      uint32_t cnt = 0u;  // surviving roots before this round
+      uint32_t cnt = 0u;      // surviving roots before this iteration
+      uint32_t crun = 0u;     // run of the last surviving root so far (runs 1 .. crun have their run_base)
       const uint32_t relb = b - gBeg;  // may wrap for the first chunk; only used added to a slot >= gBeg - b
 #pragma unroll 1
-      for (uint32_t k = k0; k < k1; ++k) {
-        const uint32_t t = 32u * k + lane, key = s.dkey[t];
-        const bool dec = key != INVALID;
-        const bool root = dec && s.label[t] == t;
-        const uint32_t r = dec ? key >> 17 : 0u;
-        const uint32_t rf = s.run_first[r];
-        uint32_t Q = 0u, np = 0u;
-        if (root) {
+      for (uint32_t i0 = 0u; i0 < nr; i0 += 32u) {
+        const bool valid = i0 + lane < nr;
+        uint32_t t = 0u, r = 0u, Q = 0u, np = 0u;
+        if (valid) {
+          t = rlist[i0 + lane];
+          r = s.dkey[t] >> 17;
           const uint32_t v = qn[t];
           Q = v & 0xFFFFFFu; np = v >> 24;
           if (np == 0u) np = 256u;
           if (Q > Q_SAFE) s.run_bad[r] = 1;  // 32-bit weighted sums may have wrapped
         }
-        const bool surv = root && (int32_t)Q >= c.cut;  // S9: equality keeps
+        const bool surv = valid && (int32_t)Q >= c.cut;  // S9: equality keeps
         const uint32_t sm = __ballot_sync(FULL, surv);
-        const uint32_t rank = cnt + __popc(sm & lt_mask);
-        if (dec && rf == t) s.run_base[r] = (uint16_t)rank;
-        if (root) {
-          uint32_t id = NO_INDEX;
-          if (surv) {
-            const uint32_t base = rf >= 32u * k ? cnt + __popc(sm & ((1u << (rf & 31u)) - 1u)) : s.run_base[r];
-            id = rank - base;
-            const uint32_t o = relb + rf + id;
-            c.t_first[o] = s.run_ifirst[r] + (t - rf);
-            c.t_npix[o] = np;
-            c.t_charge[o] = Q;
-            c.t_x[o] = (float)sx[t] / (float)Q;  // S18; exact integer sums, one rounding each (within 1e-5)
-            c.t_y[o] = (float)sy[t] / (float)Q;
-          }
-          lid[t] = id;
-        }
+        const uint32_t before = sm & lt_mask;
+        const uint32_t rank = cnt + __popc(before);
+        const int pl = before ? 31 - __clz(before) : 0;
+        uint32_t rp = __shfl_sync(FULL, r, pl);  // run of the previous surviving root
+        if (!before) rp = crun;
+        if (surv)
+          for (uint32_t q = rp + 1u; q <= r; ++q) s.run_base[q] = (uint16_t)rank;  // first survivor of run r
+        if (sm) crun = __shfl_sync(FULL, r, 31 - __clz(sm));
         cnt += __popc(sm);
-        __syncwarp();  // run_base of this round's runs is visible to later rounds
+        __syncwarp();
+        if (valid) {
+          uint32_t id = NO_ID;
+          if (surv) {
+            id = rank - s.run_base[r];
+            const uint32_t rf = s.run_first[r];
+            // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
+            const float fq = (float)Q;
+            put_temp(c.t_rec + (relb + rf + id), s.run_ifirst[r] + (t - rf), np, Q, __fdividef((float)sx[t], fq),
+                     __fdividef((float)sy[t], fq));
+          }
+          lid[t] = (uint16_t)id;
+        }
       }
-      if (lane == 0) s.run_base[Rn + 1u] = (uint16_t)cnt;
+      for (uint32_t q = crun + 1u + lane; q <= Rn + 1u; q += 32u) s.run_base[q] = (uint16_t)cnt;
     }
     __syncwarp();  // run_base, run_bad, local ids final
     for (uint32_t r = 1u + lane; r <= Rn; r += 32u) {
@@ -530,7 +549,7 @@ __global__ void __launch_bounds__(FT, 3) fused_kernel(const __grid_constant__ Ch
       else if (lab == MARK_BELOW) { so = ST_BELOW; cntA += 0x10000u; }
       else {
         const uint32_t id = lid[lab];
-        if (id != NO_INDEX) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
+        if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
         n_pre += lab == t ? 1u : 0u;
       }
       c.d_status[b + t] = (uint8_t)so; c.d_clus[b + t] = cl;
@@ -562,7 +581,7 @@ __global__ void __launch_bounds__(FT, 3) fused_kernel(const __grid_constant__ Ch
           if (lab == MARK_DUP) atomicAdd(ec + EC_DUP, 1u);
           else if (lab == MARK_BELOW) atomicAdd(ec + EC_BELOW, 1u);
           else {
-            atomicAdd(ec + (lid[lab] != NO_INDEX ? EC_OK : EC_CUT), 1u);
+            atomicAdd(ec + (lid[lab] != NO_ID ? EC_OK : EC_CUT), 1u);
             if (lab == t) atomicAdd(ec + EC_PRECUT, 1u);
           }
         }
@@ -590,7 +609,7 @@ cudaError_t configure_fused_kernel() {
 }
 
 void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
-  fused_kernel<<<grid_for(words_bound + 31u, WPB * HC, n_sm * 3), FT, WPB * sizeof(WarpSmem), stream>>>(c);
+  fused_kernel<<<grid_for(words_bound + 31u, WPB * HC, n_sm * 8), FT, WPB * sizeof(WarpSmem), stream>>>(c);
 }
 
 }  // namespace pix

@@ -42,6 +42,12 @@ enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_WORDS = 1
 // so that row = row0 + srow * (pxid >> 1), col = col0 + scol * (2*dcol + (pxid & 1)).
 typedef uint2 CabEntry;
 
+// temp cluster record (one 128-bit store + one 32-bit store; 32-byte stride)
+struct __align__(16) TempRec { uint4 a; float y; uint32_t pad[3]; };  // a = first_digi, n_pix, charge, x_col bits
+__device__ __forceinline__ void put_temp(TempRec* r, uint32_t first, uint32_t npix, uint32_t charge, float x, float y) {
+  r->a = make_uint4(first, npix, charge, __float_as_uint(x)); r->y = y;
+}
+
 // Everything a kernel needs for one chunk of events [e0, e1).  Passed by value (__grid_constant__).
 struct Chunk {
   // ---- input (device)
@@ -73,7 +79,7 @@ struct Chunk {
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
   // temp cluster records, indexed by chunk-relative word index (run first + local id)
-  uint32_t* t_first; uint32_t* t_npix; uint32_t* t_charge; float* t_x; float* t_y;
+  TempRec* t_rec;
   // overflow-kernel scratch, indexed by chunk-relative word index
   unsigned long long* g_hash;  // [2*cap_words]
   uint32_t* g_pos; uint32_t* g_q; uint32_t* g_npix; unsigned long long* g_sx; unsigned long long* g_sy;
