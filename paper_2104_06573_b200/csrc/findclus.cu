@@ -1,20 +1,16 @@
-// fused.cu -- init, and the fused warp kernel: a1 decode (S1-S6), a2 calibrate (S7-S9), a3 module
-// boundaries (S11, S12), a4 findClus (S10, S13) and a5 sums / charge cut / renumber / temp records (S9, S14,
-// S18) of the path PAPER.md:31 describes ("unpacks them, calibrates the individual pixels, and clusters the
-// pixels on each detector module"), in ONE pass over the raw words.
+// findclus.cu -- the warp cluster kernel: a4 findClus (S10, S13) and a5 sums / charge cut / renumber /
+// temp records (S9, S14, S18) of the path PAPER.md:31 describes ("clusters the pixels on each detector module").
 //
-// The word stream is cut into home chunks of 128 words, one warp per chunk, 32 words (one per lane) per round.
+// The word stream is cut into home chunks of 128 words, one warp per chunk, 32 digis (one per lane) per round.
 // A module's decodable words form one run (S11); a run belongs to the warp whose home chunk holds its first
-// word.  Warps never wait for each other (no block barrier); all tables are per-warp shared memory.  A warp
-//   A  clears its position hash, finds the (event, FED) segment of its chunk, and looks back for the last
-//      decodable word before the chunk (its run may continue into the chunk)
-//   B  home rounds 0-3: decodes + calibrates its 128 words, stores module/row/col/charge (and the final status
-//      of undecodable words), finds run starts with a ballot/shuffle "previous decodable word" scan (a3), and
-//      inserts every owned digi into the position hash keyed by (run, row, col); equal keys keep the lowest digi
-//   C  extension rounds 4-7: decodes on until the first word of another run, to complete its last run
+// word (the start bits come from decode.cu).  Warps never wait for each other (no block barrier); all tables are
+// per-warp shared memory.  A warp
+//   A  clears its position hash and reads the start bits of its window (home chunk + up to 128 more words)
+//   B  reads row / col / charge of the digis of its runs and inserts them into the position hash keyed by
+//      (run, row, col); equal keys keep the lowest digi (S10)
 //   D  looks up the forward neighbours of its digis, compacts the adjacent pairs into a dense edge list and
 //      unites them (lock-free min-index union-find, all lanes busy)
-//   E  every live digi adds charge | 1 << 24, charge*col, charge*row into its root's accumulators
+//   E  every live digi adds charge | 1 << 24, charge*col, charge*row into its root's accumulators; dense root list
 //   F  surviving roots (Q >= cut) are numbered in digi order per run (ballot/popc), temp records written
 //   G  final status and clus of every digi the warp owns; per-event counters
 // Runs that do not fit the 256-word window, chunks with more than RC runs and charge sums that could overflow
@@ -27,118 +23,11 @@ namespace {
 
 constexpr uint32_t NOKEY = 0xFFFFFFFFu;
 
-// ------------------------------------------------------------------ init
-// One warp per event of the chunk builds the clamped, monotone segment table
-//   segB[e_rel*F + f] = global word index where FED f of event e starts,  segB[Ec*F] = end of chunk.
-// Offsets are clamped into [lo, hi] (lo = start of chunk, hi = min(n_total, lo + cap_words)) so that
-// whatever the caller's offset arrays hold, every index derived later stays inside the buffers.
-// Other threads initialise the per-(event,module) range sentinels and zero the counters.
-__global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk c, uint32_t n_total) {
-  const uint32_t Ec = c.e1 - c.e0;
-  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
-  uint32_t lo = ev_offset(c, c.e0);
-  lo = lo < n_total ? lo : n_total;
-  const uint32_t room = n_total - lo;
-  const uint32_t hi = lo + (room < c.cap_words ? room : c.cap_words);
-  if (tid < CTL_WORDS) c.ctl[tid] = 0;
-  // one warp per event: lanes take FEDs, the running max over the clamped offsets is a warp max-scan
-  const uint32_t lane = threadIdx.x & 31u, wid = tid >> 5, nwarp = nth >> 5;
-  for (uint32_t er = wid; er < Ec; er += nwarp) {
-    const uint32_t e = c.e0 + er;
-    const uint32_t rb = ev_offset(c, e), re = ev_offset(c, e + 1);
-    const uint32_t b = rb < lo ? lo : (rb > hi ? hi : rb);
-    const uint32_t en = re < b ? b : (re > hi ? hi : re);
-    const uint32_t nw = en - b;
-    const uint32_t flags = (re > hi || rb > hi || re < rb || rb < lo) ? FLAG_TOO_LARGE : 0u;
-    uint32_t carry = 0;
-    for (uint32_t f0 = 0; f0 < c.F; f0 += 32u) {
-      const uint32_t f = f0 + lane;
-      uint32_t fo = (f == 0 || f >= c.F || !c.fed_off) ? 0u : c.fed_off[(size_t)e * (c.F + 1) + f];
-      fo = fo > nw ? nw : fo;
-      fo = fo > carry ? fo : carry;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, fo, d);
-        if (lane >= (uint32_t)d && o > fo) fo = o;
-      }
-      if (f < c.F) c.segB[er * c.F + f] = b + fo;  // monotone by construction
-      carry = __shfl_sync(0xFFFFFFFFu, fo, 31);
-    }
-    if (er == Ec - 1 && lane == 0) c.segB[Ec * c.F] = en;
-    if (lane < EC_STRIDE) c.ev_cnt[(size_t)er * EC_STRIDE + lane] = (lane == EC_FLAGS) ? flags : 0u;
-  }
-  const uint32_t nmod = Ec * c.M;
-  uint32_t* mf = c.module_first + (size_t)c.e0 * c.M;
-  uint32_t* me = c.module_end + (size_t)c.e0 * c.M;
-  for (uint32_t t = tid; t < nmod; t += nth) { mf[t] = NO_INDEX; me[t] = 0u; c.n_clus[t] = 0u; }
-}
-
-// ------------------------------------------------------------------ decode / calibrate
-// S1-S6 with the pre-digested cabling entry (pix_common.cuh).  Returns the status; module/row/col are defined
-// only for ST_OK.  fedbase = fed * 2048.
-__device__ __forceinline__ uint32_t decode_word(const CabEntry* __restrict__ cab, uint32_t w, uint32_t fedbase,
-                                                uint32_t& module, uint32_t& row, uint32_t& col) {
-  const CabEntry e = __ldg(cab + fedbase + (w >> 21));  // index (fed*64 + link)*32 + roc
-  const uint32_t dcol = (w >> 16) & 31u, pxid = (w >> 8) & 255u;
-  const uint32_t bad = (e.x >> 16) & 0xFFu;
-  uint32_t st = ST_OK;
-  if (pxid >= 160u) st = ST_ERR_PXID;
-  if (dcol >= 26u) st = ST_ERR_DCOL;
-  if (bad) st = bad;
-  if (w == 0u) st = ST_EMPTY;
-  const int rr = (int)(pxid >> 1), cc = (int)(2u * dcol + (pxid & 1u));
-  module = e.x & 0xFFFFu;
-  row = (uint32_t)((int)(e.y & 0xFFu) + rr * ((int)e.y >> 24));
-  col = (uint32_t)((int)((e.y >> 8) & 0x1FFu) + cc * ((int)e.x >> 24));
-  return st;
-}
-
-// S7: four separately rounded binary32 RN operations (the _rn intrinsics are never contracted to FMA),
-// then NaN/negative -> 0, clamp, truncate.
-__device__ __forceinline__ int32_t calibrate(const Chunk& c, uint32_t adc, float2 gp) {
-  const float f1 = __fsub_rn((float)adc, gp.y);
-  const float f2 = __fmul_rn(f1, gp.x);
-  const float f3 = __fmul_rn(f2, c.vcal_gain);
-  const float f4 = __fadd_rn(f3, c.vcal_offset);
-  if (!(f4 >= 0.0f)) return 0;
-  return __float2int_rz(fminf(f4, c.max_e_f));
-}
-
-// last s in [0, S) with segB[s] <= g, given segB[0] <= g < segB[S]; warp-cooperative 32-ary search
-__device__ __forceinline__ uint32_t warp_find_segment(const uint32_t* __restrict__ segB, uint32_t S, uint32_t g,
-                                                      uint32_t lane) {
-  uint32_t lo = 0, hi = S;  // invariant: segB[lo] <= g < segB[hi]
-  while (hi - lo > 1) {
-    const uint32_t step = (hi - lo + 31u) / 32u;
-    const uint32_t p = lo + (lane + 1u) * step;
-    const bool le = (p < hi) && (segB[p] <= g);
-    const uint32_t cnt = __popc(__ballot_sync(0xFFFFFFFFu, le));
-    const uint32_t nlo = lo + cnt * step;
-    const uint32_t nhi = nlo + step;
-    lo = nlo;
-    hi = nhi < hi ? nhi : hi;
-  }
-  return lo;
-}
-
-// a3: module_first / module_end are keyed by module id (S12); a second run of a module flags the event (S11)
-__device__ __forceinline__ uint32_t run_start(const Chunk& c, uint32_t key, uint32_t g) {
-  const uint32_t er = key >> 16, m = key & 0xFFFFu;
-  const uint32_t i = g - c.segB[er * c.F];
-  const uint32_t old = atomicMin(c.module_first + ((size_t)(c.e0 + er) * c.M + m), i);
-  if (old != NO_INDEX) atomicOr(c.ev_cnt + (size_t)er * EC_STRIDE + EC_FLAGS, FLAG_NONCONTIGUOUS);
-  return i;
-}
-__device__ __forceinline__ void run_end(const Chunk& c, uint32_t key, uint32_t g) {
-  const uint32_t er = key >> 16, m = key & 0xFFFFu;
-  atomicMax(c.module_end + ((size_t)(c.e0 + er) * c.M + m), g - c.segB[er * c.F] + 1u);
-}
 __device__ __forceinline__ void push_overflow(const Chunk& c, uint32_t key) {
   const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u);
   if (i < c.ovf_cap) c.ovf_list[i] = (key >> 16) * c.M + (key & 0xFFFFu);
 }
 
-// ------------------------------------------------------------------ the fused warp kernel
 constexpr int WPB = 4;                    // warps per block (they share nothing but the block)
 constexpr int FT = WPB * 32;
 constexpr uint32_t HC = 128;              // words of a home chunk (rounds 0-3)
@@ -229,17 +118,7 @@ __device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
 }
 
 // (event, FED) of word g >= b, given the segment sg0 of the chunk's first word and the next boundary nextB0
-__device__ __forceinline__ void seg_of(const uint32_t* __restrict__ segB, uint32_t S, uint32_t F, uint32_t g, uint32_t sg0,
-                                       uint32_t nextB0, uint32_t er0, uint32_t fed0, uint32_t& er, uint32_t& fed) {
-  er = er0; fed = fed0;
-  if (g >= nextB0) {  // rare: a FED / event boundary inside the window (g < segB[S] always)
-    uint32_t sg = sg0 + 1u;
-    while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
-    er = sg / F; fed = sg - er * F;
-  }
-}
-
-__global__ void __launch_bounds__(FT, 8) fused_kernel(const __grid_constant__ Chunk c) {
+__global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   WarpSmem& s = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
@@ -247,7 +126,7 @@ __global__ void __launch_bounds__(FT, 8) fused_kernel(const __grid_constant__ Ch
   const uint32_t* __restrict__ segB = c.segB;
   const uint32_t gBeg = segB[0], gEnd = segB[S];
   if (gBeg >= gEnd) return;
-  const uint32_t T0 = gBeg & ~31u;  // rounds are 128-byte aligned
+  const uint32_t T0 = gBeg & ~(CHUNK_WORDS - 1u);
   const uint32_t n_chunks = (gEnd - T0 + HC - 1u) / HC;
   const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
   constexpr uint32_t FULL = 0xFFFFFFFFu;
@@ -259,13 +138,11 @@ __global__ void __launch_bounds__(FT, 8) fused_kernel(const __grid_constant__ Ch
 
   for (uint32_t ci = blockIdx.x * WPB + warp; ci < n_chunks; ci += gridDim.x * WPB) {
     const uint32_t b = T0 + ci * HC;
-    // ================================================================== A: load; clear; segment; look-back
-    uint32_t w[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const uint32_t g = b + 32u * k + lane;
-      w[k] = (g >= gBeg && g < gEnd) ? __ldg(c.words + g) : 0u;
-    }
+    // ================================================================== A: start bits of the window; clear
+    uint32_t sbv = 0u;  // lane k < 8: start bits of round k
+    if (lane < 8u && ci * 4u + lane < n_chunks * 4u) sbv = c.startbits[ci * 4u + lane];
+    const uint32_t home = __ballot_sync(FULL, lane < 4u && sbv != 0u);
+    if (!home) continue;  // no run starts here: nothing owned
     {
       uint4* t4 = reinterpret_cast<uint4*>(s.tab);
       const uint4 e4 = make_uint4(EMPTY, EMPTY, EMPTY, EMPTY);
@@ -273,139 +150,73 @@ __global__ void __launch_bounds__(FT, 8) fused_kernel(const __grid_constant__ Ch
       for (int k = 0; k < (int)(WTAB / 4 / 32); ++k) t4[lane + 32 * k] = e4;
       if (lane < (RC + 2u) / 4u) reinterpret_cast<uint32_t*>(s.run_bad)[lane] = 0u;
     }
-    const uint32_t gw = b < gBeg ? gBeg : b;  // b < gEnd by the chunk count
-    const uint32_t sg0 = warp_find_segment(segB, S, gw, lane);
-    const uint32_t er0 = sg0 / F, fed0 = sg0 - er0 * F, nextB0 = segB[sg0 + 1u];
-    uint32_t ckey = NOKEY, cg = 0u;  // last decodable word so far (warp-uniform)
-    {
-      uint32_t g = gw;  // words [gBeg, g) are still to be searched, backwards
-      while (g > gBeg) {
-        const bool in = lane < g - gBeg;
-        const uint32_t gi = g - 1u - lane;
-        uint32_t key = NOKEY;
-        if (in) {
-          uint32_t sg = sg0;
-          while (segB[sg] > gi) --sg;  // segB[0] = gBeg <= gi
-          const uint32_t er = sg / F, fed = sg - er * F;
-          uint32_t m, r, cc;
-          if (decode_word(c.cab, __ldg(c.words + gi), fed << 11, m, r, cc) == ST_OK) key = (er << 16) | m;
-        }
-        const uint32_t bal = __ballot_sync(FULL, key != NOKEY);
-        if (bal) {
-          const int src = __ffs(bal) - 1;
-          ckey = __shfl_sync(FULL, key, src);
-          cg = g - 1u - (uint32_t)src;
-          break;
-        }
-        g = (g - gBeg > 32u) ? g - 32u : gBeg;
-      }
+    uint32_t sb[8], rb[8];  // start bits of round k; runs started before round k (warp-uniform)
+    uint32_t R = 0u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      sb[k] = __shfl_sync(FULL, sbv, k);
+      rb[k] = R;
+      if (k < 4) R += __popc(sb[k]);
     }
+    const uint32_t kf = (uint32_t)__ffs(home) - 1u;
+    const uint32_t f_t = 32u * kf + (uint32_t)__ffs(__shfl_sync(FULL, sbv, kf)) - 1u;  // first owned slot
+    // end of the last run: the first start bit after the home chunk, the end of the data, or "does not fit"
+    const uint32_t ext = __ballot_sync(FULL, lane >= 4u && lane < 8u && sbv != 0u);
+    uint32_t e_t;
+    bool fits = true;
+    if (ext) {
+      const uint32_t ke = (uint32_t)__ffs(ext) - 1u;
+      e_t = 32u * ke + (uint32_t)__ffs(__shfl_sync(FULL, sbv, ke)) - 1u;
+    } else if (b + MAXT >= gEnd) {
+      e_t = gEnd - b;
+    } else {
+      fits = false; e_t = MAXT;
+    }
+    const uint32_t Rn = R < RC ? R : RC;
     __syncwarp();  // the cleared hash is visible
 
-    // ================================================================== B: home rounds
-    uint32_t R = 0u;        // runs started in the home chunk so far
-    uint32_t f_t = MAXT;    // window slot of the first owned digi
+    // ================================================================== B: stage + insert the digis of the owned runs
     bool dup_seen = false;
+    const uint32_t kl = (e_t + 31u) >> 5;  // rounds kf .. kl-1 hold the window
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (uint32_t k = 0; k < 8; ++k) {
+      if (k < kf || k >= kl) continue;  // warp-uniform
       const uint32_t t = 32u * k + lane, g = b + t;
-      const bool in = g >= gBeg && g < gEnd;
-      uint32_t er, fed;
-      seg_of(segB, S, F, g, sg0, nextB0, er0, fed0, er, fed);
-      uint32_t m = 0xFFFFu, row = 0xFFFFu, col = 0xFFFFu, st = 0xFFu;
+      const uint32_t r = (k < 4u ? rb[k] : R) + __popc(sb[k] & le_mask & (k < 4u ? FULL : 0u));
+      const bool in = t >= f_t && t < e_t && r <= RC;
+      uint32_t row = 0xFFFFu, col = 0u;
       int32_t e = 0;
-      bool dec = false;
-      if (in) {
-        uint32_t dm, dr, dc;
-        st = decode_word(c.cab, w[k], fed << 11, dm, dr, dc);
-        dec = st == ST_OK;
-        if (dec) {
-          m = dm; row = dr; col = dc;
-          const float2 gp = __ldg(c.gp + (m * (uint32_t)COLS + col));  // S8: one pair per (module, col)
-          e = calibrate(c, w[k] & 255u, gp);
-          if (e < c.thr) st = ST_BELOW;                                // S9
-        } else {  // undecodable: finished here
-          atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
-          c.d_status[g] = (uint8_t)st; c.d_clus[g] = -1;
-        }
-        c.d_module[g] = (uint16_t)m; c.d_row[g] = (uint16_t)row; c.d_col[g] = (uint16_t)col; c.d_charge[g] = e;
+      if (in) { row = c.d_row[g]; col = c.d_col[g]; e = c.d_charge[g]; }
+      if (in && k < 4u && (sb[k] >> lane & 1u)) {  // the first digi of run r
+        uint32_t sg = c.chunk_seg[ci];
+        while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
+        const uint32_t er = sg / F;
+        s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | c.d_module[g]; s.run_ifirst[r] = g - segB[er * F];
       }
-      // ---- a3: previous decodable word of every lane (ballot + shuffle, carry across rounds)
-      const uint32_t key = dec ? ((er << 16) | m) : NOKEY;
-      const uint32_t has = __ballot_sync(FULL, dec);
-      const uint32_t below_l = has & lt_mask;
-      const int src = below_l ? 31 - __clz(below_l) : 0;
-      uint32_t pkey = __shfl_sync(FULL, key, src), pg = b + 32u * k + (uint32_t)src;
-      if (!below_l) { pkey = ckey; pg = cg; }
-      const bool start = dec && key != pkey;
-      uint32_t ifirst = 0u;
-      if (start) {
-        ifirst = run_start(c, key, g);
-        if (pkey != NOKEY) run_end(c, pkey, pg);
-      }
-      const uint32_t sm = __ballot_sync(FULL, start);
-      const uint32_t r = R + __popc(sm & le_mask);  // run of this word; 0: a run of an earlier chunk
-      if (start) {
-        if (r <= RC) { s.run_first[r] = (uint16_t)t; s.run_ifirst[r] = ifirst; s.run_key[r] = key; }
-        else push_overflow(c, key);
-      }
-      const bool own = dec && r >= 1u && r <= RC;
-      const uint32_t dk = own ? ((r << 17) | (row << 9) | col) : INVALID;
+      const bool dec = in && row != 0xFFFFu;
+      const bool below = e < c.thr;  // S9
+      const uint32_t dk = dec ? ((r << 17) | (row << 9) | col) : INVALID;
       s.dkey[t] = dk;
-      s.label[t] = (own && st == ST_OK) ? t : MARK_BELOW;
+      s.label[t] = (dec && !below) ? t : MARK_BELOW;
       s.chg[t] = (uint16_t)e;
-      if (own) dup_seen |= hinsert(s, dk, t, st == ST_BELOW ? 1u : 0u);
-      if (has) {
-        const int top = 31 - __clz(has);
-        ckey = __shfl_sync(FULL, key, top); cg = b + 32u * k + (uint32_t)top;
-      }
-      if (R == 0u && sm) f_t = 32u * k + (uint32_t)(__ffs(sm) - 1);
-      R += __popc(sm);
-    }
-    if (ci == n_chunks - 1u && lane == 0 && ckey != NOKEY) run_end(c, ckey, cg);  // the chunk's last run
-    if (R == 0u) continue;  // nothing owned
-    const uint32_t Rn = R < RC ? R : RC;
-
-    // ================================================================== C: extension rounds for the last run
-    uint32_t n_t = HC;  // window slots staged
-    if (R <= RC) {
-      const uint32_t keyR = ckey;  // the last decodable word of the home chunk is in the last run
-      bool ended = b + HC >= gEnd;
-#pragma unroll 1
-      for (uint32_t k = 4; k < MAXT / 32u && !ended; ++k) {
-        const uint32_t t = 32u * k + lane, g = b + t;
-        const bool in = g < gEnd;
-        bool dec = false, stop = true;  // the end of the data stops the run
-        uint32_t key = NOKEY, m = 0, row = 0, col = 0, wv = 0;
-        if (in) {
-          uint32_t er, fed;
-          seg_of(segB, S, F, g, sg0, nextB0, er0, fed0, er, fed);
-          wv = __ldg(c.words + g);
-          dec = decode_word(c.cab, wv, fed << 11, m, row, col) == ST_OK;
-          key = (er << 16) | m;
-          stop = dec && key != keyR;
-        }
-        const uint32_t stopmask = __ballot_sync(FULL, stop);
-        const uint32_t first = stopmask ? (uint32_t)(__ffs(stopmask) - 1) : 32u;
-        const bool own = dec && lane < first;
-        uint32_t dk = INVALID, lb = MARK_BELOW;
-        if (own) {
-          const float2 gp = __ldg(c.gp + (m * (uint32_t)COLS + col));
-          const int32_t e = calibrate(c, wv & 255u, gp);
-          dk = (R << 17) | (row << 9) | col;
-          const bool below = e < c.thr;
-          if (!below) lb = t;
-          s.chg[t] = (uint16_t)e;
-          dup_seen |= hinsert(s, dk, t, below ? 1u : 0u);
-        }
-        s.dkey[t] = dk; s.label[t] = lb;
-        n_t = 32u * (k + 1u);
-        ended = stopmask != 0u;
-      }
-      if (!ended && b + MAXT < gEnd && lane == 0) s.run_bad[R] = 1;  // the run does not fit the window: the overflow kernel takes it
+      if (dec) dup_seen |= hinsert(s, dk, t, below ? 1u : 0u);
     }
     __syncwarp();  // hash, dkey, label, run tables complete
-    const uint32_t k0 = f_t >> 5, k1 = n_t >> 5;  // rounds that hold owned digis
+    if (R > RC) {  // too many runs: the ones beyond RC go to the overflow kernel
+#pragma unroll
+      for (uint32_t k = 0; k < 4; ++k) {
+        const uint32_t g = b + 32u * k + lane;
+        if ((sb[k] >> lane & 1u) && rb[k] + __popc(sb[k] & le_mask) > RC) {
+          uint32_t sg = c.chunk_seg[ci];
+          while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
+          push_overflow(c, ((sg / F) << 16) | c.d_module[g]);
+        }
+      }
+    } else if (!fits && lane == 0) {
+      s.run_bad[R] = 1;  // the last run does not fit the window: the overflow kernel takes it
+    }
+    __syncwarp();
+    const uint32_t k0 = kf, k1 = kl;  // rounds that hold owned digis
 
     // ================================================================== D: duplicates; neighbours -> edges -> unions
     if (__any_sync(FULL, dup_seen)) {  // rare: some pixel appears twice; the digi not in the slot is a DUPLICATE (S10)
@@ -593,23 +404,15 @@ __global__ void __launch_bounds__(FT, 8) fused_kernel(const __grid_constant__ Ch
 
 }  // namespace
 
-static inline int grid_for(uint32_t work_items, uint32_t per_block, int cap_blocks) {
-  uint64_t b = ((uint64_t)work_items + per_block - 1) / per_block;
-  if (b < 1) b = 1;
-  return (int)(b < (uint64_t)cap_blocks ? b : (uint64_t)cap_blocks);
+cudaError_t configure_findclus_kernel() {
+  return cudaFuncSetAttribute(findclus_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WPB * sizeof(WarpSmem)));
 }
 
-void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream) {
-  const uint32_t Ec = c.e1 - c.e0;
-  init_kernel<<<grid_for(Ec * c.M, 256, n_sm * 8), 256, 0, stream>>>(c, n_total);
-}
-
-cudaError_t configure_fused_kernel() {
-  return cudaFuncSetAttribute(fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WPB * sizeof(WarpSmem)));
-}
-
-void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
-  fused_kernel<<<grid_for(words_bound + 31u, WPB * HC, n_sm * 8), FT, WPB * sizeof(WarpSmem), stream>>>(c);
+void launch_findclus(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
+  uint64_t nb = ((uint64_t)words_bound + CHUNK_WORDS + WPB * HC - 1) / (WPB * HC);
+  if (nb < 1) nb = 1;
+  if (nb > (uint64_t)n_sm * 8) nb = (uint64_t)n_sm * 8;
+  findclus_kernel<<<(int)nb, FT, WPB * sizeof(WarpSmem), stream>>>(c);
 }
 
 }  // namespace pix

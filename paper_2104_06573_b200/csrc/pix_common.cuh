@@ -6,8 +6,9 @@
 //
 // Kernel chain for one chunk of events:
 //   init      -> segment table, range sentinels, zeroed counters
-//   fused     -> a1 decode + a2 calibrate + a3 run boundaries + a4 findClus + a5 sums/cut/renumber for every
-//                module run that fits a warp's 256-word window (home chunk of 128 words + look-ahead)
+//   decode    -> a1 decode + a2 calibrate + a3 run boundaries, streaming, 4 words per thread; one start bit per word
+//   findclus  -> a4 findClus + a5 sums/cut/renumber for every module run that fits a warp's 256-word window
+//                (home chunk of 128 words + look-ahead)
 //   overflow  -> a4 + a5 for the runs the fused kernel could not take (longer than the window, pathological
 //                charge sums): generic block-per-run kernel, tables in global workspace
 //   offsets   -> a6 clamp + prefix scan (Fig. 3), summary, scatter work list
@@ -29,6 +30,7 @@ enum : uint8_t { ST_OK = 0, ST_CUT = 1, ST_BELOW = 2, ST_DUP = 3, ST_EMPTY = 4, 
 
 constexpr uint32_t FLAG_NONCONTIGUOUS = 1u, FLAG_CAPACITY = 2u, FLAG_TOO_LARGE = 4u;
 constexpr uint32_t NO_INDEX = 0xFFFFFFFFu;
+constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus; chunk ci starts at (gBeg & ~127) + 128 ci
 
 // per-event counters (integer atomics only), one row of EC_STRIDE per event of the chunk
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
@@ -76,6 +78,8 @@ struct Chunk {
   uint32_t* ctl;            // [CTL_WORDS]
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
   uint32_t ovf_cap;
+  uint32_t* startbits;      // [cap_words/32 + 8] bit (g - T0): word g starts a module run (decode -> findclus)
+  uint32_t* chunk_seg;      // [cap_words/128 + 2] segment (event_rel*F + fed) of the chunk's first word
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
   // temp cluster records, indexed by chunk-relative word index (run first + local id)
@@ -91,13 +95,14 @@ __device__ __forceinline__ uint32_t ev_offset(const Chunk& c, uint32_t e) {
 
 // launchers (host), one per kernel; all asynchronous on `stream`
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream);
-void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
+void launch_decode(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
+void launch_findclus(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);
-cudaError_t configure_fused_kernel();
+cudaError_t configure_findclus_kernel();
 cudaError_t configure_finalize_kernel();
 cudaError_t configure_overflow_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 5;    // init, fused, overflow, offsets, scatter
+constexpr int LAUNCHES_PER_CHUNK = 6;    // init, decode, findclus, overflow, offsets, scatter
 
 }  // namespace pix
