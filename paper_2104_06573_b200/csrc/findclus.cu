@@ -32,21 +32,22 @@ constexpr int WPB = 4;                    // warps per block (they share nothing
 constexpr int FT = WPB * 32;
 constexpr uint32_t HC = 128;              // words of a home chunk (rounds 0-3)
 constexpr uint32_t MAXT = 256;            // window: home chunk + up to 4 extension rounds
-constexpr uint32_t WTAB = 512;            // hash slots per warp
+constexpr uint32_t WTAB = 1024;           // hash slots per warp: 256 buckets of 4
 constexpr uint32_t RC = 62;               // runs a warp can own
-constexpr uint32_t ECAP = 3 * MAXT;       // at most 3 forward edges per digi
+constexpr uint32_t ECAP = 256;            // edge list; flushed (united) when a round might not fit
 constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
 constexpr uint32_t HASH_MUL = 0x9E3779B1u;
-constexpr uint32_t KEY_BITS = 23, KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = 14, TAG_MASK = (1u << TAG_BITS) - 1u;
-static_assert(((RC + 1u) << 17) <= (1u << KEY_BITS) && (1u << (KEY_BITS - TAG_BITS)) == WTAB && MAXT <= 256,
-              "key: run (6 bits) | row (8) | col (9); slot: disp (9) | tag (14) | digi (8) | below (1)");
+constexpr uint32_t KEY_BITS = 23, KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = 15, TAG_MASK = (1u << TAG_BITS) - 1u;
+constexpr uint32_t NBUCKET = WTAB / 4, MAX_DISP = 3;
+static_assert(((RC + 1u) << 17) <= (1u << KEY_BITS) && (1u << (KEY_BITS - TAG_BITS)) == NBUCKET && MAXT <= 256,
+              "key: run (6 bits) | row (8) | col (9); slot: disp (2) | tag (15) | digi (8) | below (1)");
 
 // digi key inside the window: run (6 bits) | row (8 bits) | col (9 bits).  Neighbour keys are key+1 (col+1)
 // and key+512-1, +512, +512+1 (row+1): col 416..511 and row 160..255 never occur, so no bounds checks (S13).
 struct __align__(16) WarpSmem {
-  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D, tab + edge: qn = tab, sx = tab + 256, sy = tab + 512
+  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D: qn = tab, sx = tab + 256, sy = tab + 512, root list
   uint16_t edge[ECAP];     // a | b << 8
   uint32_t dkey[MAXT];     // key of the digi in window slot t (word b + t), INVALID if not owned / undecodable
   uint32_t label[MAXT];    // union-find parent, or MARK_*
@@ -57,38 +58,54 @@ struct __align__(16) WarpSmem {
   uint16_t run_base[RC + 2];    // survivors before the run
   uint8_t run_bad[RC + 2];      // the run is left to the overflow kernel
 };
-static_assert(WTAB * 4 + ECAP * 2 >= 3 * MAXT * 4 + MAXT, "the sums and the root list fit in tab + edge");
+static_assert(WTAB * 4 >= 3 * MAXT * 4 + MAXT, "the sums and the root list fit in tab");
 static_assert(sizeof(WarpSmem) % 16 == 0, "per-warp slices stay 16-byte aligned");
 
-// Position hash, open addressing, one word per slot.  h = key * HASH_MUL mod 2^23 is a bijection on the 23-bit
-// keys; home slot = top 9 bits of h, tag = the other 14, so (home, tag) names the key exactly.  A key stored
-// i slots after its home records the displacement: slot = disp (9) | tag (14) | digi (8) | below_threshold (1).
-// Slots are never emptied; equal keys meet in one slot and keep the lowest digi (S10).
+// Position hash: 256 buckets of 4 slots, one 128-bit shared load per lookup and no probing loop on the common
+// path.  h = key * HASH_MUL mod 2^23 is a bijection on the 23-bit keys; bucket = top 8 bits of h, tag = the
+// other 15, so (bucket, tag) names the key exactly.  A key whose home bucket is full goes to the next bucket(s)
+// and records the displacement: slot = 0 | disp (2) | tag (15) | digi (8) | below_threshold (1).  Slots of a
+// bucket fill in order and are never emptied; equal keys meet in one slot and keep the lowest digi (S10).
 __device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
 
-// returns true when the key was already there (a duplicate pixel, S10)
-__device__ __forceinline__ bool hinsert(WarpSmem& s, uint32_t key, uint32_t t, uint32_t below) {
-  const uint32_t h = hmix(key);
-  uint32_t p = h >> TAG_BITS, want = h & TAG_MASK;
+// 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets
+__device__ __forceinline__ uint32_t hinsert(WarpSmem& s, uint32_t key, uint32_t t, uint32_t below) {
+  const uint32_t h = hmix(key), tag = h & TAG_MASK;
+  uint32_t p = (h >> TAG_BITS) * 4u, res = 2u;
 #pragma unroll 1
-  while (true) {
-    const uint32_t mine = (want << 9) | (t << 1) | below;
+  for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u) && res == 2u; ++i, p = (p + 1u) & (WTAB - 1u)) {
+    const uint32_t want = ((i >> 2) << TAG_BITS) | tag, mine = (want << 9) | (t << 1) | below;
     const uint32_t old = atomicCAS(&s.tab[p], EMPTY, mine);
-    if (old == EMPTY) return false;
-    if ((old >> 9) == want) { atomicMin(&s.tab[p], mine); return true; }  // same pixel: the lowest digi owns it
-    p = (p + 1u) & (WTAB - 1u); want += 1u << TAG_BITS;  // at most 256 of the 512 slots are ever taken
+    if (old == EMPTY) res = 0u;
+    else if ((old >> 9) == want) { atomicMin(&s.tab[p], mine); res = 1u; }  // same pixel: the lowest digi owns it
   }
+  return res;
+}
+__device__ __forceinline__ uint32_t half_match(const uint4& e, uint32_t want) {
+  uint32_t r = EMPTY;
+  if ((e.w >> 9) == want) r = e.w;
+  if ((e.z >> 9) == want) r = e.z;
+  if ((e.y >> 9) == want) r = e.y;
+  if ((e.x >> 9) == want) r = e.x;
+  return r;
+}
+__device__ __noinline__ uint32_t hfind_slow(const WarpSmem& s, uint32_t h) {
+  const uint32_t tag = h & TAG_MASK;
+  uint32_t b = h >> TAG_BITS, r = EMPTY;
+  for (uint32_t i = 1; i <= MAX_DISP && r == EMPTY; ++i) {  // the buckets after the (full) home bucket
+    b = (b + 1u) & (NBUCKET - 1u);
+    const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[b * 4u]);
+    r = half_match(e, (i << TAG_BITS) | tag);
+    if (e.w == EMPTY) break;
+  }
+  return r;
 }
 // slot contents of the key whose mixed value is h, or EMPTY
 __device__ __forceinline__ uint32_t hfind(const WarpSmem& s, uint32_t h) {
-  uint32_t p = h >> TAG_BITS, want = h & TAG_MASK;
-  uint32_t e = s.tab[p];
-#pragma unroll 1
-  while (e != EMPTY && (e >> 9) != want) {
-    p = (p + 1u) & (WTAB - 1u); want += 1u << TAG_BITS;
-    e = s.tab[p];
-  }
-  return e;
+  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> TAG_BITS) * 4u]);
+  uint32_t r = half_match(e, h & TAG_MASK);
+  if (r == EMPTY && e.w != EMPTY) r = hfind_slow(s, h);  // home bucket full, no match (rare): displaced keys
+  return r;
 }
 __device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0xFFu; }
 __device__ __forceinline__ bool slot_live(uint32_t e) { return e != EMPTY && !(e & 1u); }
@@ -118,7 +135,7 @@ __device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
 }
 
 // (event, FED) of word g >= b, given the segment sg0 of the chunk's first word and the next boundary nextB0
-__global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__ Chunk c) {
+__global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   WarpSmem& s = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
@@ -136,11 +153,27 @@ __global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__
   uint8_t* const rlist = reinterpret_cast<uint8_t*>(w0 + 3 * MAXT);  // roots in digi order (after phase D)
   constexpr uint32_t NO_ID = 0xFFFFu;
 
-  for (uint32_t ci = blockIdx.x * WPB + warp; ci < n_chunks; ci += gridDim.x * WPB) {
+  const uint32_t stride = gridDim.x * WPB;
+  uint32_t ci = blockIdx.x * WPB + warp;
+  uint32_t sbv_n = 0u, sg_n = 0u;  // prefetched for the next chunk: start bits (lane k < 8: round k), segment
+  if (ci < n_chunks) {
+    if (lane < 8u && ci * 4u + lane < n_chunks * 4u) sbv_n = c.startbits[ci * 4u + lane];
+    sg_n = c.chunk_seg[ci];
+  }
+  for (; ci < n_chunks; ci += stride) {
     const uint32_t b = T0 + ci * HC;
     // ================================================================== A: start bits of the window; clear
-    uint32_t sbv = 0u;  // lane k < 8: start bits of round k
-    if (lane < 8u && ci * 4u + lane < n_chunks * 4u) sbv = c.startbits[ci * 4u + lane];
+    const uint32_t sbv = sbv_n, sg0 = sg_n;
+    const uint32_t nextB0 = segB[sg0 + 1u];  // segment of the chunk's first word: its end, its event, the event's base
+    const uint32_t er0 = sg0 / F, ebase0 = segB[er0 * F];
+    {
+      const uint32_t cn = ci + stride;
+      sbv_n = 0u;
+      if (cn < n_chunks) {
+        if (lane < 8u && cn * 4u + lane < n_chunks * 4u) sbv_n = c.startbits[cn * 4u + lane];
+        sg_n = c.chunk_seg[cn];
+      }
+    }
     const uint32_t home = __ballot_sync(FULL, lane < 4u && sbv != 0u);
     if (!home) continue;  // no run starts here: nothing owned
     {
@@ -179,27 +212,51 @@ __global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__
     bool dup_seen = false;
     const uint32_t kl = (e_t + 31u) >> 5;  // rounds kf .. kl-1 hold the window
 #pragma unroll
-    for (uint32_t k = 0; k < 8; ++k) {
-      if (k < kf || k >= kl) continue;  // warp-uniform
-      const uint32_t t = 32u * k + lane, g = b + t;
-      const uint32_t r = (k < 4u ? rb[k] : R) + __popc(sb[k] & le_mask & (k < 4u ? FULL : 0u));
-      const bool in = t >= f_t && t < e_t && r <= RC;
-      uint32_t row = 0xFFFFu, col = 0u;
-      int32_t e = 0;
-      if (in) { row = c.d_row[g]; col = c.d_col[g]; e = c.d_charge[g]; }
-      if (in && k < 4u && (sb[k] >> lane & 1u)) {  // the first digi of run r
-        uint32_t sg = c.chunk_seg[ci];
-        while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
-        const uint32_t er = sg / F;
-        s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | c.d_module[g]; s.run_ifirst[r] = g - segB[er * F];
+    for (uint32_t half = 0; half < 2; ++half) {
+      const uint32_t ks = 4u * half;
+      if (kl <= ks || kf >= ks + 4u) continue;  // warp-uniform
+      // all global loads of the four rounds first, then the staging: one exposed latency per half
+      uint32_t rw[4], cl[4], md[4];
+      int32_t ch[4];
+#pragma unroll
+      for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t k = ks + j, t = 32u * k + lane, g = b + t;
+        const bool in0 = k >= kf && k < kl && t >= f_t && t < e_t;
+        rw[j] = in0 ? (uint32_t)c.d_row[g] : 0xFFFFu;
+        cl[j] = in0 ? (uint32_t)c.d_col[g] : 0u;
+        ch[j] = in0 ? c.d_charge[g] : 0;
+        md[j] = (in0 && half == 0u && (sb[k] >> lane & 1u)) ? (uint32_t)c.d_module[g] : 0xFFFFFFFFu;
       }
-      const bool dec = in && row != 0xFFFFu;
-      const bool below = e < c.thr;  // S9
-      const uint32_t dk = dec ? ((r << 17) | (row << 9) | col) : INVALID;
-      s.dkey[t] = dk;
-      s.label[t] = (dec && !below) ? t : MARK_BELOW;
-      s.chg[t] = (uint16_t)e;
-      if (dec) dup_seen |= hinsert(s, dk, t, below ? 1u : 0u);
+#pragma unroll
+      for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t k = ks + j;
+        if (k < kf || k >= kl) continue;  // warp-uniform
+        const uint32_t t = 32u * k + lane, g = b + t;
+        const uint32_t r = (half == 0u ? rb[k] : R) + __popc(sb[k] & le_mask & (half == 0u ? FULL : 0u));
+        const bool in = t >= f_t && t < e_t && r <= RC;
+        const uint32_t row = rw[j], col = cl[j];
+        const int32_t e = ch[j];
+        if (in && md[j] != 0xFFFFFFFFu) {  // the first digi of run r
+          uint32_t er = er0, eb = ebase0;
+          if (g >= nextB0) {  // rare: a FED / event boundary inside the window
+            uint32_t sg = sg0 + 1u;
+            while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
+            er = sg / F; eb = segB[er * F];
+          }
+          s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | md[j]; s.run_ifirst[r] = g - eb;
+        }
+        const bool dec = in && row != 0xFFFFu;
+        const bool below = e < c.thr;  // S9
+        const uint32_t dk = dec ? ((r << 17) | (row << 9) | col) : INVALID;
+        s.dkey[t] = dk;
+        s.label[t] = (dec && !below) ? t : MARK_BELOW;
+        s.chg[t] = (uint16_t)e;
+        if (dec) {
+          const uint32_t ins = hinsert(s, dk, t, below ? 1u : 0u);
+          dup_seen |= ins == 1u;
+          if (ins == 2u) s.run_bad[r] = 1;  // no room near the home bucket: the overflow kernel takes the run
+        }
+      }
     }
     __syncwarp();  // hash, dkey, label, run tables complete
     if (R > RC) {  // too many runs: the ones beyond RC go to the overflow kernel
@@ -207,7 +264,7 @@ __global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__
       for (uint32_t k = 0; k < 4; ++k) {
         const uint32_t g = b + 32u * k + lane;
         if ((sb[k] >> lane & 1u) && rb[k] + __popc(sb[k] & le_mask) > RC) {
-          uint32_t sg = c.chunk_seg[ci];
+          uint32_t sg = sg0;
           while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
           push_overflow(c, ((sg / F) << 16) | c.d_module[g]);
         }
@@ -229,10 +286,22 @@ __global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__
     // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE are
     // joined to it by their own E edges, so d-S alone is enough.
     uint32_t ne = 0u;
+    bool flushed = false;  // the edge list was united early at least once (dense window)
 #pragma unroll 1
     for (uint32_t k = k0; k < k1; ++k) {
       const uint32_t t = 32u * k + lane, key = s.dkey[t];
-      const bool live = key != INVALID && s.label[t] == t;
+      if (ne + 96u > ECAP) {  // the round's edges might not fit: unite what is listed (warp-uniform)
+        __syncwarp();
+        for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
+          if (i0 + lane < ne) {
+            const uint32_t e = s.edge[i0 + lane];
+            uf_unite(s.label, e & 0xFFu, e >> 8);
+          }
+          __syncwarp();
+        }
+        ne = 0u; flushed = true;
+      }
+      const bool live = key != INVALID && s.label[t] < MAXT;
       bool f0 = false, f1 = false, f2 = false;
       uint32_t n0 = 0, n1 = 0, n2 = 0;
       if (live) {
@@ -253,6 +322,26 @@ __global__ void __launch_bounds__(FT, 8) findclus_kernel(const __grid_constant__
       ne += __popc(m2);
     }
     __syncwarp();
+    if (!flushed) {
+      // first pass: every digi is still its own root, so an edge is one atomicMin (larger index under smaller).  A
+      // digi with two smaller neighbours keeps only the smaller one; the full pass below re-unites the other.
+      for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
+        if (i0 + lane < ne) {
+          const uint32_t e = s.edge[i0 + lane], a = e & 0xFFu, bb = e >> 8;
+          atomicMin(&s.label[a > bb ? a : bb], a > bb ? bb : a);
+        }
+      }
+      __syncwarp();
+#pragma unroll 1
+      for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: chains of the first pass shrink 4x
+        for (uint32_t k = k0; k < k1; ++k) {
+          const uint32_t t = 32u * k + lane;
+          const uint32_t l = s.label[t];
+          if (l < MAXT) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
+        }
+        __syncwarp();
+      }
+    }
     for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
       if (i0 + lane < ne) {
         const uint32_t e = s.edge[i0 + lane];
@@ -411,7 +500,7 @@ cudaError_t configure_findclus_kernel() {
 void launch_findclus(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
   uint64_t nb = ((uint64_t)words_bound + CHUNK_WORDS + WPB * HC - 1) / (WPB * HC);
   if (nb < 1) nb = 1;
-  if (nb > (uint64_t)n_sm * 8) nb = (uint64_t)n_sm * 8;
+  if (nb > (uint64_t)n_sm * 7) nb = (uint64_t)n_sm * 7;
   findclus_kernel<<<(int)nb, FT, WPB * sizeof(WarpSmem), stream>>>(c);
 }
 
