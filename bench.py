@@ -74,9 +74,25 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
+def shard_seeds(n_events: int, rank: int):
+    """Event seeds of one rank: events are independent, so the path shards by events with no
+    data-path collective; rank r takes seeds r*1000 .. r*1000 + n_events - 1 (weak scaling)."""
+    return rank * 1000 + np.arange(n_events)
+
+
+def max_over_ranks(value: float, dist=None, device=None) -> float:
+    """The step time of the job is the slowest rank's (one scalar all_reduce(MAX), outside the timed region)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def generate(n_events: int, rank: int):
     det = pixgen.detector("full")
-    batch = pixgen.events(det, "pu50", rank * 1000 + np.arange(n_events), cap_words_per_event=1 << 17)
+    batch = pixgen.events(det, "pu50", shard_seeds(n_events, rank), cap_words_per_event=1 << 17)
     return det, batch
 
 
@@ -177,10 +193,7 @@ def run_ours(args):
     barrier()
     ms = ev0.elapsed_time(ev1) / args.steps
     launches = pix.pix_kernel_launches(h) - n0
-    if dist is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, dev)
 
     # ---- per-kernel device time (CUDA events between the kernels, on the launch stream), same steps again
     pix.pix_set_profiling(h, True)
@@ -243,10 +256,7 @@ def run_ours(args):
             hstep()  # synchronous: returns after the device->host copies have landed
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
-        if dist is not None:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dist, dev)
         h2d = W * 4 + (E + 1) * 4 + E * (F + 1) * 4
         d2h = W * 15 + E * kmax * 22 + E * (3 * M + 1 + 16) * 4
         e2e = {"value": E * world / dt, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

@@ -83,3 +83,40 @@ def test_clamp_and_capacity(gu, full):
     check(gu, full, b, params=dict(P, max_clusters_per_module=8))
     got, _ = check(gu, full, b, kmax=1000)
     assert all(int(g["summary"][15]) & 2 for g in got)
+
+
+def test_cfg2_full_size_sampled(gu, full):
+    """BASELINE.json configs[2] at full size, in the launch configuration bench.py times (1000 events, one
+    pix_process_batch call, library-default launch groups): 24 sampled events are compared element by element
+    with the oracle; every event must satisfy the counting identities of the summary."""
+    import torch
+    import paper_2104_06573_b200 as pix
+    E, kmax = 1000, 20480
+    b = pixgen.events(full, "pu50", np.arange(E), cap_words_per_event=1 << 17)
+    sizes = np.diff(b.event_offsets.astype(np.int64))
+    W, M, F = int(sizes.sum()), full.n_modules, full.n_feds
+    wmax = (int(sizes.max()) + 1023) // 1024 * 1024
+    h = pix.pix_create(full.cabling, F, M, full.gain, full.pedestal, pix.make_params(P, wmax, kmax, E, 0))
+    try:
+        words = torch.from_numpy(np.concatenate([b.words, np.zeros(16, np.uint32)]).view(np.int32)).cuda()
+        ev_off = torch.from_numpy(b.event_offsets.view(np.int32).copy()).cuda()
+        fed_off = torch.from_numpy(b.fed_offsets.view(np.int32).reshape(-1).copy()).cuda()
+        digis, cl = pix.alloc_outputs(W, E, M, kmax, "cuda", fill=0xCD)
+        pix.pix_process_batch(h, None, E, words, W, ev_off, fed_off, digis, cl)
+        got = gu.split_events(full, b, gu.to_numpy(digis), gu.to_numpy(cl), kmax)
+    finally:
+        torch.cuda.synchronize()
+        pix.pix_destroy(h)
+    for e, g in enumerate(got):
+        s = g["summary"].astype(np.int64)
+        assert s[0] == sizes[e] and s[1] == s[0] - s[2:7].sum()
+        assert s[1] == s[7] + s[8] + s[9] + s[10]                      # every decoded word has exactly one status
+        assert s[14] == s[13] == g["clus_module_start"][-1] and s[15] == 0
+        assert np.count_nonzero(g["clus"] >= 0) == s[9]
+        assert int(g["c_n_pix"].sum()) == s[9]                         # pixels of surviving clusters = OK digis
+    rng = np.random.default_rng(7)
+    for e in sorted(set([0, E - 1]) | set(rng.choice(E, 22, replace=False).tolist())):
+        o = gu.oracle_events(full, type(b)(b.words[int(b.event_offsets[e]):int(b.event_offsets[e + 1])],
+                                           np.array([0, sizes[e]], np.uint32), b.fed_offsets[e:e + 1], b.tally[e:e + 1]),
+                             P, kmax=kmax)[0]
+        gu.assert_event_equal(got[e], o, tag=f"cfg2 full size, event {e}")
