@@ -120,3 +120,16 @@ def test_cfg2_full_size_sampled(gu, full):
                                            np.array([0, sizes[e]], np.uint32), b.fed_offsets[e:e + 1], b.tally[e:e + 1]),
                              P, kmax=kmax)[0]
         gu.assert_event_equal(got[e], o, tag=f"cfg2 full size, event {e}")
+
+
+def test_deterministic_and_stream_independent(gu, full):
+    """Two runs of the same batch (default stream, then a side stream) are bit-identical (several
+    events in flight must give the same physics as one at a time)."""
+    import torch
+    b = pixgen.events(full, "pu50", np.arange(200, 216))
+    a1 = gu.run_batch(full, b, P)
+    st = torch.cuda.Stream()
+    a2 = gu.run_batch(full, b, P, stream=st, chunk_events=7)
+    for x, y in zip(a1, a2):
+        for k in x:
+            assert np.array_equal(x[k], y[k]), k
