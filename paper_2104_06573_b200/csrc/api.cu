@@ -71,6 +71,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.ev_cnt = (uint32_t*)take(Ec * pix::EC_STRIDE * 4);
   c.ctl = (uint32_t*)take(pix::CTL_WORDS * 4);
   c.ovf_list = (uint32_t*)take(Ec * M * 4);
+  c.mid_list = (uint32_t*)take(Ec * M * 4);
   c.ovf_cap = (uint32_t)(Ec * M);
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.startbits = (uint32_t*)take((W / 32 + 8) * 4);
@@ -120,7 +121,7 @@ void bind_outputs(pix::Chunk& c, const pix_digis* d, const pix_clusters* k) {
 }
 
 // the launch sequence of one chunk
-constexpr int PROF_EVENTS = 6;  // families: init, decode, findclus, overflow, finalize (offsets + scatter)
+constexpr int PROF_EVENTS = 7;  // families: init, decode, findclus, findrun, overflow, finalize (offsets + scatter)
 int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t words_bound, cudaStream_t s) {
   cudaEvent_t* ev = nullptr;
   if (h->profiling) {
@@ -139,10 +140,12 @@ int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t wor
   if (ev) cudaEventRecord(ev[2], s);
   pix::launch_findclus(c, words_bound, h->n_sm, s);
   if (ev) cudaEventRecord(ev[3], s);
-  pix::launch_overflow(c, h->n_sm, s);
+  pix::launch_findrun(c, h->n_sm, s);
   if (ev) cudaEventRecord(ev[4], s);
-  pix::launch_finalize(c, h->n_sm, s);
+  pix::launch_overflow(c, h->n_sm, s);
   if (ev) cudaEventRecord(ev[5], s);
+  pix::launch_finalize(c, h->n_sm, s);
+  if (ev) cudaEventRecord(ev[6], s);
   h->launches += pix::LAUNCHES_PER_CHUNK;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
@@ -170,6 +173,7 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   cudaError_t e = cudaGetDevice(&h->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
   if (e == cudaSuccess) e = pix::configure_findclus_kernel();
+  if (e == cudaSuccess) e = pix::configure_findrun_kernel();
   if (e == cudaSuccess) e = pix::configure_finalize_kernel();
   if (e == cudaSuccess) e = pix::configure_overflow_kernel();
   if (e != cudaSuccess) { delete h; cudaGetLastError(); return PIX_ERR_CUDA; }

@@ -24,8 +24,8 @@ namespace {
 constexpr uint32_t NOKEY = 0xFFFFFFFFu;
 
 __device__ __forceinline__ void push_overflow(const Chunk& c, uint32_t key) {
-  const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u);
-  if (i < c.ovf_cap) c.ovf_list[i] = (key >> 16) * c.M + (key & 0xFFFFu);
+  const uint32_t i = atomicAdd(c.ctl + CTL_MID_COUNT, 1u);  // the warp-per-run kernel (findrun.cu) is next
+  if (i < c.ovf_cap) c.mid_list[i] = (key >> 16) * c.M + (key & 0xFFFFu);
 }
 
 constexpr int WPB = 4;                    // warps per block (they share nothing but the block)

@@ -1,0 +1,329 @@
+// findrun.cu -- the warp-per-run cluster kernel: a4 findClus (S10, S13) and a5 sums / charge cut /
+// renumber / temp records (S9, S14, S18) for the module runs the chunk kernel (findclus.cu) could not take
+// because they do not fit its 256-word window ("clusters the pixels on each detector module").
+//
+// One warp per run of up to RMAX = 512 words, tables in 15 KB of per-warp shared memory, the same phases as
+// findclus.cu with a single run: stage + insert into the position hash (512 buckets of 4 slots), duplicates,
+// forward-neighbour lookups -> edge list (united whenever it fills) -> lock-free min-index union-find, sums by
+// shared atomics, dense root list, cut + renumber in digi order, temp records, final status / clus, counters.
+// Longer runs, runs whose hash bucket neighbourhood overflows and charge sums beyond 32 bits go on to the block
+// kernel (cluster.cu).  Nothing here is shared with oracle/.
+#include "pix_common.cuh"
+
+namespace pix {
+
+namespace {
+
+constexpr int RWPB = 2;                   // warps per block
+constexpr uint32_t RMAX = 512;            // words of a run
+constexpr uint32_t RTAB = 2048;           // hash slots: 512 buckets of 4
+constexpr uint32_t RECAP = 256;           // edge list entries
+constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
+constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;
+constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;
+constexpr uint32_t HASH_MUL = 0x9E3779B1u;
+constexpr uint32_t KEY_BITS = 17, KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = 8, TAG_MASK = (1u << TAG_BITS) - 1u;
+constexpr uint32_t NBUCKET = RTAB / 4, MAX_DISP = 3;
+static_assert((1u << (KEY_BITS - TAG_BITS)) == NBUCKET, "key: row (8) | col (9); slot: disp (2) | tag (8) | digi (9) | below (1)");
+
+struct __align__(16) RunSmem {
+  uint32_t tab[RTAB];     // position hash; after the lookups: q = tab, np = tab + 512, sx = tab + 1024, sy = tab + 1536
+  uint32_t dkey[RMAX];    // row << 9 | col, INVALID for an undecodable word
+  uint32_t label[RMAX];   // union-find parent, or MARK_*
+  uint32_t edge[RECAP];   // a | b << 16
+  uint16_t chg[RMAX];     // charge; after the sums: local id of a root, or NO_ID
+  uint16_t rlist[RMAX];   // roots in digi order
+};
+
+__device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
+// 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets
+__device__ __forceinline__ uint32_t hinsert(RunSmem& s, uint32_t key, uint32_t t, uint32_t below) {
+  const uint32_t h = hmix(key), tag = h & TAG_MASK;
+  uint32_t p = (h >> TAG_BITS) * 4u, res = 2u;
+#pragma unroll 1
+  for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u) && res == 2u; ++i, p = (p + 1u) & (RTAB - 1u)) {
+    const uint32_t want = ((i >> 2) << TAG_BITS) | tag, mine = (want << 10) | (t << 1) | below;
+    const uint32_t old = atomicCAS(&s.tab[p], EMPTY, mine);
+    if (old == EMPTY) res = 0u;
+    else if ((old >> 10) == want) { atomicMin(&s.tab[p], mine); res = 1u; }  // same pixel: the lowest digi owns it
+  }
+  return res;
+}
+__device__ __forceinline__ uint32_t half_match(const uint4& e, uint32_t want) {
+  uint32_t r = EMPTY;
+  if ((e.w >> 10) == want) r = e.w;
+  if ((e.z >> 10) == want) r = e.z;
+  if ((e.y >> 10) == want) r = e.y;
+  if ((e.x >> 10) == want) r = e.x;
+  return r;
+}
+__device__ __noinline__ uint32_t hfind_slow(const RunSmem& s, uint32_t h) {
+  const uint32_t tag = h & TAG_MASK;
+  uint32_t b = h >> TAG_BITS, r = EMPTY;
+  for (uint32_t i = 1; i <= MAX_DISP && r == EMPTY; ++i) {
+    b = (b + 1u) & (NBUCKET - 1u);
+    const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[b * 4u]);
+    r = half_match(e, (i << TAG_BITS) | tag);
+    if (e.w == EMPTY) break;
+  }
+  return r;
+}
+__device__ __forceinline__ uint32_t hfind(const RunSmem& s, uint32_t h) {
+  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> TAG_BITS) * 4u]);
+  uint32_t r = half_match(e, h & TAG_MASK);
+  if (r == EMPTY && e.w != EMPTY) r = hfind_slow(s, h);
+  return r;
+}
+__device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x1FFu; }
+__device__ __forceinline__ bool slot_live(uint32_t e) { return e != EMPTY && !(e & 1u); }
+
+__device__ __forceinline__ uint32_t uf_find(volatile uint32_t* L, uint32_t x) {
+  uint32_t p = L[x];
+  while (p != x) {
+    const uint32_t gp = L[p];
+    if (gp != p) L[x] = gp;  // path halving
+    x = p; p = gp;
+  }
+  return x;
+}
+__device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
+  bool done = false;  // single exit: the lanes of a warp reconverge after the loop
+  while (!done) {
+    a = uf_find(L, a); b = uf_find(L, b);
+    if (a == b) { done = true; }
+    else {
+      if (a < b) { const uint32_t t = a; a = b; b = t; }
+      const uint32_t old = atomicMin(L + a, b);
+      if (old == a) done = true;
+      else a = old;
+    }
+  }
+}
+__device__ __forceinline__ void unite_edges(RunSmem& s, uint32_t ne, uint32_t lane) {
+  for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count
+    if (i0 + lane < ne) {
+      const uint32_t e = s.edge[i0 + lane];
+      uf_unite(s.label, e & 0xFFFFu, e >> 16);
+    }
+    __syncwarp();
+  }
+}
+__device__ __forceinline__ void push_block(const Chunk& c, uint32_t task) {
+  const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u);
+  if (i < c.ovf_cap) c.ovf_list[i] = task;
+}
+
+__global__ void __launch_bounds__(RWPB * 32) findrun_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  RunSmem& s = reinterpret_cast<RunSmem*>(smem_raw)[warp];
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  constexpr uint32_t FULL = 0xFFFFFFFFu, NO_ID = 0xFFFFu;
+  uint32_t* const q = s.tab; uint32_t* const np = s.tab + RMAX; uint32_t* const sx = s.tab + 2 * RMAX;
+  uint32_t* const sy = s.tab + 3 * RMAX;
+  uint16_t* const lid = s.chg;
+  uint32_t count = c.ctl[CTL_MID_COUNT];
+  count = count < c.ovf_cap ? count : c.ovf_cap;
+  const uint32_t gBeg = c.segB[0];
+
+  while (true) {
+    uint32_t ti = 0u;
+    if (lane == 0) ti = atomicAdd(c.ctl + CTL_MID_TICKET, 1u);
+    ti = __shfl_sync(FULL, ti, 0);
+    if (ti >= count) break;
+    const uint32_t task = c.mid_list[ti];
+    const uint32_t er = task / c.M, m = task - er * c.M;
+    if (c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] & FLAG_NONCONTIGUOUS) continue;  // S11: not clustered
+    const size_t mo = (size_t)(c.e0 + er) * c.M + m;
+    const uint32_t first = c.module_first[mo], n = c.module_end[mo] - first;
+    if (n > RMAX) {  // too long for a warp: the block kernel takes it
+      if (lane == 0) push_block(c, task);
+      continue;
+    }
+    const uint32_t gb = c.segB[er * c.F] + first;  // global index of the run's digi 0
+    const uint32_t nk = (n + 31u) >> 5;
+    {
+      uint4* t4 = reinterpret_cast<uint4*>(s.tab);
+      const uint4 e4 = make_uint4(EMPTY, EMPTY, EMPTY, EMPTY);
+#pragma unroll
+      for (int k = 0; k < (int)(RTAB / 4 / 32); ++k) t4[lane + 32 * k] = e4;
+    }
+    __syncwarp();
+    // ---- stage + insert
+    bool dup_seen = false, full_seen = false;
+#pragma unroll 1
+    for (uint32_t k = 0; k < nk; ++k) {
+      const uint32_t t = 32u * k + lane;
+      const bool in = t < n;
+      const uint32_t row = in ? (uint32_t)c.d_row[gb + t] : 0xFFFFu, col = in ? (uint32_t)c.d_col[gb + t] : 0u;
+      const int32_t e = in ? c.d_charge[gb + t] : 0;
+      const bool dec = row != 0xFFFFu, below = e < c.thr;  // S9
+      const uint32_t dk = dec ? ((row << 9) | col) : INVALID;
+      s.dkey[t] = dk;
+      s.label[t] = (dec && !below) ? t : MARK_BELOW;
+      s.chg[t] = (uint16_t)e;
+      if (dec) {
+        const uint32_t ins = hinsert(s, dk, t, below ? 1u : 0u);
+        dup_seen |= ins == 1u; full_seen |= ins == 2u;
+      }
+    }
+    __syncwarp();
+    if (__any_sync(FULL, full_seen)) {  // no room near a home bucket (dense run): the block kernel takes it
+      if (lane == 0) push_block(c, task);
+      continue;
+    }
+    // ---- duplicates (S10): the digi that is not in the slot
+    if (__any_sync(FULL, dup_seen)) {
+      for (uint32_t k = 0; k < nk; ++k) {
+        const uint32_t t = 32u * k + lane, key = s.dkey[t];
+        if (key != INVALID && slot_digi(hfind(s, hmix(key))) != t) s.label[t] = MARK_DUP;
+      }
+      __syncwarp();
+    }
+    // ---- forward neighbours (S13) -> edges -> unions
+    uint32_t ne = 0u;
+    bool flushed = false;
+#pragma unroll 1
+    for (uint32_t k = 0; k < nk; ++k) {
+      const uint32_t t = 32u * k + lane, key = s.dkey[t];
+      if (ne + 96u > RECAP) {  // the round's edges might not fit: unite what is listed (warp-uniform)
+        __syncwarp();
+        unite_edges(s, ne, lane);
+        ne = 0u; flushed = true;
+      }
+      const bool live = key != INVALID && s.label[t] < RMAX;
+      bool f0 = false, f1 = false, f2 = false;
+      uint32_t n0 = 0, n1 = 0, n2 = 0;
+      if (live) {
+        const uint32_t h = hmix(key);
+        const uint32_t eE = hfind(s, (h + HASH_MUL) & KEY_MASK), eS = hfind(s, (h + 512u * HASH_MUL) & KEY_MASK);
+        const uint32_t eSW = hfind(s, (h + 511u * HASH_MUL) & KEY_MASK), eSE = hfind(s, (h + 513u * HASH_MUL) & KEY_MASK);
+        const bool hS = slot_live(eS);
+        f0 = slot_live(eE); n0 = slot_digi(eE);
+        f1 = hS || slot_live(eSW); n1 = slot_digi(hS ? eS : eSW);
+        f2 = !hS && slot_live(eSE); n2 = slot_digi(eSE);
+      }
+      const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
+      if (f0) s.edge[ne + __popc(m0 & lt_mask)] = t | (n0 << 16);
+      ne += __popc(m0);
+      if (f1) s.edge[ne + __popc(m1 & lt_mask)] = t | (n1 << 16);
+      ne += __popc(m1);
+      if (f2) s.edge[ne + __popc(m2 & lt_mask)] = t | (n2 << 16);
+      ne += __popc(m2);
+    }
+    __syncwarp();
+    if (!flushed) {  // first pass: every digi is still its own root, so an edge is one atomicMin; then two jumps
+      for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
+        if (i0 + lane < ne) {
+          const uint32_t e = s.edge[i0 + lane], a = e & 0xFFFFu, bb = e >> 16;
+          atomicMin(&s.label[a > bb ? a : bb], a > bb ? bb : a);
+        }
+      }
+      __syncwarp();
+#pragma unroll 1
+      for (int pass = 0; pass < 2; ++pass) {
+        for (uint32_t k = 0; k < nk; ++k) {
+          const uint32_t t = 32u * k + lane;
+          const uint32_t l = s.label[t];
+          if (l < RMAX) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
+        }
+        __syncwarp();
+      }
+    }
+    unite_edges(s, ne, lane);
+    __syncwarp();  // components complete; the hash is dead, its memory becomes q / np / sx / sy
+    // ---- sums; dense list of the roots
+    {
+      uint4* t4 = reinterpret_cast<uint4*>(s.tab);
+      const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+      for (int k = 0; k < (int)(RTAB / 4 / 32); ++k) t4[lane + 32 * k] = z4;
+    }
+    __syncwarp();
+    uint32_t nr = 0u;
+#pragma unroll 1
+    for (uint32_t k = 0; k < nk; ++k) {
+      const uint32_t t = 32u * k + lane;
+      volatile uint32_t* L = s.label;
+      uint32_t r = L[t];
+      const bool live = r < RMAX;  // else MARK_*
+      if (live) {
+        while (true) { const uint32_t nx = L[r]; if (nx == r) break; r = nx; }
+        L[t] = r;
+        const uint32_t key = s.dkey[t], e = s.chg[t];
+        atomicAdd(&q[r], e); atomicAdd(&np[r], 1u);
+        atomicAdd(&sx[r], e * (key & 511u));
+        atomicAdd(&sy[r], e * (key >> 9));
+      }
+      const bool root = live && r == t;
+      const uint32_t rm = __ballot_sync(FULL, root);
+      if (root) s.rlist[nr + __popc(rm & lt_mask)] = (uint16_t)t;  // digi order
+      nr += __popc(rm);
+    }
+    __syncwarp();
+    // ---- cut, renumber (S14: local id = rank among the surviving roots, in digi order), temp records (S18)
+    uint32_t cnt = 0u;
+    bool wrapped = false;
+#pragma unroll 1
+    for (uint32_t i0 = 0u; i0 < nr; i0 += 32u) {
+      const bool valid = i0 + lane < nr;
+      uint32_t t = 0u, Q = 0u;
+      if (valid) { t = s.rlist[i0 + lane]; Q = q[t]; wrapped |= Q > Q_SAFE; }
+      const bool surv = valid && (long long)Q >= (long long)c.cut;  // S9: equality keeps
+      const uint32_t sm = __ballot_sync(FULL, surv);
+      const uint32_t id = cnt + __popc(sm & lt_mask);
+      if (valid) {
+        if (surv) {
+          const float fq = (float)Q;
+          put_temp(c.t_rec + ((gb - gBeg) + id), first + t, np[t], Q, __fdividef((float)sx[t], fq), __fdividef((float)sy[t], fq));
+        }
+        lid[t] = surv ? (uint16_t)id : (uint16_t)NO_ID;
+      }
+      cnt += __popc(sm);
+    }
+    __syncwarp();
+    if (__any_sync(FULL, wrapped)) {  // 32-bit weighted sums may have wrapped: the block kernel redoes the run
+      if (lane == 0) push_block(c, task);
+      continue;
+    }
+    // ---- final status and clus, counters
+    uint32_t cntA = 0u, cntB = 0u;  // dup | below << 16 ; ok | cut << 16
+#pragma unroll 1
+    for (uint32_t k = 0; k < nk; ++k) {
+      const uint32_t t = 32u * k + lane, key = s.dkey[t];
+      if (key == INVALID) continue;
+      const uint32_t lab = s.label[t];
+      uint32_t so; int32_t cl = -1;
+      if (lab == MARK_DUP) { so = ST_DUP; cntA += 1u; }
+      else if (lab == MARK_BELOW) { so = ST_BELOW; cntA += 0x10000u; }
+      else {
+        const uint32_t id = lid[lab];
+        if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
+      }
+      c.d_status[gb + t] = (uint8_t)so; c.d_clus[gb + t] = cl;
+    }
+    const uint32_t a = __reduce_add_sync(FULL, cntA), bb = __reduce_add_sync(FULL, cntB);
+    if (lane == 0) {
+      c.n_clus[task] = cnt;
+      uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
+      if (a & 0xFFFFu) atomicAdd(ec + EC_DUP, a & 0xFFFFu);
+      if (a >> 16) atomicAdd(ec + EC_BELOW, a >> 16);
+      if (bb & 0xFFFFu) atomicAdd(ec + EC_OK, bb & 0xFFFFu);
+      if (bb >> 16) atomicAdd(ec + EC_CUT, bb >> 16);
+      if (nr) atomicAdd(ec + EC_PRECUT, nr);
+    }
+    __syncwarp();  // shared state is rewritten by the next run
+  }
+}
+
+}  // namespace
+
+cudaError_t configure_findrun_kernel() {
+  return cudaFuncSetAttribute(findrun_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RWPB * sizeof(RunSmem)));
+}
+
+void launch_findrun(const Chunk& c, int n_sm, cudaStream_t stream) {
+  findrun_kernel<<<n_sm * 7, RWPB * 32, RWPB * sizeof(RunSmem), stream>>>(c);
+}
+
+}  // namespace pix
