@@ -214,6 +214,8 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
 
   pix::Chunk& c = h->proto;
   c.F = F; c.M = M; c.cab = t->cab; c.gp = t->gp;
+  c.F_shift = 0xFFFFFFFFu;
+  for (uint32_t sh = 0; sh < 17; ++sh) if ((1u << sh) == F) c.F_shift = sh;
   c.vcal_gain = params->vcal_gain; c.vcal_offset = params->vcal_offset; c.max_e_f = (float)params->max_electrons;
   c.thr = params->pixel_threshold_e; c.cut = params->cluster_charge_cut_e;
   c.cap_mod = params->max_clusters_per_module; c.cap_ev = params->max_clusters_per_event; c.cap_words = h->cap_words;

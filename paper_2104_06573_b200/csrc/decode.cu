@@ -124,6 +124,9 @@ __device__ __forceinline__ void run_end(const Chunk& c, uint32_t key, uint32_t g
   const uint32_t er = key >> 16, m = key & 0xFFFFu;
   atomicMax(c.module_end + ((size_t)(c.e0 + er) * c.M + m), g - c.segB[er * c.F] + 1u);
 }
+// sg / F (F is a power of two in both detector configurations: a shift)
+__device__ __forceinline__ uint32_t div_F(const Chunk& c, uint32_t sg) { return c.F_shift != 0xFFFFFFFFu ? sg >> c.F_shift : sg / c.F; }
+
 // ------------------------------------------------------------------ the streaming decode kernel
 constexpr int DT = 256;
 
@@ -155,16 +158,26 @@ __global__ void __launch_bounds__(DT) decode_kernel(const __grid_constant__ Chun
     const uint32_t sg0 = warp_find_segment(segB, S, gw, lane);
     if (lane == 0) c.chunk_seg[ci] = sg0;
     uint32_t ckey = NOKEY, cg = 0u;
-    {
+    if (gw > gBeg) {
+      // common case, warp-uniform: the word just before the chunk is decodable
       uint32_t g = gw;  // words [gBeg, g) are still to be searched, backwards
-      while (g > gBeg) {
+      {
+        const uint32_t gi = gw - 1u;
+        uint32_t sg = sg0;
+        while (segB[sg] > gi) --sg;  // segB[0] = gBeg <= gi
+        const uint32_t er = div_F(c, sg), fed = sg - er * F;
+        uint32_t m, r, cc;
+        if (decode_word(c.cab, __ldg(c.words + gi), fed << 11, m, r, cc) == ST_OK) { ckey = (er << 16) | m; cg = gi; g = gBeg; }
+        else g = gi;
+      }
+      while (g > gBeg) {  // rare: undecodable words before the chunk, 32 at a time
         const bool in = lane < g - gBeg;
         const uint32_t gi = g - 1u - lane;
         uint32_t key = NOKEY;
         if (in) {
           uint32_t sg = sg0;
-          while (segB[sg] > gi) --sg;  // segB[0] = gBeg <= gi
-          const uint32_t er = sg / F, fed = sg - er * F;
+          while (segB[sg] > gi) --sg;
+          const uint32_t er = div_F(c, sg), fed = sg - er * F;
           uint32_t m, r, cc;
           if (decode_word(c.cab, __ldg(c.words + gi), fed << 11, m, r, cc) == ST_OK) key = (er << 16) | m;
         }
@@ -190,7 +203,7 @@ __global__ void __launch_bounds__(DT) decode_kernel(const __grid_constant__ Chun
         const uint32_t gf = g0 < gBeg ? gBeg : g0;
         while (sg + 1u < S && segB[sg + 1u] <= gf) ++sg;
       }
-      uint32_t er = sg / F, fed = sg - er * F;
+      uint32_t er = div_F(c, sg), fed = sg - er * F;
       uint32_t nextB = segB[sg + 1u];
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -200,7 +213,7 @@ __global__ void __launch_bounds__(DT) decode_kernel(const __grid_constant__ Chun
         inmask |= 1u << j;
         if (g >= nextB) {  // rare: the thread's words straddle a FED / event boundary
           while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
-          er = sg / F; fed = sg - er * F; nextB = segB[sg + 1u];
+          er = div_F(c, sg); fed = sg - er * F; nextB = segB[sg + 1u];
         }
         uint32_t m, r, cc;
         st[j] = decode_word(c.cab, w[j], fed << 11, m, r, cc);
@@ -244,15 +257,32 @@ __global__ void __launch_bounds__(DT) decode_kernel(const __grid_constant__ Chun
     uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = __shfl_sync(FULL, tg, src);
     if (!below_l) { pkey = ckey; pg = cg; }
     uint32_t startmask = 0u;
+    uint32_t s_key = NOKEY, s_g = 0u, s_pkey = NOKEY, s_pg = 0u;  // the lane's first run start and its predecessor
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       if (key[j] == NOKEY) continue;
       if (key[j] != pkey) {
+        if (!startmask) { s_key = key[j]; s_g = g0 + j; s_pkey = pkey; s_pg = pg; }
         startmask |= 1u << j;
-        run_start(c, key[j], g0 + j);
-        if (pkey != NOKEY) run_end(c, pkey, pg);
       }
       pkey = key[j]; pg = g0 + j;
+    }
+    if (s_key != NOKEY) {  // one copy of the atomics for the usual case of at most one start per lane
+      run_start(c, s_key, s_g);
+      if (s_pkey != NOKEY) run_end(c, s_pkey, s_pg);
+    }
+    if (startmask & (startmask - 1u)) {  // rare: several runs start inside the lane's four words
+      uint32_t pk = NOKEY, pgg = 0u;
+      bool first = true;
+#pragma unroll 1
+      for (int j = 0; j < 4; ++j) {
+        if (key[j] == NOKEY) continue;
+        if (startmask >> j & 1u) {
+          if (!first) { run_start(c, key[j], g0 + j); run_end(c, pk, pgg); }
+          first = false;
+        }
+        pk = key[j]; pgg = g0 + j;
+      }
     }
     if (ci == n_chunks - 1u) {  // the chunk's last run ends at the last decodable word
       const int top = has ? 31 - __clz(has) : 0;

@@ -60,6 +60,7 @@ struct Chunk {
   uint32_t n_single;
   uint32_t e0, e1;          // event range of this chunk
   uint32_t F, M;
+  uint32_t F_shift;         // log2(F) when F is a power of two, else 0xFFFFFFFF
   // ---- tables (device, owned by the handle)
   const CabEntry* cab;      // [F*64*32]
   const float2* gp;         // [M*416] (gain, pedestal) interleaved
