@@ -3,7 +3,8 @@
 // pixels, and clusters the pixels on each detector module").
 //
 // One warp per 128 consecutive words, 4 per lane (one 128-bit load, 128-bit / 64-bit stores).  The warp
-//   - finds the (event, FED) segment of its words and looks back for the last decodable word before them
+//   - reads the (event, FED) segment of its first word (segfill_kernel) and looks back for the last decodable
+//     word before the chunk
 //   - decodes + calibrates, stores module / row / col / charge, and finishes the undecodable words
 //     (status, clus = -1, per-event error counters)
 //   - finds run starts (a decodable word whose (event, module) differs from the previous decodable word's)
@@ -95,23 +96,6 @@ __device__ __forceinline__ int32_t calibrate(const Chunk& c, uint32_t adc, float
   return __float2int_rz(fminf(f4, c.max_e_f));
 }
 
-// last s in [0, S) with segB[s] <= g, given segB[0] <= g < segB[S]; warp-cooperative 32-ary search
-__device__ __forceinline__ uint32_t warp_find_segment(const uint32_t* __restrict__ segB, uint32_t S, uint32_t g,
-                                                      uint32_t lane) {
-  uint32_t lo = 0, hi = S;  // invariant: segB[lo] <= g < segB[hi]
-  while (hi - lo > 1) {
-    const uint32_t step = (hi - lo + 31u) / 32u;
-    const uint32_t p = lo + (lane + 1u) * step;
-    const bool le = (p < hi) && (segB[p] <= g);
-    const uint32_t cnt = __popc(__ballot_sync(0xFFFFFFFFu, le));
-    const uint32_t nlo = lo + cnt * step;
-    const uint32_t nhi = nlo + step;
-    lo = nlo;
-    hi = nhi < hi ? nhi : hi;
-  }
-  return lo;
-}
-
 // a3: module_first / module_end are keyed by module id (S12); a second run of a module flags the event (S11)
 __device__ __forceinline__ uint32_t run_start(const Chunk& c, uint32_t key, uint32_t g) {
   const uint32_t er = key >> 16, m = key & 0xFFFFu;
@@ -124,6 +108,22 @@ __device__ __forceinline__ void run_end(const Chunk& c, uint32_t key, uint32_t g
   const uint32_t er = key >> 16, m = key & 0xFFFFu;
   atomicMax(c.module_end + ((size_t)(c.e0 + er) * c.M + m), g - c.segB[er * c.F] + 1u);
 }
+// chunk_seg[ci] = segment (event, FED) of the first word of 128-word chunk ci (its first word inside the launch
+// group).  One thread per segment writes the chunks that start inside it.
+__global__ void __launch_bounds__(256) segfill_kernel(const __grid_constant__ Chunk c) {
+  const uint32_t S = (c.e1 - c.e0) * c.F;
+  const uint32_t gBeg = c.segB[0], gEnd = c.segB[S];
+  if (gBeg >= gEnd) return;
+  const uint32_t T0 = gBeg & ~(CHUNK_WORDS - 1u);
+  for (uint32_t sgi = blockIdx.x * blockDim.x + threadIdx.x; sgi < S; sgi += gridDim.x * blockDim.x) {
+    const uint32_t lo = c.segB[sgi], hi = c.segB[sgi + 1u];
+    if (lo >= hi) continue;
+    const uint32_t c_lo = lo == gBeg ? 0u : (lo - T0 + CHUNK_WORDS - 1u) / CHUNK_WORDS;
+    const uint32_t c_hi = (hi - T0 + CHUNK_WORDS - 1u) / CHUNK_WORDS;  // exclusive
+    for (uint32_t ci = c_lo; ci < c_hi; ++ci) c.chunk_seg[ci] = sgi;
+  }
+}
+
 // sg / F (F is a power of two in both detector configurations: a shift)
 __device__ __forceinline__ uint32_t div_F(const Chunk& c, uint32_t sg) { return c.F_shift != 0xFFFFFFFFu ? sg >> c.F_shift : sg / c.F; }
 
@@ -155,8 +155,9 @@ __global__ void __launch_bounds__(DT) decode_kernel(const __grid_constant__ Chun
     }
     // ---- segment (event, FED) of the chunk's first word; look-back for the last decodable word before it
     const uint32_t gw = b < gBeg ? gBeg : b;  // b < gEnd by the chunk count
-    const uint32_t sg0 = warp_find_segment(segB, S, gw, lane);
-    if (lane == 0) c.chunk_seg[ci] = sg0;
+    const uint32_t sg0 = c.chunk_seg[ci];  // filled by segfill_kernel
+    const uint32_t nextB0 = segB[sg0 + 1u];
+    const bool allfull = __all_sync(FULL, full);
     uint32_t ckey = NOKEY, cg = 0u;
     if (gw > gBeg) {
       // common case, warp-uniform: the word just before the chunk is decodable
@@ -198,18 +199,18 @@ __global__ void __launch_bounds__(DT) decode_kernel(const __grid_constant__ Chun
       uint32_t mod[4], row[4], col[4];
       int32_t chg[4];
       uint32_t inmask = 0u;
-      uint32_t sg = sg0;
-      if (any) {
+      uint32_t sg = sg0, nextB = nextB0;
+      if (b + CHUNK_WORDS > nextB0 && any) {  // warp-uniform test; rare: a FED / event boundary inside the chunk
         const uint32_t gf = g0 < gBeg ? gBeg : g0;
         while (sg + 1u < S && segB[sg + 1u] <= gf) ++sg;
+        nextB = segB[sg + 1u];
       }
       uint32_t er = div_F(c, sg), fed = sg - er * F;
-      uint32_t nextB = segB[sg + 1u];
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const uint32_t g = g0 + j;
         st[j] = 0xFFu; key[j] = NOKEY; mod[j] = row[j] = col[j] = 0xFFFFu; chg[j] = 0;
-        if (!any || g < gBeg || g >= gEnd) continue;
+        if (!allfull && (!any || g < gBeg || g >= gEnd)) continue;
         inmask |= 1u << j;
         if (g >= nextB) {  // rare: the thread's words straddle a FED / event boundary
           while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
@@ -308,6 +309,7 @@ static inline int grid_for(uint32_t work_items, uint32_t per_block, int cap_bloc
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream) {
   const uint32_t Ec = c.e1 - c.e0;
   init_kernel<<<grid_for(Ec * c.M, 256, n_sm * 8), 256, 0, stream>>>(c, n_total);
+  segfill_kernel<<<grid_for(Ec * c.F, 256, n_sm * 8), 256, 0, stream>>>(c);
 }
 
 void launch_decode(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {

@@ -5,7 +5,7 @@
 // (lines 76-81).  Readings S1..S24 of DESIGN.md fix what the paper leaves open.
 //
 // Kernel chain for one chunk of events:
-//   init      -> segment table, range sentinels, zeroed counters
+//   init      -> segment table, range sentinels, zeroed counters; segfill -> segment of every 128-word chunk
 //   decode    -> a1 decode + a2 calibrate + a3 run boundaries, streaming, 4 words per thread; one start bit per word
 //   findclus  -> a4 findClus + a5 sums/cut/renumber for every module run that fits a warp's 256-word window
 //                (home chunk of 128 words + look-ahead)
@@ -108,6 +108,6 @@ cudaError_t configure_findrun_kernel();
 cudaError_t configure_finalize_kernel();
 cudaError_t configure_overflow_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 7;    // init, decode, findclus, findrun, overflow, offsets, scatter
+constexpr int LAUNCHES_PER_CHUNK = 8;    // init, segfill, decode, findclus, findrun, overflow, offsets, scatter
 
 }  // namespace pix
