@@ -10,7 +10,9 @@
  *  - pix_create/pix_clone/pix_destroy take HOST pointers.  pix_process and pix_process_batch take
  *    DEVICE pointers only (caller-owned, e.g. torch tensors) and a CUDA stream; they never
  *    allocate, free, synchronise or copy to the host, so they are legal during stream capture.
- *    pix_process_batch_host takes HOST pointers and does the copies itself (synchronous).
+ *    pix_process_batch_host takes HOST pointers and does the copies itself (synchronous; internally the
+ *    input copy, the kernels and the output copy of consecutive groups of events overlap on three streams;
+ *    pass pinned host memory for the overlap to take effect).
  *  - The library owns device copies of the two tables and a workspace, all allocated in
  *    pix_create / pix_clone (a memory pool gave 4.5x; here nothing allocates per event).
  *  - One in-flight call per handle; use pix_clone to get one handle per stream.
@@ -151,7 +153,7 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
 uint64_t pix_kernel_launches(const pix_handle* h);
 
 /* Diagnostic: module runs the LAST internal chunk of the last call left to the overflow kernel (runs longer than the
- * fused kernel's window, pathological charge sums).  Synchronises the device; not for the hot path. */
+ * warp kernels' windows, pathological charge sums).  Synchronises the device; not for the hot path. */
 int pix_overflow_runs(pix_handle* h, uint32_t* out);
 
 /* Optional per-kernel timing for benchmarks (not legal during stream capture).  While enabled, every chunk

@@ -27,6 +27,8 @@ struct HostStage {  // device staging of pix_process_batch_host, allocated on fi
   float *c_x = nullptr, *c_y = nullptr;
   uint32_t *module_first = nullptr, *module_end = nullptr, *clus_module_start = nullptr, *summary = nullptr;
   std::vector<void*> allocs;
+  cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of the pipelined host path
+  std::vector<cudaEvent_t> ev;                   // two per launch group: input landed, group computed
 };
 
 }  // namespace
@@ -241,6 +243,9 @@ int pix_destroy(pix_handle* h) {
   if (!h) return PIX_ERR_INVALID_ARG;
   cudaFree(h->ws);
   for (void* p : h->hs.allocs) cudaFree(p);
+  for (cudaEvent_t x : h->hs.ev) cudaEventDestroy(x);
+  if (h->hs.s_in) cudaStreamDestroy(h->hs.s_in);
+  if (h->hs.s_out) cudaStreamDestroy(h->hs.s_out);
   for (cudaEvent_t x : h->prof_events) cudaEventDestroy(x);
   release_tables(h->tables);
   delete h;
@@ -298,6 +303,10 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
   if (h->F > 1 && !fed_offsets) return fail(h, PIX_ERR_INVALID_ARG, "fed_offsets is NULL but n_feds > 1");
   if (n_events > h->p.max_events_per_batch) return fail(h, PIX_ERR_CAPACITY, "n_events > max_events_per_batch");
   if ((uint64_t)n_words_total > h->cap_total) return fail(h, PIX_ERR_CAPACITY, "n_words_total > capacity");
+  if (!od->module || !od->row || !od->col || !od->charge || !od->clus || !od->status || !oc->module || !oc->first_digi ||
+      !oc->n_pix || !oc->charge || !oc->x_col || !oc->y_row || !oc->module_first || !oc->module_end ||
+      !oc->clus_module_start || !oc->summary)
+    return fail(h, PIX_ERR_INVALID_ARG, "an output array is NULL");
   HostStage& s = h->hs;
   const size_t E = h->p.max_events_per_batch, W = (size_t)h->cap_total, M = h->M, F = h->F, K = h->p.max_clusters_per_event;
   if (!s.ready) {
@@ -319,23 +328,71 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
     if (!ok) { for (void* p : s.allocs) cudaFree(p); s.allocs.clear(); return fail(h, PIX_ERR_ALLOC, "staging allocation failed"); }
     s.ready = true;
   }
+  // Pipeline over launch groups of events (the transfer is part of the module):
+  // group g's input copy (stream s_in), its kernels (the caller's stream) and its output copy (stream s_out) overlap
+  // with the neighbouring groups'.  The workspace is shared, so the kernels of the groups run in stream order.
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const size_t n = n_words_total, Ev = n_events;
+  if (!s.s_in) {
+    if (cudaStreamCreateWithFlags(&s.s_in, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&s.s_out, cudaStreamNonBlocking) != cudaSuccess) {
+      cudaGetLastError(); s.s_in = s.s_out = nullptr;
+      return fail(h, PIX_ERR_ALLOC, "stream creation failed");
+    }
+  }
+  uint32_t ge = (n_events + 7u) / 8u;  // about eight groups per call
+  if (ge < 1u) ge = 1u;
+  if (ge > h->chunk_events) ge = h->chunk_events;
+  const uint32_t n_groups = (n_events + ge - 1u) / ge;
+  while (s.ev.size() < 2 * (size_t)n_groups + 1) {
+    cudaEvent_t x;
+    if (cudaEventCreateWithFlags(&x, cudaEventDisableTiming) != cudaSuccess) return fail(h, PIX_ERR_ALLOC, "cudaEventCreate");
+    s.ev.push_back(x);
+  }
+  const size_t Ev = n_events;
   cudaError_t e = cudaSuccess;
-  auto h2d = [&](void* d, const void* src, size_t bytes) { if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st); };
-  auto d2h = [&](void* dst, const void* d, size_t bytes) { if (e == cudaSuccess && dst && bytes) e = cudaMemcpyAsync(dst, d, bytes, cudaMemcpyDeviceToHost, st); };
-  h2d(s.words, raw_words, n * 4); h2d(s.ev_off, event_word_offsets, (Ev + 1) * 4);
+  auto h2d = [&](void* d, const void* src, size_t bytes) { if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, s.s_in); };
+  auto d2h = [&](void* dst, const void* d, size_t bytes) { if (e == cudaSuccess && dst && bytes) e = cudaMemcpyAsync(dst, d, bytes, cudaMemcpyDeviceToHost, s.s_out); };
+  // the copy streams start after whatever the caller's stream holds so far
+  if (e == cudaSuccess) e = cudaEventRecord(s.ev[2 * n_groups], st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s.s_in, s.ev[2 * n_groups], 0);
+  h2d(s.ev_off, event_word_offsets, (Ev + 1) * 4);
   if (F > 1) h2d(s.fed_off, fed_offsets, Ev * (F + 1) * 4);
   if (e != cudaSuccess) return fail_cuda(h, e, "host->device copy");
   pix_digis dd{s.d_module, s.d_row, s.d_col, s.d_charge, s.d_clus, s.d_status};
   pix_clusters dc{s.c_module, s.c_first, s.c_npix, s.c_charge, s.c_x, s.c_y, s.module_first, s.module_end, s.clus_module_start, s.summary};
-  if (int rc = pix_process_batch(h, cuda_stream, n_events, s.words, n_words_total, s.ev_off, F > 1 ? s.fed_off : nullptr, &dd, &dc)) return rc;
-  d2h(od->module, s.d_module, n * 2); d2h(od->row, s.d_row, n * 2); d2h(od->col, s.d_col, n * 2);
-  d2h(od->charge, s.d_charge, n * 4); d2h(od->clus, s.d_clus, n * 4); d2h(od->status, s.d_status, n);
-  d2h(oc->module, s.c_module, Ev * K * 2); d2h(oc->first_digi, s.c_first, Ev * K * 4); d2h(oc->n_pix, s.c_npix, Ev * K * 4);
-  d2h(oc->charge, s.c_charge, Ev * K * 4); d2h(oc->x_col, s.c_x, Ev * K * 4); d2h(oc->y_row, s.c_y, Ev * K * 4);
-  d2h(oc->module_first, s.module_first, Ev * M * 4); d2h(oc->module_end, s.module_end, Ev * M * 4);
-  d2h(oc->clus_module_start, s.clus_module_start, Ev * (M + 1) * 4); d2h(oc->summary, s.summary, Ev * 16 * 4);
+  pix::Chunk c = h->proto;
+  c.words = s.words; c.ev_off = s.ev_off; c.fed_off = F > 1 ? s.fed_off : nullptr; c.n_single = 0;
+  bind_outputs(c, &dd, &dc);
+  for (uint32_t g = 0; g < n_groups; ++g) {
+    const uint32_t e0 = g * ge, e1 = (n_events - e0 > ge) ? e0 + ge : n_events;
+    // host-side view of the group's word range, clamped like the device does
+    size_t w0 = event_word_offsets[e0], w1 = event_word_offsets[e1];
+    if (w1 > n_words_total) w1 = n_words_total;
+    if (w0 > w1) w0 = w1;
+    h2d(s.words + w0, raw_words + w0, (w1 - w0) * 4);
+    if (e == cudaSuccess) e = cudaEventRecord(s.ev[2 * g], s.s_in);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s.ev[2 * g], 0);
+    if (e != cudaSuccess) return fail_cuda(h, e, "host->device copy");
+    c.e0 = e0; c.e1 = e1;
+    size_t bound = w1 - w0;
+    if (bound > h->cap_words) bound = h->cap_words;
+    if (int rc = run_chunk(h, c, n_words_total, (uint32_t)bound, st)) return rc;
+    if (e == cudaSuccess) e = cudaEventRecord(s.ev[2 * g + 1], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s.s_out, s.ev[2 * g + 1], 0);
+    const size_t nw = w1 - w0, ne = e1 - e0;
+    d2h(od->module + w0, s.d_module + w0, nw * 2); d2h(od->row + w0, s.d_row + w0, nw * 2); d2h(od->col + w0, s.d_col + w0, nw * 2);
+    d2h(od->charge + w0, s.d_charge + w0, nw * 4); d2h(od->clus + w0, s.d_clus + w0, nw * 4); d2h(od->status + w0, s.d_status + w0, nw);
+    const size_t k0 = (size_t)e0 * K;
+    d2h(oc->module + k0, s.c_module + k0, ne * K * 2); d2h(oc->first_digi + k0, s.c_first + k0, ne * K * 4);
+    d2h(oc->n_pix + k0, s.c_npix + k0, ne * K * 4); d2h(oc->charge + k0, s.c_charge + k0, ne * K * 4);
+    d2h(oc->x_col + k0, s.c_x + k0, ne * K * 4); d2h(oc->y_row + k0, s.c_y + k0, ne * K * 4);
+    d2h(oc->module_first + (size_t)e0 * M, s.module_first + (size_t)e0 * M, ne * M * 4);
+    d2h(oc->module_end + (size_t)e0 * M, s.module_end + (size_t)e0 * M, ne * M * 4);
+    d2h(oc->clus_module_start + (size_t)e0 * (M + 1), s.clus_module_start + (size_t)e0 * (M + 1), ne * (M + 1) * 4);
+    d2h(oc->summary + (size_t)e0 * 16, s.summary + (size_t)e0 * 16, ne * 16 * 4);
+    if (e != cudaSuccess) return fail_cuda(h, e, "device->host copy");
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s.s_out);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) return fail_cuda(h, e, "device->host copy");
   return PIX_OK;

@@ -133,3 +133,10 @@ def test_deterministic_and_stream_independent(gu, full):
     for x, y in zip(a1, a2):
         for k in x:
             assert np.array_equal(x[k], y[k]), k
+
+
+def test_cfg2_host_pipelined(gu, full):
+    """pix_process_batch_host over several launch groups (input copy, kernels and output copy of consecutive groups
+    overlap on three streams): 20 PU50-like events + an empty one, outputs poisoned first."""
+    b = pixgen.events(full, ["pu50"] * 10 + ["empty"] + ["pu50"] * 10, np.arange(300, 321))
+    check(gu, full, b, mode="host")
