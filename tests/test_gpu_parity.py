@@ -140,3 +140,54 @@ def test_cfg2_host_pipelined(gu, full):
     overlap on three streams): 20 PU50-like events + an empty one, outputs poisoned first."""
     b = pixgen.events(full, ["pu50"] * 10 + ["empty"] + ["pu50"] * 10, np.arange(300, 321))
     check(gu, full, b, mode="host")
+
+
+def _hand_batch(det, events):
+    """events: list of (module, row, col, adc) arrays -> pixgen.Batch (modules emitted in the order given)."""
+    words, ev_off, fed_off = [], [0], []
+    for module, row, col, adc in events:
+        w, fo, _ = det.stream(np.asarray(module), np.asarray(row), np.asarray(col), np.asarray(adc))
+        words.append(w); ev_off.append(ev_off[-1] + len(w)); fed_off.append(fo)
+    return pixgen.Batch(np.concatenate(words).astype(np.uint32), np.array(ev_off, np.uint32),
+                        np.array(fed_off, np.uint32).reshape(len(events), det.n_feds + 1),
+                        np.zeros((len(events), 5), np.uint32))
+
+
+def test_run_lengths_across_kernel_tiers(gu, full):
+    """Hand-built events: one long run of n words after a filler run of k words, for n around every size at which
+    a run changes hands (findclus window 256 minus the start offset, findrun 512, block kernel's shared tier 1024)
+    and k shifting the start inside the 128-word chunk.  Pixels form staircase lines, blobs and isolated pixels so
+    that components span many rounds."""
+    rng = np.random.default_rng(11)
+    inv = full.inverse()
+    fed_of = inv["fed"]
+    mods = np.nonzero(fed_of == 0)[0][:2]  # two modules of FED 0: filler run, then the run under test
+    events = []
+    for n in (1, 31, 32, 33, 127, 128, 129, 130, 200, 255, 256, 257, 300, 511, 512, 513, 700, 1023, 1024, 1025, 1500):
+        for k in (0, 1, 64, 127):
+            pos = rng.choice(160 * 416, size=n, replace=False)          # scattered pixels ...
+            line = (np.arange(n) % 160) * 416 + (np.arange(n) * 3 // 2) % 416
+            sel = np.unique(np.where(rng.random(n) < 0.5, pos, line))    # ... mixed with staircase lines
+            rng.shuffle(sel)
+            sel = sel[:n]
+            fr, fc = np.arange(k) % 160, (np.arange(k) * 7) % 416
+            module = np.concatenate([np.full(k, mods[0]), np.full(len(sel), mods[1])])
+            row = np.concatenate([fr, sel // 416]); col = np.concatenate([fc, sel % 416])
+            adc = rng.integers(1, 256, size=len(module))
+            events.append((module, row, col, adc))
+    b = _hand_batch(full, events)
+    check(gu, full, b, chunk_events=9)
+
+
+def test_random_recipes(gu, full):
+    """Seeded sweep over the generator's knobs (cluster count from nearly empty to PU200-dense, long-cluster share,
+    read-out or shuffled word order, every edge class), ragged launch groups."""
+    rng = np.random.default_rng(5)
+    recipes = []
+    for _ in range(36):
+        recipes.append(dict(n_clusters=int(rng.choice([3, 50, 700, 5000, 15000, 30000, 45000])),
+                            inner_modules=int(rng.choice([0, 16, 96])), inner_weight=int(rng.choice([1, 4, 16])),
+                            long_permille=int(rng.choice([0, 0, 20, 150])), shuffle_order=int(rng.integers(0, 2)),
+                            edge_class=int(rng.choice([0, 0, 0, 1, 2, 3, 4]))))
+    b = pixgen.events(full, recipes, 9000 + np.arange(len(recipes)), cap_words_per_event=1 << 19)
+    check(gu, full, b, chunk_events=int(rng.integers(3, 9)))
