@@ -1,6 +1,6 @@
 // cluster.cu -- the overflow kernel: a4 findClus fused with a5 (cluster sums, charge cut, renumber, temp records)
-// for the module runs the fused tile kernel (fused.cu) could not take: runs longer than its window, tiles with
-// too many runs, charge sums beyond 32 bits.  One block per run, tables in the global workspace, 64-bit sums.
+// for the module runs the warp kernels (findclus.cu, findrun.cu) could not take: runs longer than 512 words, dense
+// runs that overflow a hash bucket neighbourhood, charge sums beyond 32 bits.  One block per run, tables in the global workspace, 64-bit sums.
 //
 // "clusters the pixels on each detector module".  The connectivity rule, the duplicate rule,
 // the canonical numbering and the charge cut are DESIGN.md readings S9, S10, S13, S14, S18.
@@ -17,7 +17,7 @@
 //   5  roots in digi order: Q >= cut survives and takes the next local id (ballot/popc scan); the root
 //      writes the temp record at (run first + id)
 //   6  per digi: final status and clus; per task: counts
-// The digi fields (row, col, charge) are read back from the output arrays the fused kernel has written.
+// The digi fields (row, col, charge) are read back from the output arrays the decode kernel has written.
 #include "pix_common.cuh"
 
 namespace pix {
@@ -243,7 +243,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     n_pre += tot_pre; n_post += tot_post;
   }
   g.sync();
-  // 6: final status and clus of every decodable digi (undecodable ones were finished by the fused kernel)
+  // 6: final status and clus of every decodable digi (undecodable ones were finished by the decode kernel)
   uint32_t n_ok = 0, n_cut = 0;
   for (uint32_t k = rk; k < n; k += gs) {
     const uint32_t p = T.pos[k];
