@@ -205,6 +205,18 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None  # sampled over the timed steps and their per-kernel repeat
     chunks_per_step = n_chunks // args.steps
 
+    # ---- SURVEY 8f NEXT-1, outside the step: RecHits-lite over the step's outputs (CUDA events on the launch stream)
+    hits = pix.alloc_hits(E, kmax, dev)
+    pix.pix_rechits(h, stream, E, ev_off, digis, clusters, hits)
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    r0.record(stream)
+    for _ in range(5):
+        pix.pix_rechits(h, stream, E, ev_off, digis, clusters, hits)
+    r1.record(stream)
+    torch.cuda.synchronize()
+    rechits_ms = r0.elapsed_time(r1) / 5
+    del hits
+
     # ---- what the step produced (for the byte counts) + a parity spot check against the oracle (rank 0)
     torch.cuda.synchronize()
     summ = clusters["summary"].cpu().numpy().reshape(E, 16).astype(np.int64)
@@ -303,6 +315,7 @@ def run_ours(args):
                                "algorithmic_bytes_per_step": chain_bytes, "formula": "19 W + 22 K + (12 M + 68) E"},
             "kernel_ms_per_step": prof, "kernel_algorithmic_bytes_per_step": kernel_bytes,
             "cpu_baseline": cpu, "parity_spot_check": parity,
+            "next": {"rechits_lite_ms_per_1000_events": rechits_ms * 1000.0 / E, "note": "pix_rechits, not part of the step"},
         }
         print(json.dumps(line))
     if dist is not None:

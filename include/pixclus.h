@@ -149,6 +149,28 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
                            uint32_t n_words_total, const uint32_t* event_word_offsets, const uint32_t* fed_offsets,
                            const pix_digis* out_digis, const pix_clusters* out_clusters);
 
+/* RecHits-lite ("The RecHits module estimates the 3D position of each cluster
+ * forming hits" -- only the module-local part: the detector geometry conditions are not available).
+ * Readings S25-S28 of DESIGN.md.  One hit per emitted cluster record, same index and same per-event stride
+ * (max_clusters_per_event): the per-module offsets of the hits are clus_module_start, which is what the
+ * paper's fillHitsModuleStart (Fig. 3) fills.
+ *   x_local, y_local  cm, origin at the module centre: x = (y_row + 0.5 - 80) * 0.0100, y = (x_col + 0.5 - 208) * 0.0150
+ *                     (binary32, three separately rounded operations each)
+ *   min_row .. max_col bounding box over the cluster's digis
+ *   flags             bit0 ON_EDGE (box touches row 0 / 159 or col 0 / 415), bit1 SPANS_ROC (box crosses the row
+ *                     79|80 boundary or a multiple-of-52 column boundary), bit2 SINGLE_PIXEL
+ * All pointers DEVICE.  Inputs are the outputs of pix_process_batch on the same handle / sizes (n_events events,
+ * event_word_offsets as given there).  Never allocates or synchronises; elements at and beyond an event's
+ * n_clusters_emitted are left untouched. */
+typedef struct {
+  float* x_local; float* y_local; uint16_t* min_row; uint16_t* max_row; uint16_t* min_col; uint16_t* max_col; uint8_t* flags;
+} pix_hits;
+#define PIX_HIT_ON_EDGE 1u
+#define PIX_HIT_SPANS_ROC 2u
+#define PIX_HIT_SINGLE_PIXEL 4u
+int pix_rechits(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* event_word_offsets,
+                const pix_digis* digis, const pix_clusters* clusters, const pix_hits* out_hits);
+
 /* Number of CUDA kernels this handle has launched so far (for launch accounting). */
 uint64_t pix_kernel_launches(const pix_handle* h);
 

@@ -51,6 +51,8 @@ def _load():
         lib.pixo_decode_word.restype = ctypes.c_int
         lib.pixo_calibrate.argtypes = [ctypes.c_uint8, ctypes.c_float, ctypes.c_float, ctypes.POINTER(Params)]
         lib.pixo_calibrate.restype = ctypes.c_int32
+        lib.pixo_rechits.argtypes = [ctypes.c_uint32, ctypes.c_uint32] + [vp] * 6 + [ctypes.c_uint32] + [vp] * 10
+        lib.pixo_rechits.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -102,3 +104,19 @@ def process(det, words: np.ndarray, fed_offsets, params: dict, max_clusters_per_
     for name in ("c_module", "c_first_digi", "c_n_pix", "c_charge", "c_x_col", "c_y_row"):
         out[name] = out[name][:k]
     return out
+
+
+def rechits(det, o: dict) -> dict:
+    """RecHits-lite (S25-S28) from one event's process() output -> hit arrays, one per emitted record."""
+    k = int(o["summary"][14])
+    h = dict(x_local=np.zeros(k, np.float32), y_local=np.zeros(k, np.float32), min_row=np.zeros(k, np.uint16),
+             max_row=np.zeros(k, np.uint16), min_col=np.zeros(k, np.uint16), max_col=np.zeros(k, np.uint16),
+             flags=np.zeros(k, np.uint8))
+    ins = [np.ascontiguousarray(o[n]) for n in ("module", "row", "col", "clus", "status", "clus_module_start")]
+    recs = [np.ascontiguousarray(o[n]) for n in ("c_n_pix", "c_x_col", "c_y_row")]
+    rc = _load().pixo_rechits(len(o["module"]), det.n_modules, *[a.ctypes.data for a in ins], k,
+                              *[a.ctypes.data for a in recs],
+                              *[h[n].ctypes.data for n in ("x_local", "y_local", "min_row", "max_row", "min_col", "max_col", "flags")])
+    if rc != 0:
+        raise ValueError(f"pixo_rechits returned {rc}")
+    return h

@@ -19,6 +19,8 @@
 // checkerboard, lattice, stripes, diagonal, no-wrap pair); the address bijection; step-by-step
 // numpy.float32 calibration over all 256 ADC values; charge conservation and the structural
 // invariants; metamorphic permutations; the generator's injected-error tallies.
+// RecHits-lite (pixo_rechits, readings S25-S28): closed forms on hand-built clusters and a numpy group-by
+// recomputation (tests/test_oracle_rechits.py).
 // PARITY UNPINNED against paper-printed values: the paper prints no worked example, count or
 // intermediate value for this path.
 #include <cstdint>
@@ -239,6 +241,45 @@ int pixo_process(uint32_t n_feds, uint32_t n_modules, const uint32_t* cabling, c
   summary[7] = n_dup; summary[8] = n_below; summary[9] = n_ok; summary[10] = n_cut;
   summary[11] = n_modules_present; summary[12] = n_precut; summary[13] = n_postcut; summary[14] = n_emitted;
   summary[15] = flags;
+  return 0;
+}
+
+// ---- RecHits-lite ("The RecHits module estimates the 3D position of each
+// cluster forming hits"; only the module-local part is computable here: geometry conditions are missing).
+// Readings S25-S28 of DESIGN.md: one hit per emitted cluster record, same index (the offsets are Fig. 3's
+// fillHitsModuleStart); bounding box over the cluster's OK digis; local position in cm from the
+// charge-weighted centroid with the module centre as origin and pitches 0.0100 cm (rows) x 0.0150 cm (columns),
+// three separately rounded binary32 operations per coordinate; flags ON_EDGE | SPANS_ROC << 1 | SINGLE_PIXEL << 2.
+// Inputs are one event's outputs of pixo_process.  Plain loops, no shared code with the CUDA path.
+int pixo_rechits(uint32_t n_words, uint32_t M, const uint16_t* d_module, const uint16_t* d_row, const uint16_t* d_col,
+                 const int32_t* d_clus, const uint8_t* d_status, const uint32_t* clus_module_start, uint32_t n_emitted,
+                 const uint32_t* c_n_pix, const float* c_x_col, const float* c_y_row,
+                 float* h_x_local, float* h_y_local, uint16_t* h_min_row, uint16_t* h_max_row, uint16_t* h_min_col,
+                 uint16_t* h_max_col, uint8_t* h_flags) {
+  for (uint32_t g = 0; g < n_emitted; ++g) { h_min_row[g] = 0xFFFF; h_max_row[g] = 0; h_min_col[g] = 0xFFFF; h_max_col[g] = 0; }
+  for (uint32_t i = 0; i < n_words; ++i) {
+    if (d_status[i] != ST_OK || d_clus[i] < 0) continue;
+    const uint32_t m = d_module[i];
+    if (m >= M) return 1;
+    const uint32_t l = (uint32_t)d_clus[i];
+    if (l >= clus_module_start[m + 1] - clus_module_start[m]) continue;  // beyond the per-module clamp: no record
+    const uint32_t g = clus_module_start[m] + l;
+    if (g >= n_emitted) continue;                                        // beyond the event capacity: no record
+    if (d_row[i] < h_min_row[g]) h_min_row[g] = d_row[i];
+    if (d_row[i] > h_max_row[g]) h_max_row[g] = d_row[i];
+    if (d_col[i] < h_min_col[g]) h_min_col[g] = d_col[i];
+    if (d_col[i] > h_max_col[g]) h_max_col[g] = d_col[i];
+  }
+  for (uint32_t g = 0; g < n_emitted; ++g) {
+    volatile float fx = c_y_row[g] + 0.5f; fx = fx - 80.0f; fx = fx * 0.0100f;    // S27: local x runs along the rows
+    volatile float fy = c_x_col[g] + 0.5f; fy = fy - 208.0f; fy = fy * 0.0150f;   //      local y along the columns
+    h_x_local[g] = fx; h_y_local[g] = fy;
+    uint8_t f = 0;
+    if (h_min_row[g] == 0 || h_max_row[g] == ROWS - 1 || h_min_col[g] == 0 || h_max_col[g] == COLS - 1) f |= 1;  // ON_EDGE
+    if ((h_min_row[g] < ROC_ROWS && h_max_row[g] >= ROC_ROWS) || h_min_col[g] / ROC_COLS != h_max_col[g] / ROC_COLS) f |= 2;  // SPANS_ROC
+    if (c_n_pix[g] == 1) f |= 4;                                                                                   // SINGLE_PIXEL
+    h_flags[g] = f;
+  }
   return 0;
 }
 

@@ -24,7 +24,8 @@ SUMMARY = ("n_words", "n_decoded", "n_empty", "n_err_link", "n_err_roc", "n_err_
            "n_clusters_emitted", "flags")
 FLAG_NONCONTIGUOUS, FLAG_CLUSTER_CAPACITY_OVERFLOW, FLAG_EVENT_TOO_LARGE = 1, 2, 4
 EXPORTS = ("pix_create", "pix_clone", "pix_destroy", "pix_process", "pix_process_batch", "pix_process_batch_host",
-           "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile", "pix_overflow_runs")
+           "pix_rechits", "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile",
+           "pix_overflow_runs")
 
 _vp, _u32 = ctypes.c_void_p, ctypes.c_uint32
 
@@ -51,6 +52,10 @@ class Digis(ctypes.Structure):
 class Clusters(ctypes.Structure):
     _fields_ = [(n, _vp) for n in ("module", "first_digi", "n_pix", "charge", "x_col", "y_row", "module_first",
                                    "module_end", "clus_module_start", "summary")]
+
+
+class Hits(ctypes.Structure):
+    _fields_ = [(n, _vp) for n in ("x_local", "y_local", "min_row", "max_row", "min_col", "max_col", "flags")]
 
 
 _lib = None
@@ -231,6 +236,34 @@ def pix_process_batch_host(h: Handle, stream, n_events: int, raw_words, n_words_
     rc = load().pix_process_batch_host(h.ptr, _stream_ptr(stream), n_events, _ptr(raw_words), n_words_total,
                                        _ptr(event_word_offsets), _ptr(fed_offsets), ctypes.byref(d), ctypes.byref(c))
     return _check(h, rc, raise_on_error)
+
+
+def pix_rechits(h: Handle, stream, n_events: int, event_word_offsets, digis: dict, clusters: dict, out_hits: dict,
+                raise_on_error: bool = True) -> int:
+    """RecHits-lite over the outputs of pix_process_batch (device pointers, asynchronous on `stream`)."""
+    d, c = _structs(digis, clusters)
+    hh = Hits(*[_ptr(out_hits.get(n)) for n, _ in Hits._fields_])
+    lib = load()
+    lib.pix_rechits.argtypes = [_vp, _vp, _u32, _vp, ctypes.POINTER(Digis), ctypes.POINTER(Clusters), ctypes.POINTER(Hits)]
+    lib.pix_rechits.restype = ctypes.c_int
+    rc = lib.pix_rechits(h.ptr, _stream_ptr(stream), n_events, _ptr(event_word_offsets), ctypes.byref(d), ctypes.byref(c),
+                         ctypes.byref(hh))
+    return _check(h, rc, raise_on_error)
+
+
+HIT_DTYPES = dict(x_local="float32", y_local="float32", min_row="uint16", max_row="uint16", min_col="uint16",
+                  max_col="uint16", flags="uint8")
+
+
+def alloc_hits(n_events: int, max_clusters_per_event: int, device="cuda", fill: int | None = None):
+    import torch
+    out = {}
+    for k, dt in HIT_DTYPES.items():
+        t = torch.empty(max(n_events * max_clusters_per_event, 1), dtype=getattr(torch, dt), device=device)
+        if fill is not None:
+            t.view(torch.uint8).fill_(fill)
+        out[k] = t
+    return out
 
 
 # ---------------------------------------------------------------- output buffers (torch: device memory only)

@@ -10,6 +10,11 @@
 #include "../../include/pixclus.h"
 #include "pix_common.cuh"
 
+namespace pix {
+void launch_rechits(uint32_t n_events, uint32_t M, uint32_t cap_ev, const uint32_t* ev_off, const pix_digis& d,
+                    const pix_clusters& k, const pix_hits& h, cudaStream_t stream);
+}
+
 namespace {
 
 struct SharedTables {  // read-only device tables shared by clones
@@ -395,6 +400,25 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
   if (e == cudaSuccess) e = cudaStreamSynchronize(s.s_out);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) return fail_cuda(h, e, "device->host copy");
+  return PIX_OK;
+}
+
+int pix_rechits(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* event_word_offsets,
+                const pix_digis* digis, const pix_clusters* clusters, const pix_hits* out_hits) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  h->err.clear();
+  if (n_events == 0) return PIX_OK;
+  if (!event_word_offsets || !out_hits) return fail(h, PIX_ERR_INVALID_ARG, "NULL argument");
+  if (int rc = check_outputs(h, digis, clusters)) return rc;
+  if (!out_hits->x_local || !out_hits->y_local || !out_hits->min_row || !out_hits->max_row || !out_hits->min_col ||
+      !out_hits->max_col || !out_hits->flags)
+    return fail(h, PIX_ERR_INVALID_ARG, "a hit output array is NULL");
+  if (n_events > h->p.max_events_per_batch) return fail(h, PIX_ERR_CAPACITY, "n_events > max_events_per_batch");
+  pix::launch_rechits(n_events, h->M, h->p.max_clusters_per_event, event_word_offsets, *digis, *clusters, *out_hits,
+                      (cudaStream_t)cuda_stream);
+  h->launches += (n_events + 65534u) / 65535u;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
   return PIX_OK;
 }
 

@@ -101,6 +101,7 @@ void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream
 void launch_decode(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
 void launch_findclus(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
 void launch_findrun(const Chunk& c, int n_sm, cudaStream_t stream);
+
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);
 cudaError_t configure_findclus_kernel();

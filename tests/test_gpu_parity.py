@@ -191,3 +191,41 @@ def test_random_recipes(gu, full):
                             edge_class=int(rng.choice([0, 0, 0, 1, 2, 3, 4]))))
     b = pixgen.events(full, recipes, 9000 + np.arange(len(recipes)), cap_words_per_event=1 << 19)
     check(gu, full, b, chunk_events=int(rng.integers(3, 9)))
+
+
+def test_rechits_lite(gu, full):
+    """pix_rechits (S25-S28) against the oracle's rechits on PU50, edge, duplicate, dense and PU200 events:
+    boxes and flags bit-exact, local positions within 1e-5 relative (they inherit the centroid's tolerance)."""
+    import oracle
+    import torch
+    import paper_2104_06573_b200 as pix
+    b = pixgen.events(full, ["pu50", "edges", "dups", "pu200", "dense", "empty", "pu50"], 500 + np.arange(7),
+                      cap_words_per_event=1 << 19)
+    E, M, F = b.n_events, full.n_modules, full.n_feds
+    sizes = np.diff(b.event_offsets.astype(np.int64))
+    W, wmax = int(sizes.sum()), int(sizes.max())
+    kmax = wmax
+    h = pix.pix_create(full.cabling, F, M, full.gain, full.pedestal, pix.make_params(P, wmax, kmax, E, 3))
+    try:
+        words = torch.from_numpy(np.concatenate([b.words, np.zeros(16, np.uint32)]).view(np.int32)).cuda()
+        ev_off = torch.from_numpy(b.event_offsets.view(np.int32).copy()).cuda()
+        fed_off = torch.from_numpy(b.fed_offsets.view(np.int32).reshape(-1).copy()).cuda()
+        digis, cl = pix.alloc_outputs(W, E, M, kmax, "cuda", fill=0xCD)
+        hits = pix.alloc_hits(E, kmax, "cuda", fill=0xCD)
+        pix.pix_process_batch(h, None, E, words, W, ev_off, fed_off, digis, cl)
+        pix.pix_rechits(h, None, E, ev_off, digis, cl, hits)
+        hn = gu.to_numpy(hits)
+        summ = gu.to_numpy({"s": cl["summary"]})["s"].reshape(E, 16)
+    finally:
+        torch.cuda.synchronize()
+        pix.pix_destroy(h)
+    for e in range(E):
+        o = oracle.process(full, *b.event(e), P, max_clusters_per_event=kmax)
+        ho = oracle.rechits(full, o)
+        k = int(summ[e, 14])
+        assert k == len(ho["flags"])
+        for name in ("min_row", "max_row", "min_col", "max_col", "flags"):
+            assert np.array_equal(hn[name][e * kmax:e * kmax + k], ho[name]), (e, name)
+        for name in ("x_local", "y_local"):
+            np.testing.assert_allclose(hn[name][e * kmax:e * kmax + k], ho[name], rtol=1e-5, atol=2e-6, err_msg=f"{e} {name}")
+        assert np.all(hn["flags"][e * kmax + k:(e + 1) * kmax] == 0xCD)  # untouched beyond n_clusters_emitted
