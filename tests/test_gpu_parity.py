@@ -229,3 +229,41 @@ def test_rechits_lite(gu, full):
         for name in ("x_local", "y_local"):
             np.testing.assert_allclose(hn[name][e * kmax:e * kmax + k], ho[name], rtol=1e-5, atol=2e-6, err_msg=f"{e} {name}")
         assert np.all(hn["flags"][e * kmax + k:(e + 1) * kmax] == 0xCD)  # untouched beyond n_clusters_emitted
+
+
+def test_graph_replay_equals_direct_launch(gu, full):
+    """pix_process never allocates, synchronises or copies to the host, so it can be captured into a CUDA graph
+    (BASELINE.json configs[2]: one graph launch per event); two replays reproduce the direct launch bit by bit."""
+    import torch
+    import paper_2104_06573_b200 as pix
+    b = pixgen.events(full, "pu50", [77])
+    n, M, F = len(b.words), full.n_modules, full.n_feds
+    h = gu.make_handle(full, P, n, n, 1, 1)
+    try:
+        words = torch.from_numpy(np.concatenate([b.words, np.zeros(16, np.uint32)]).view(np.int32)).cuda()
+        fo = torch.from_numpy(b.fed_offsets.view(np.int32).reshape(-1).copy()).cuda()
+        d0, c0 = pix.alloc_outputs(n, 1, M, n, "cuda", fill=0xCD)
+        s = torch.cuda.Stream()
+        pix.pix_process(h, s, words, fo, n, d0, c0)
+        torch.cuda.synchronize()
+        d1, c1 = pix.alloc_outputs(n, 1, M, n, "cuda", fill=0xCD)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            pix.pix_process(h, s, words, fo, n, d1, c1)
+        for _ in range(2):
+            for t in list(d1.values()) + list(c1.values()):
+                t.view(torch.uint8).fill_(0xCD)
+            torch.cuda.synchronize()
+            with torch.cuda.stream(s):
+                g.replay()
+            torch.cuda.synchronize()
+            k = int(c0["summary"][14])
+            for name in d0:
+                assert torch.equal(d0[name][:n], d1[name][:n]), name
+            for name in ("module", "first_digi", "n_pix", "charge", "x_col", "y_row"):
+                assert torch.equal(c0[name][:k], c1[name][:k]), name
+            for name in ("module_first", "module_end", "clus_module_start", "summary"):
+                assert torch.equal(c0[name], c1[name]), name
+    finally:
+        torch.cuda.synchronize()
+        pix.pix_destroy(h)
