@@ -47,7 +47,7 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.rows, self.proc = [], None
+        self.rows, self.proc, self.first = [], None, 0
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", "20"],
@@ -61,11 +61,20 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append([x.strip() for x in line.split(",")])
 
+    def mark(self, timeout=2.0):
+        """Waits until nvidia-smi delivers rows, then marks the start of the region of interest."""
+        t0 = time.perf_counter()
+        while self.proc and not self.rows and time.perf_counter() - t0 < timeout:
+            time.sleep(0.005)
+        self.first = len(self.rows)
+
     def stop(self):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
         self.t.join(timeout=2)
+        if len(self.rows) > self.first:
+            self.rows = self.rows[self.first:]  # samples taken after mark(): under load
         sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
@@ -241,11 +250,13 @@ def run_ours(args):
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events on the launch stream.
     # Inputs (242 MB) + outputs (~1.3 GB) per step exceed the 126 MB L2, so no explicit flush is needed.
+    sampler = ClockSampler(local) if rank == 0 else None  # started early: nvidia-smi needs ~0.1 s to deliver rows
     for _ in range(args.warmup):
         step()
+    if sampler:
+        sampler.mark()  # rows from here on are taken under load (timed steps + their per-kernel repeat)
     barrier()
     n0 = pix.pix_kernel_launches(h)
-    sampler = ClockSampler(local) if rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record(stream)
     for _ in range(args.steps):
