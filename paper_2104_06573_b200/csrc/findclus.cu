@@ -110,27 +110,18 @@ __device__ __forceinline__ uint32_t hfind(const WarpSmem& s, uint32_t h) {
 __device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0xFFu; }
 __device__ __forceinline__ bool slot_live(uint32_t e) { return e != EMPTY && !(e & 1u); }
 
-// union-find on s.label; labels strictly decrease along parents
-__device__ __forceinline__ uint32_t uf_find(volatile uint32_t* L, uint32_t x) {
-  uint32_t p = L[x];
-  while (p != x) {
-    const uint32_t gp = L[p];
-    if (gp != p) L[x] = gp;  // path halving; a racing hook only ever lowers a parent inside the same component
-    x = p; p = gp;
-  }
-  return x;
-}
-__device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
-  bool done = false;  // single exit: the lanes of a warp reconverge after the loop
+// Union on s.label (parent links, L[x] <= x): hook-and-descend, no root searches.  For the edge (a, b) with
+// hi = max, lo = min: p = atomicMin(&L[hi], lo).  p == hi: hi was a root and now hangs under lo; p == lo: already
+// linked.  Otherwise hi keeps the smaller of p and lo as its parent and the other one still has to be joined to it:
+// go on with the edge (p, lo), whose larger end is below hi, so the descent ends.  Links only ever join digis of one
+// component and point to smaller indices, so every component ends as one tree rooted at its lowest digi (S14).
+__device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
+  bool done = a == b;  // single exit: the lanes of a warp reconverge after the loop
   while (!done) {
-    a = uf_find(L, a); b = uf_find(L, b);
-    if (a == b) { done = true; }
-    else {
-      if (a < b) { const uint32_t t = a; a = b; b = t; }
-      const uint32_t old = atomicMin(L + a, b);  // hook the larger root under the smaller
-      if (old == a) done = true;
-      else a = old;                            // a was no longer a root: keep merging its parent with b
-    }
+    const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
+    const uint32_t p = atomicMin(L + hi, lo);
+    if (p == hi || p == lo) done = true;
+    else { a = p; b = lo; }
   }
 }
 
@@ -286,7 +277,6 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
     // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE are
     // joined to it by their own E edges, so d-S alone is enough.
     uint32_t ne = 0u;
-    bool flushed = false;  // the edge list was united early at least once (dense window)
 #pragma unroll 1
     for (uint32_t k = k0; k < k1; ++k) {
       const uint32_t t = 32u * k + lane, key = s.dkey[t];
@@ -295,11 +285,11 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
         for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
           if (i0 + lane < ne) {
             const uint32_t e = s.edge[i0 + lane];
-            uf_unite(s.label, e & 0xFFu, e >> 8);
+            hook(s.label, e & 0xFFu, e >> 8);
           }
           __syncwarp();
         }
-        ne = 0u; flushed = true;
+        ne = 0u;
       }
       const bool live = key != INVALID && s.label[t] < MAXT;
       bool f0 = false, f1 = false, f2 = false;
@@ -322,30 +312,19 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
       ne += __popc(m2);
     }
     __syncwarp();
-    if (!flushed) {
-      // first pass: every digi is still its own root, so an edge is one atomicMin (larger index under smaller).  A
-      // digi with two smaller neighbours keeps only the smaller one; the full pass below re-unites the other.
-      for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
-        if (i0 + lane < ne) {
-          const uint32_t e = s.edge[i0 + lane], a = e & 0xFFu, bb = e >> 8;
-          atomicMin(&s.label[a > bb ? a : bb], a > bb ? bb : a);
-        }
-      }
-      __syncwarp();
-#pragma unroll 1
-      for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: chains of the first pass shrink 4x
-        for (uint32_t k = k0; k < k1; ++k) {
-          const uint32_t t = 32u * k + lane;
-          const uint32_t l = s.label[t];
-          if (l < MAXT) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
-        }
-        __syncwarp();
-      }
-    }
     for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
       if (i0 + lane < ne) {
         const uint32_t e = s.edge[i0 + lane];
-        uf_unite(s.label, e & 0xFFu, e >> 8);
+        hook(s.label, e & 0xFFu, e >> 8);
+      }
+      __syncwarp();
+    }
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: the chains shrink 4x before the sums
+      for (uint32_t k = k0; k < k1; ++k) {
+        const uint32_t t = 32u * k + lane;
+        const uint32_t l = s.label[t];
+        if (l < MAXT) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
       }
       __syncwarp();
     }
