@@ -4,7 +4,7 @@
 //
 // One warp per run of up to RMAX = 512 words, tables in 15 KB of per-warp shared memory, the same phases as
 // findclus.cu with a single run: stage + insert into the position hash (512 buckets of 4 slots), duplicates,
-// forward-neighbour lookups -> edge list (united whenever it fills) -> lock-free min-index union-find, sums by
+// forward-neighbour lookups -> edge list (united whenever it fills) -> hook-and-descend unions, sums by
 // shared atomics, dense root list, cut + renumber in digi order, temp records, final status / clus, counters.
 // Longer runs, runs whose hash bucket neighbourhood overflows and charge sums beyond 32 bits go on to the block
 // kernel (cluster.cu).  Nothing here is shared with oracle/.
@@ -77,33 +77,21 @@ __device__ __forceinline__ uint32_t hfind(const RunSmem& s, uint32_t h) {
 __device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x1FFu; }
 __device__ __forceinline__ bool slot_live(uint32_t e) { return e != EMPTY && !(e & 1u); }
 
-__device__ __forceinline__ uint32_t uf_find(volatile uint32_t* L, uint32_t x) {
-  uint32_t p = L[x];
-  while (p != x) {
-    const uint32_t gp = L[p];
-    if (gp != p) L[x] = gp;  // path halving
-    x = p; p = gp;
-  }
-  return x;
-}
-__device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
-  bool done = false;  // single exit: the lanes of a warp reconverge after the loop
+// hook-and-descend union (see findclus.cu): one atomicMin per step, no root searches
+__device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
+  bool done = a == b;  // single exit: the lanes of a warp reconverge after the loop
   while (!done) {
-    a = uf_find(L, a); b = uf_find(L, b);
-    if (a == b) { done = true; }
-    else {
-      if (a < b) { const uint32_t t = a; a = b; b = t; }
-      const uint32_t old = atomicMin(L + a, b);
-      if (old == a) done = true;
-      else a = old;
-    }
+    const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
+    const uint32_t p = atomicMin(L + hi, lo);
+    if (p == hi || p == lo) done = true;
+    else { a = p; b = lo; }
   }
 }
 __device__ __forceinline__ void unite_edges(RunSmem& s, uint32_t ne, uint32_t lane) {
   for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count
     if (i0 + lane < ne) {
       const uint32_t e = s.edge[i0 + lane];
-      uf_unite(s.label, e & 0xFFFFu, e >> 16);
+      hook(s.label, e & 0xFFFFu, e >> 16);
     }
     __syncwarp();
   }
@@ -182,14 +170,13 @@ __global__ void __launch_bounds__(RWPB * 32) findrun_kernel(const __grid_constan
     }
     // ---- forward neighbours (S13) -> edges -> unions
     uint32_t ne = 0u;
-    bool flushed = false;
 #pragma unroll 1
     for (uint32_t k = 0; k < nk; ++k) {
       const uint32_t t = 32u * k + lane, key = s.dkey[t];
       if (ne + 96u > RECAP) {  // the round's edges might not fit: unite what is listed (warp-uniform)
         __syncwarp();
         unite_edges(s, ne, lane);
-        ne = 0u; flushed = true;
+        ne = 0u;
       }
       const bool live = key != INVALID && s.label[t] < RMAX;
       bool f0 = false, f1 = false, f2 = false;
@@ -212,25 +199,16 @@ __global__ void __launch_bounds__(RWPB * 32) findrun_kernel(const __grid_constan
       ne += __popc(m2);
     }
     __syncwarp();
-    if (!flushed) {  // first pass: every digi is still its own root, so an edge is one atomicMin; then two jumps
-      for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
-        if (i0 + lane < ne) {
-          const uint32_t e = s.edge[i0 + lane], a = e & 0xFFFFu, bb = e >> 16;
-          atomicMin(&s.label[a > bb ? a : bb], a > bb ? bb : a);
-        }
+    unite_edges(s, ne, lane);
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: the chains shrink 4x before the sums
+      for (uint32_t k = 0; k < nk; ++k) {
+        const uint32_t t = 32u * k + lane;
+        const uint32_t l = s.label[t];
+        if (l < RMAX) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
       }
       __syncwarp();
-#pragma unroll 1
-      for (int pass = 0; pass < 2; ++pass) {
-        for (uint32_t k = 0; k < nk; ++k) {
-          const uint32_t t = 32u * k + lane;
-          const uint32_t l = s.label[t];
-          if (l < RMAX) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
-        }
-        __syncwarp();
-      }
     }
-    unite_edges(s, ne, lane);
     __syncwarp();  // components complete; the hash is dead, its memory becomes q / np / sx / sy
     // ---- sums; dense list of the roots
     {
