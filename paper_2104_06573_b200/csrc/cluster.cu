@@ -11,8 +11,8 @@
 //      row*416+col; equal keys keep the MIN digi index (S10: first index wins)
 //   2  a digi that is not the owner of its position is a DUPLICATE
 //   3  every live digi (owner, charge >= threshold) looks up its 4 forward neighbours
-//      (r,c+1) (r+1,c-1) (r+1,c) (r+1,c+1) and unites with live owners: lock-free union-find,
-//      larger root hooked under smaller root with atomicMin => the root is the component's min digi index
+//      (r,c+1) (r+1,c-1) (r+1,c) (r+1,c+1) and unites with live owners: hook-and-descend with atomicMin
+//      (larger index under smaller) => the root is the component's min digi index
 //   4  flatten labels; add charge, pixel count and charge-weighted col/row into the root's accumulators
 //   5  roots in digi order: Q >= cut survives and takes the next local id (ballot/popc scan); the root
 //      writes the temp record at (run first + id)
@@ -72,15 +72,16 @@ __device__ __forceinline__ uint32_t hash_find(const SlotT* tab, uint32_t size, u
   }
 }
 
-// ------------------------------------------------------------------ union-find (labels strictly decrease along parents)
-__device__ __forceinline__ uint32_t uf_find(volatile uint32_t* L, uint32_t x) {
-  uint32_t p = L[x];
-  while (p != x) {
-    const uint32_t gp = L[p];
-    if (gp != p) L[x] = gp;  // path halving; a racing hook only ever lowers a parent inside the same component
-    x = p; p = gp;
+// ------------------------------------------------------------------ unions (labels strictly decrease along parents)
+// hook-and-descend (see findclus.cu): one atomicMin per step, no root searches
+__device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
+  bool done = a == b;
+  while (!done) {
+    const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
+    const uint32_t p = atomicMin(L + hi, lo);
+    if (p == hi || p == lo) done = true;
+    else { a = p; b = lo; }
   }
-  return x;
 }
 // read-only walk to the root (step 4: own entries are being flattened concurrently, nobody else's may be written)
 __device__ __forceinline__ uint32_t uf_root(const volatile uint32_t* L, uint32_t x) {
@@ -88,17 +89,6 @@ __device__ __forceinline__ uint32_t uf_root(const volatile uint32_t* L, uint32_t
   while (p != x) { x = p; p = L[x]; }
   return x;
 }
-__device__ __forceinline__ void uf_unite(uint32_t* L, uint32_t a, uint32_t b) {
-  while (true) {
-    a = uf_find(L, a); b = uf_find(L, b);
-    if (a == b) return;
-    if (a < b) { const uint32_t t = a; a = b; b = t; }
-    const uint32_t old = atomicMin(L + a, b);  // hook the larger root under the smaller
-    if (old == a) return;
-    a = old;                                   // a was no longer a root: keep merging its parent with b
-  }
-}
-
 // ------------------------------------------------------------------ groups
 template <int THREADS>
 struct BlockGroup {
@@ -199,7 +189,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
       const uint32_t j = hash_find(T.tab, size, nkey);
       if (j == NO_INDEX) continue;
       if (!(((volatile uint32_t*)T.pos)[j] & LIVE)) continue;
-      uf_unite(T.label, k, j);
+      hook(T.label, k, j);
     }
   }
   g.sync();
