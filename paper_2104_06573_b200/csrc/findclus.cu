@@ -68,8 +68,9 @@ static_assert(sizeof(WarpSmem) % 16 == 0, "per-warp slices stay 16-byte aligned"
 // bucket fill in order and are never emptied; equal keys meet in one slot and keep the lowest digi (S10).
 __device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
 
-// 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets
-__device__ __forceinline__ uint32_t hinsert(WarpSmem& s, uint32_t key, uint32_t t, uint32_t below) {
+// 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets.
+// Not inlined: eight copies in the unrolled staging rounds cost more in instruction fetch than the call.
+__device__ __noinline__ uint32_t hinsert(WarpSmem& s, uint32_t key, uint32_t t, uint32_t below) {
   const uint32_t h = hmix(key), tag = h & TAG_MASK;
   uint32_t p = (h >> TAG_BITS) * 4u, res = 2u;
 #pragma unroll 1
@@ -126,6 +127,14 @@ __device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
 }
 
 // (event, FED) of word g >= b, given the segment sg0 of the chunk's first word and the next boundary nextB0
+// rare: word g lies beyond the segment of the chunk's first word (a FED / event boundary inside the window)
+__device__ __noinline__ uint2 event_of(const Chunk& c, uint32_t S, uint32_t sg0, uint32_t g) {
+  uint32_t sg = sg0 + 1u;
+  while (sg + 1u < S && c.segB[sg + 1u] <= g) ++sg;
+  const uint32_t er = sg / c.F;
+  return make_uint2(er, c.segB[er * c.F]);  // event of the launch group, global index of its word 0
+}
+
 __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -229,11 +238,7 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
         const int32_t e = ch[j];
         if (in && md[j] != 0xFFFFFFFFu) {  // the first digi of run r
           uint32_t er = er0, eb = ebase0;
-          if (g >= nextB0) {  // rare: a FED / event boundary inside the window
-            uint32_t sg = sg0 + 1u;
-            while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
-            er = sg / F; eb = segB[er * F];
-          }
+          if (g >= nextB0) { const uint2 ev = event_of(c, S, sg0, g); er = ev.x; eb = ev.y; }
           s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | md[j]; s.run_ifirst[r] = g - eb;
         }
         const bool dec = in && row != 0xFFFFu;
@@ -255,9 +260,8 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
       for (uint32_t k = 0; k < 4; ++k) {
         const uint32_t g = b + 32u * k + lane;
         if ((sb[k] >> lane & 1u) && rb[k] + __popc(sb[k] & le_mask) > RC) {
-          uint32_t sg = sg0;
-          while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
-          push_overflow(c, ((sg / F) << 16) | c.d_module[g]);
+          const uint32_t er = g >= nextB0 ? event_of(c, S, sg0, g).x : er0;
+          push_overflow(c, (er << 16) | c.d_module[g]);
         }
       }
     } else if (!fits && lane == 0) {
