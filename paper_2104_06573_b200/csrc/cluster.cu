@@ -264,7 +264,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
 // ------------------------------------------------------------------ kernel
 // Runs of up to SMEM_CAP digis keep all their tables in shared memory; longer ones use the global workspace.
 constexpr int OVF_THREADS = 256;
-constexpr uint32_t SMEM_CAP = 1024;
+constexpr uint32_t SMEM_CAP = 2048;
 constexpr size_t SMEM_PER_DIGI = 8 + 8 + 2 * 4 + 4 * 5;  // sx, sy, 2 hash slots, pos, chg, label, q, npix
 constexpr size_t OVF_SMEM = SMEM_CAP * SMEM_PER_DIGI;
 
@@ -320,7 +320,7 @@ cudaError_t configure_overflow_kernel() {
 }
 
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
-  overflow_kernel<<<n_sm * 4, OVF_THREADS, OVF_SMEM, stream>>>(c);
+  overflow_kernel<<<n_sm * 2, OVF_THREADS, OVF_SMEM, stream>>>(c);
 }
 
 }  // namespace pix

@@ -2,8 +2,8 @@
 // renumber / temp records (S9, S14, S18) for the module runs the chunk kernel (findclus.cu) could not take
 // because they do not fit its 256-word window ("clusters the pixels on each detector module").
 //
-// One warp per run of up to RMAX = 512 words, tables in 15 KB of per-warp shared memory, the same phases as
-// findclus.cu with a single run: stage + insert into the position hash (512 buckets of 4 slots), duplicates,
+// One warp per run, in two sizes: up to 512 words (15 KB of per-warp shared memory) and up to 1024 words (29 KB);
+// the same phases as findclus.cu with a single run: stage + insert into the position hash (4 slots per bucket), duplicates,
 // forward-neighbour lookups -> edge list (united whenever it fills) -> hook-and-descend unions, sums by
 // shared atomics, dense root list, cut + renumber in digi order, temp records, final status / clus, counters.
 // Longer runs, runs whose hash bucket neighbourhood overflows and charge sums beyond 32 bits go on to the block
@@ -14,67 +14,74 @@ namespace pix {
 
 namespace {
 
-constexpr int RWPB = 2;                   // warps per block
-constexpr uint32_t RMAX = 512;            // words of a run
-constexpr uint32_t RTAB = 2048;           // hash slots: 512 buckets of 4
 constexpr uint32_t RECAP = 256;           // edge list entries
 constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;
 constexpr uint32_t HASH_MUL = 0x9E3779B1u;
-constexpr uint32_t KEY_BITS = 17, KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = 8, TAG_MASK = (1u << TAG_BITS) - 1u;
-constexpr uint32_t NBUCKET = RTAB / 4, MAX_DISP = 3;
-static_assert((1u << (KEY_BITS - TAG_BITS)) == NBUCKET, "key: row (8) | col (9); slot: disp (2) | tag (8) | digi (9) | below (1)");
+constexpr uint32_t KEY_BITS = 17, KEY_MASK = (1u << KEY_BITS) - 1u, MAX_DISP = 3;
+// Two sizes of the kernel: RM = 512 words per run (15 KB of shared memory per warp, 2 warps per block) and
+// RM = 1024 (29 KB, 1 warp per block).  Hash: RM buckets of 4 slots; key: row (8) | col (9);
+// slot: disp (2) | tag (17 - log2 RM) | digi (10) | below (1).
+template <uint32_t RM> struct RK {
+  static_assert(RM == 512 || RM == 1024, "run sizes");
+  static constexpr uint32_t RTAB = 4 * RM, NBUCKET = RM, TAG_BITS = RM == 512 ? 8 : 7, TAG_MASK = (1u << RK<RM>::TAG_BITS) - 1u;
+  static constexpr int WPB = RM == 512 ? 2 : 1;
+};
 
+template <uint32_t RM>
 struct __align__(16) RunSmem {
-  uint32_t tab[RTAB];     // position hash; after the lookups: q = tab, np = tab + 512, sx = tab + 1024, sy = tab + 1536
-  uint32_t dkey[RMAX];    // row << 9 | col, INVALID for an undecodable word
-  uint32_t label[RMAX];   // union-find parent, or MARK_*
+  uint32_t tab[4 * RM];   // position hash; after the lookups: q = tab, np = tab + RM, sx = tab + 2 RM, sy = tab + 3 RM
+  uint32_t dkey[RM];    // row << 9 | col, INVALID for an undecodable word
+  uint32_t label[RM];   // union-find parent, or MARK_*
   uint32_t edge[RECAP];   // a | b << 16
-  uint16_t chg[RMAX];     // charge; after the sums: local id of a root, or NO_ID
-  uint16_t rlist[RMAX];   // roots in digi order
+  uint16_t chg[RM];     // charge; after the sums: local id of a root, or NO_ID
+  uint16_t rlist[RM];   // roots in digi order
 };
 
 __device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
 // 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets
-__device__ __forceinline__ uint32_t hinsert(RunSmem& s, uint32_t key, uint32_t t, uint32_t below) {
-  const uint32_t h = hmix(key), tag = h & TAG_MASK;
-  uint32_t p = (h >> TAG_BITS) * 4u, res = 2u;
+template <uint32_t RM>
+__device__ __forceinline__ uint32_t hinsert(RunSmem<RM>& s, uint32_t key, uint32_t t, uint32_t below) {
+  const uint32_t h = hmix(key), tag = h & RK<RM>::TAG_MASK;
+  uint32_t p = (h >> RK<RM>::TAG_BITS) * 4u, res = 2u;
 #pragma unroll 1
-  for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u) && res == 2u; ++i, p = (p + 1u) & (RTAB - 1u)) {
-    const uint32_t want = ((i >> 2) << TAG_BITS) | tag, mine = (want << 10) | (t << 1) | below;
+  for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u) && res == 2u; ++i, p = (p + 1u) & (RK<RM>::RTAB - 1u)) {
+    const uint32_t want = ((i >> 2) << RK<RM>::TAG_BITS) | tag, mine = (want << 11) | (t << 1) | below;
     const uint32_t old = atomicCAS(&s.tab[p], EMPTY, mine);
     if (old == EMPTY) res = 0u;
-    else if ((old >> 10) == want) { atomicMin(&s.tab[p], mine); res = 1u; }  // same pixel: the lowest digi owns it
+    else if ((old >> 11) == want) { atomicMin(&s.tab[p], mine); res = 1u; }  // same pixel: the lowest digi owns it
   }
   return res;
 }
 __device__ __forceinline__ uint32_t half_match(const uint4& e, uint32_t want) {
   uint32_t r = EMPTY;
-  if ((e.w >> 10) == want) r = e.w;
-  if ((e.z >> 10) == want) r = e.z;
-  if ((e.y >> 10) == want) r = e.y;
-  if ((e.x >> 10) == want) r = e.x;
+  if ((e.w >> 11) == want) r = e.w;
+  if ((e.z >> 11) == want) r = e.z;
+  if ((e.y >> 11) == want) r = e.y;
+  if ((e.x >> 11) == want) r = e.x;
   return r;
 }
-__device__ __noinline__ uint32_t hfind_slow(const RunSmem& s, uint32_t h) {
-  const uint32_t tag = h & TAG_MASK;
-  uint32_t b = h >> TAG_BITS, r = EMPTY;
+template <uint32_t RM>
+__device__ __noinline__ uint32_t hfind_slow(const RunSmem<RM>& s, uint32_t h) {
+  const uint32_t tag = h & RK<RM>::TAG_MASK;
+  uint32_t b = h >> RK<RM>::TAG_BITS, r = EMPTY;
   for (uint32_t i = 1; i <= MAX_DISP && r == EMPTY; ++i) {
-    b = (b + 1u) & (NBUCKET - 1u);
+    b = (b + 1u) & (RK<RM>::NBUCKET - 1u);
     const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[b * 4u]);
-    r = half_match(e, (i << TAG_BITS) | tag);
+    r = half_match(e, (i << RK<RM>::TAG_BITS) | tag);
     if (e.w == EMPTY) break;
   }
   return r;
 }
-__device__ __forceinline__ uint32_t hfind(const RunSmem& s, uint32_t h) {
-  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> TAG_BITS) * 4u]);
-  uint32_t r = half_match(e, h & TAG_MASK);
-  if (r == EMPTY && e.w != EMPTY) r = hfind_slow(s, h);
+template <uint32_t RM>
+__device__ __forceinline__ uint32_t hfind(const RunSmem<RM>& s, uint32_t h) {
+  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> RK<RM>::TAG_BITS) * 4u]);
+  uint32_t r = half_match(e, h & RK<RM>::TAG_MASK);
+  if (r == EMPTY && e.w != EMPTY) r = hfind_slow<RM>(s, h);
   return r;
 }
-__device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x1FFu; }
+__device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x3FFu; }
 __device__ __forceinline__ bool slot_live(uint32_t e) { return e != EMPTY && !(e & 1u); }
 
 // hook-and-descend union (see findclus.cu): one atomicMin per step, no root searches
@@ -87,7 +94,8 @@ __device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
     else { a = p; b = lo; }
   }
 }
-__device__ __forceinline__ void unite_edges(RunSmem& s, uint32_t ne, uint32_t lane) {
+template <uint32_t RM>
+__device__ __forceinline__ void unite_edges(RunSmem<RM>& s, uint32_t ne, uint32_t lane) {
   for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count
     if (i0 + lane < ne) {
       const uint32_t e = s.edge[i0 + lane];
@@ -101,31 +109,37 @@ __device__ __forceinline__ void push_block(const Chunk& c, uint32_t task) {
   if (i < c.ovf_cap) c.ovf_list[i] = task;
 }
 
-__global__ void __launch_bounds__(RWPB * 32) findrun_kernel(const __grid_constant__ Chunk c) {
+template <uint32_t RM>
+__global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_constant__ Chunk c, const uint32_t* __restrict__ in_list, uint32_t ctl_count,
+                                                                   uint32_t ctl_ticket, uint32_t* __restrict__ long_list, uint32_t ctl_long) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  RunSmem& s = reinterpret_cast<RunSmem*>(smem_raw)[warp];
+  RunSmem<RM>& s = reinterpret_cast<RunSmem<RM>*>(smem_raw)[warp];
+  constexpr uint32_t RMAX = RM, RTAB = RK<RM>::RTAB;
   const uint32_t lt_mask = (1u << lane) - 1u;
   constexpr uint32_t FULL = 0xFFFFFFFFu, NO_ID = 0xFFFFu;
   uint32_t* const q = s.tab; uint32_t* const np = s.tab + RMAX; uint32_t* const sx = s.tab + 2 * RMAX;
   uint32_t* const sy = s.tab + 3 * RMAX;
   uint16_t* const lid = s.chg;
-  uint32_t count = c.ctl[CTL_MID_COUNT];
+  uint32_t count = c.ctl[ctl_count];
   count = count < c.ovf_cap ? count : c.ovf_cap;
   const uint32_t gBeg = c.segB[0];
 
   while (true) {
     uint32_t ti = 0u;
-    if (lane == 0) ti = atomicAdd(c.ctl + CTL_MID_TICKET, 1u);
+    if (lane == 0) ti = atomicAdd(c.ctl + ctl_ticket, 1u);
     ti = __shfl_sync(FULL, ti, 0);
     if (ti >= count) break;
-    const uint32_t task = c.mid_list[ti];
+    const uint32_t task = in_list[ti];
     const uint32_t er = task / c.M, m = task - er * c.M;
     if (c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] & FLAG_NONCONTIGUOUS) continue;  // S11: not clustered
     const size_t mo = (size_t)(c.e0 + er) * c.M + m;
     const uint32_t first = c.module_first[mo], n = c.module_end[mo] - first;
-    if (n > RMAX) {  // too long for a warp: the block kernel takes it
-      if (lane == 0) push_block(c, task);
+    if (n > RMAX) {  // too long for this size of the kernel: the next one takes it
+      if (lane == 0) {
+        const uint32_t i = atomicAdd(c.ctl + ctl_long, 1u);
+        if (i < c.ovf_cap) long_list[i] = task;
+      }
       continue;
     }
     const uint32_t gb = c.segB[er * c.F] + first;  // global index of the run's digi 0
@@ -297,11 +311,19 @@ __global__ void __launch_bounds__(RWPB * 32) findrun_kernel(const __grid_constan
 }  // namespace
 
 cudaError_t configure_findrun_kernel() {
-  return cudaFuncSetAttribute(findrun_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RWPB * sizeof(RunSmem)));
+  cudaError_t e = cudaFuncSetAttribute(findrun_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)(RK<512>::WPB * sizeof(RunSmem<512>)));
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(findrun_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)(RK<1024>::WPB * sizeof(RunSmem<1024>)));
 }
 
+// runs of up to 512 words first (findclus's list); what is longer goes to the 1024-word size, then to the block kernel
 void launch_findrun(const Chunk& c, int n_sm, cudaStream_t stream) {
-  findrun_kernel<<<n_sm * 7, RWPB * 32, RWPB * sizeof(RunSmem), stream>>>(c);
+  findrun_kernel<512><<<n_sm * 7, RK<512>::WPB * 32, RK<512>::WPB * sizeof(RunSmem<512>), stream>>>(
+      c, c.mid_list, CTL_MID_COUNT, CTL_MID_TICKET, c.big_list, CTL_BIG_COUNT);
+  findrun_kernel<1024><<<n_sm * 7, RK<1024>::WPB * 32, RK<1024>::WPB * sizeof(RunSmem<1024>), stream>>>(
+      c, c.big_list, CTL_BIG_COUNT, CTL_BIG_TICKET, c.ovf_list, CTL_OVF_COUNT);
 }
 
 }  // namespace pix

@@ -9,7 +9,7 @@
 //   decode    -> a1 decode + a2 calibrate + a3 run boundaries, streaming, 4 words per thread; one start bit per word
 //   findclus  -> a4 findClus + a5 sums/cut/renumber for every module run that fits a warp's 256-word window
 //                (home chunk of 128 words + look-ahead)
-//   findrun   -> a4 + a5 for runs of up to 512 words that do not fit a findclus window: one warp per run
+//   findrun   -> a4 + a5 for runs that do not fit a findclus window: one warp per run, two sizes (512 / 1024 words)
 //   overflow  -> a4 + a5 for the runs neither could take (longer than the window, pathological
 //                charge sums): generic block-per-run kernel, tables in global workspace
 //   offsets   -> a6 clamp + prefix scan (Fig. 3), summary, scatter work list
@@ -37,7 +37,7 @@ constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus;
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
        EC_PRECUT, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_WORDS = 16 };
 
 // Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
 //   x = module | bad << 16 | scol << 24     bad: 0, ST_ERR_LINK or ST_ERR_ROC; scol = +1 / -1 (int8)
@@ -79,6 +79,7 @@ struct Chunk {
   uint32_t* ev_cnt;         // [(e1-e0)*EC_STRIDE]
   uint32_t* ctl;            // [CTL_WORDS]
   uint32_t* mid_list;       // [(e1-e0)*M] task ids left by findclus to the warp-per-run kernel (findrun)
+  uint32_t* big_list;       // [(e1-e0)*M] runs of 513..1024 words, left by findrun<512> to findrun<1024>
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
   uint32_t ovf_cap;
   uint32_t* startbits;      // [cap_words/32 + 8] bit (g - T0): word g starts a module run (decode -> findclus)
@@ -109,6 +110,6 @@ cudaError_t configure_findrun_kernel();
 cudaError_t configure_finalize_kernel();
 cudaError_t configure_overflow_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 8;    // init, segfill, decode, findclus, findrun, overflow, offsets, scatter
+constexpr int LAUNCHES_PER_CHUNK = 9;    // init, segfill, decode, findclus, findrun x2, overflow, offsets, scatter
 
 }  // namespace pix
