@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
       __syncwarp();
     }
     // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE are
-    // joined to it by their own E edges, so d-S alone is enough.
+    // joined to it by their own E edges, so d-S alone is enough; when E is live, SE is E's S neighbour.
     uint32_t ne = 0u;
 #pragma unroll 1
     for (uint32_t k = k0; k < k1; ++k) {
@@ -305,7 +305,7 @@ __global__ void __launch_bounds__(FT, 7) findclus_kernel(const __grid_constant__
         const bool hS = slot_live(eS);
         f0 = slot_live(eE); n0 = slot_digi(eE);
         f1 = hS || slot_live(eSW); n1 = slot_digi(hS ? eS : eSW);
-        f2 = !hS && slot_live(eSE); n2 = slot_digi(eSE);
+        f2 = !hS && !f0 && slot_live(eSE); n2 = slot_digi(eSE);  // with E live, SE is E's S: E joins it
       }
       const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
       if (f0) s.edge[ne + __popc(m0 & lt_mask)] = (uint16_t)(t | (n0 << 8));

@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
         const bool hS = slot_live(eS);
         f0 = slot_live(eE); n0 = slot_digi(eE);
         f1 = hS || slot_live(eSW); n1 = slot_digi(hS ? eS : eSW);
-        f2 = !hS && slot_live(eSE); n2 = slot_digi(eSE);
+        f2 = !hS && !f0 && slot_live(eSE); n2 = slot_digi(eSE);  // with E live, SE is E's S: E joins it
       }
       const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
       if (f0) s.edge[ne + __popc(m0 & lt_mask)] = t | (n0 << 16);
