@@ -296,7 +296,7 @@ def run_ours(args):
     # algorithmic bytes per kernel: decode reads the raw word and writes module/row/col/charge
     # (11 B); findclus writes clus + status (5 B) and the 20 B temp record (its digi inputs are intermediates, not
     # algorithmic traffic); finalize moves the records (20 B in, 22 B out) and writes the per-event arrays
-    kernel_bytes = {"init": 12 * M * E, "decode": 15 * W, "findclus": 5 * W + 20 * K, "findrun": 0, "overflow": 0,
+    kernel_bytes = {"init": 12 * M * E, "fused": 19 * W + 20 * K, "findrun": 0, "overflow": 0,
                     "finalize": 42 * K + (4 * (M + 1) + 64 + 4 * M) * E}
     top = max(prof, key=prof.get)
     peak, peak_src = peak_hbm()

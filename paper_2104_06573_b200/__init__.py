@@ -180,7 +180,7 @@ def pix_overflow_runs(h: Handle) -> int:
     return int(n.value)
 
 
-KERNEL_FAMILIES = ("init", "decode", "findclus", "findrun", "overflow", "finalize")
+KERNEL_FAMILIES = ("init", "fused", "findrun", "overflow", "finalize")
 
 
 def pix_set_profiling(h: Handle, enable: bool) -> None:

@@ -80,12 +80,12 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.ovf_list = (uint32_t*)take(Ec * M * 4);
   c.mid_list = (uint32_t*)take(Ec * M * 4);
   c.big_list = (uint32_t*)take(Ec * M * 4);
-  c.ovf_cap = (uint32_t)(Ec * M);
+  c.list_cap = (uint32_t)(Ec * M);
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
-  c.startbits = (uint32_t*)take((W / 32 + 8) * 4);
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
   c.n_clus = (uint32_t*)take(Ec * M * 4);
-  c.t_rec = (pix::TempRec*)take(W * sizeof(pix::TempRec));
+  c.t_a = (uint4*)take(W * sizeof(uint4));
+  c.t_y = (float*)take(W * sizeof(float));
   c.g_hash = (unsigned long long*)take(W * 16);
   c.g_pos = (uint32_t*)take(W * 4); c.g_q = (uint32_t*)take(W * 4); c.g_npix = (uint32_t*)take(W * 4);
   c.g_sx = (unsigned long long*)take(W * 8); c.g_sy = (unsigned long long*)take(W * 8);
@@ -129,7 +129,7 @@ void bind_outputs(pix::Chunk& c, const pix_digis* d, const pix_clusters* k) {
 }
 
 // the launch sequence of one chunk
-constexpr int PROF_EVENTS = 7;  // families: init, decode, findclus, findrun, overflow, finalize (offsets + scatter)
+constexpr int PROF_EVENTS = 6;  // families: init, fused, findrun, overflow, finalize (offsets + scatter)
 int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t words_bound, cudaStream_t s) {
   cudaEvent_t* ev = nullptr;
   if (h->profiling) {
@@ -144,16 +144,14 @@ int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t wor
   }
   pix::launch_init(c, n_total, h->n_sm, s);
   if (ev) cudaEventRecord(ev[1], s);
-  pix::launch_decode(c, words_bound, h->n_sm, s);
+  pix::launch_fused(c, words_bound, h->n_sm, s);
   if (ev) cudaEventRecord(ev[2], s);
-  pix::launch_findclus(c, words_bound, h->n_sm, s);
-  if (ev) cudaEventRecord(ev[3], s);
   pix::launch_findrun(c, h->n_sm, s);
-  if (ev) cudaEventRecord(ev[4], s);
+  if (ev) cudaEventRecord(ev[3], s);
   pix::launch_overflow(c, h->n_sm, s);
-  if (ev) cudaEventRecord(ev[5], s);
+  if (ev) cudaEventRecord(ev[4], s);
   pix::launch_finalize(c, h->n_sm, s);
-  if (ev) cudaEventRecord(ev[6], s);
+  if (ev) cudaEventRecord(ev[5], s);
   h->launches += pix::LAUNCHES_PER_CHUNK;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
@@ -180,7 +178,7 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   h->F = F; h->M = M; h->p = *params;
   cudaError_t e = cudaGetDevice(&h->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
-  if (e == cudaSuccess) e = pix::configure_findclus_kernel();
+  if (e == cudaSuccess) e = pix::configure_fused_kernel();
   if (e == cudaSuccess) e = pix::configure_findrun_kernel();
   if (e == cudaSuccess) e = pix::configure_finalize_kernel();
   if (e == cudaSuccess) e = pix::configure_overflow_kernel();

@@ -1,5 +1,5 @@
 // cluster.cu -- the overflow kernel: a4 findClus fused with a5 (cluster sums, charge cut, renumber, temp records)
-// for the module runs the warp kernels (findclus.cu, findrun.cu) could not take: runs longer than 512 words, dense
+// for the module runs the warp kernels (fused.cu, findrun.cu) could not take: runs longer than 512 words, dense
 // runs that overflow a hash bucket neighbourhood, charge sums beyond 32 bits.  One block per run, tables in the global workspace, 64-bit sums.
 //
 // "clusters the pixels on each detector module".  The connectivity rule, the duplicate rule,
@@ -19,13 +19,14 @@
 //   6  per digi: final status and clus; per task: counts
 // The digi fields (row, col, charge) are read back from the output arrays the decode kernel has written.
 #include "pix_common.cuh"
+#include "pix_device.cuh"
 
 namespace pix {
 
 namespace {
 
 constexpr uint32_t LIVE = 0x80000000u, KEYMASK = 0x0001FFFFu, NOPOS = 0xFFFFFFFFu;
-constexpr uint32_t HASH_MUL = 0x9E3779B1u;
+constexpr uint32_t HASH_MUL = 0x9E3779B1u;  // linear-probing table of 2n slots (sized per run, unlike the bucket hash)
 
 // ------------------------------------------------------------------ hash slots
 template <typename SlotT> struct SlotOps;
@@ -72,17 +73,7 @@ __device__ __forceinline__ uint32_t hash_find(const SlotT* tab, uint32_t size, u
   }
 }
 
-// ------------------------------------------------------------------ unions (labels strictly decrease along parents)
-// hook-and-descend (see findclus.cu): one atomicMin per step, no root searches
-__device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
-  bool done = a == b;
-  while (!done) {
-    const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
-    const uint32_t p = atomicMin(L + hi, lo);
-    if (p == hi || p == lo) done = true;
-    else { a = p; b = lo; }
-  }
-}
+// ------------------------------------------------------------------ unions: hook() of pix_device.cuh
 // read-only walk to the root (step 4: own entries are being flattened concurrently, nobody else's may be written)
 __device__ __forceinline__ uint32_t uf_root(const volatile uint32_t* L, uint32_t x) {
   uint32_t p = L[x];
@@ -225,7 +216,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     if (root) {
       if (surv) {
         const uint32_t o = rb + id;
-        put_temp(c.t_rec + o, first + k, T.npix[k], Q, (float)((double)T.sx[k] / (double)Q),
+        put_temp(c, o, first + k, T.npix[k], Q, (float)((double)T.sx[k] / (double)Q),
                  (float)((double)T.sy[k] / (double)Q));
       }
       T.q[k] = surv ? id : NO_INDEX;
@@ -287,7 +278,7 @@ __global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_cons
   __shared__ uint32_t s_task;
   const BlockGroup<OVF_THREADS> g{s_scan};
   uint32_t count = c.ctl[CTL_OVF_COUNT];
-  count = count < c.ovf_cap ? count : c.ovf_cap;
+  count = count < c.list_cap ? count : c.list_cap;
   while (true) {
     __syncthreads();
     if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + CTL_OVF_TICKET, 1u);

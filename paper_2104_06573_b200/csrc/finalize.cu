@@ -61,10 +61,24 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
   const uint32_t ebase = c.segB[er * c.F];
   const uint32_t n_words = c.segB[(er + 1u) * c.F] - ebase;
 
+  // ---- an event whose modules are not contiguous is not clustered (S11): every decodable word is BELOW_THRESHOLD or
+  // CUT with clus = -1, whatever the cluster kernels did or did not do with its runs
+  uint32_t fix_below = 0u, fix_cut = 0u;
+  if (skip) {
+    for (uint32_t i = tid; i < n_words; i += FIN_THREADS) {
+      const size_t g = (size_t)ebase + i;
+      c.d_clus[g] = -1;
+      if (c.d_row[g] != 0xFFFFu) {
+        const bool below = c.d_charge[g] < c.thr;
+        c.d_status[g] = below ? ST_BELOW : ST_CUT;
+        fix_below += below ? 1u : 0u; fix_cut += below ? 0u : 1u;
+      }
+    }
+  }
   // ---- offsets + summary + work items
   uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
   for (uint32_t m = tid; m <= M; m += FIN_THREADS) cms[m] = s_start[m];
-  uint32_t acc[2] = {0, 0};  // modules present, clusters surviving the cut
+  uint32_t acc[4] = {0, 0, fix_below, fix_cut};  // modules present, clusters surviving the cut, S11 counts
   for (uint32_t m = tid; m < M; m += FIN_THREADS) {
     const bool present = c.module_end[(size_t)e * M + m] > 0u;
     if (!present) c.module_first[(size_t)e * M + m] = 0u;  // S12: absent -> 0,0 (init left the atomicMin sentinel)
@@ -72,7 +86,7 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
     acc[1] += skip ? 0u : n_clus[m];
   }
 #pragma unroll
-  for (int k = 0; k < 2; ++k) {
+  for (int k = 0; k < 4; ++k) {
     const uint32_t v = __reduce_add_sync(0xFFFFFFFFu, acc[k]);
     if (lane == 0 && v) atomicAdd(s_red + k, v);
   }
@@ -83,18 +97,15 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
     const uint32_t bad = ec[EC_EMPTY] + ec[EC_ERR_LINK] + ec[EC_ERR_ROC] + ec[EC_ERR_DCOL] + ec[EC_ERR_PXID];
     s[0] = n_words; s[1] = n_words - bad; s[2] = ec[EC_EMPTY];
     s[3] = ec[EC_ERR_LINK]; s[4] = ec[EC_ERR_ROC]; s[5] = ec[EC_ERR_DCOL]; s[6] = ec[EC_ERR_PXID];
-    s[7] = ec[EC_DUP]; s[8] = ec[EC_BELOW]; s[9] = ec[EC_OK]; s[10] = ec[EC_CUT];
-    s[11] = s_red[0]; s[12] = ec[EC_PRECUT]; s[13] = s_red[1]; s[14] = n_emit;
+    s[7] = skip ? 0u : ec[EC_DUP]; s[8] = skip ? s_red[2] : ec[EC_BELOW]; s[9] = skip ? 0u : ec[EC_OK];
+    s[10] = skip ? s_red[3] : ec[EC_CUT];
+    s[11] = s_red[0]; s[12] = skip ? 0u : ec[EC_PRECUT]; s[13] = s_red[1]; s[14] = n_emit;
     s[15] = flags | (total > c.cap_ev ? FLAG_CAPACITY : 0u);
     const uint32_t nsl = (n_emit + SLICE - 1u) / SLICE;
     if (nsl) {
       const uint32_t at = atomicAdd(c.ctl + CTL_SLICE_COUNT, nsl);
       for (uint32_t q = 0; q < nsl; ++q) c.slice_list[at + q] = (er << 16) | q;  // cap_ev <= 2^26 records (pix_create)
     }
-  }
-  // ---- an event whose modules are not contiguous was not clustered: define clus for its decodable words
-  if (skip) {
-    for (uint32_t i = tid; i < n_words; i += FIN_THREADS) c.d_clus[(size_t)ebase + i] = -1;
   }
 }
 
@@ -126,8 +137,8 @@ __global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_const
       const uint32_t src = rel + mfirst[lo] + (g - s_start[lo]);
       const size_t o = (size_t)e * c.cap_ev + g;
       c.c_module[o] = (uint16_t)lo;
-      const uint4 a = c.t_rec[src].a;
-      const float y = c.t_rec[src].y;
+      const uint4 a = c.t_a[src];
+      const float y = c.t_y[src];
       c.c_first[o] = a.x; c.c_npix[o] = a.y; c.c_charge[o] = a.z; c.c_x[o] = __uint_as_float(a.w); c.c_y[o] = y;
     }
   }

@@ -1,5 +1,5 @@
 // findrun.cu -- the warp-per-run cluster kernel: a4 findClus (S10, S13) and a5 sums / charge cut /
-// renumber / temp records (S9, S14, S18) for the module runs the chunk kernel (findclus.cu) could not take
+// renumber / temp records (S9, S14, S18) for the module runs the fused kernel (fused.cu) could not take
 // because they do not fit its 256-word window ("clusters the pixels on each detector module").
 //
 // One warp per run, in two sizes: up to 512 words (15 KB of per-warp shared memory) and up to 1024 words (29 KB);
@@ -9,6 +9,7 @@
 // Longer runs, runs whose hash bucket neighbourhood overflows and charge sums beyond 32 bits go on to the block
 // kernel (cluster.cu).  Nothing here is shared with oracle/.
 #include "pix_common.cuh"
+#include "pix_device.cuh"
 
 namespace pix {
 
@@ -18,14 +19,13 @@ constexpr uint32_t RECAP = 256;           // edge list entries
 constexpr uint32_t EMPTY = 0xFFFFFFFFu, INVALID = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;
-constexpr uint32_t HASH_MUL = 0x9E3779B1u;
-constexpr uint32_t KEY_BITS = 17, KEY_MASK = (1u << KEY_BITS) - 1u, MAX_DISP = 3;
 // Two sizes of the kernel: RM = 512 words per run (15 KB of shared memory per warp, 2 warps per block) and
-// RM = 1024 (29 KB, 1 warp per block).  Hash: RM buckets of 4 slots; key: row (8) | col (9);
+// RM = 1024 (29 KB, 1 warp per block).  Hash (pix_device.cuh): RM buckets of 4 slots; key: row (8) | col (9);
 // slot: disp (2) | tag (17 - log2 RM) | digi (10) | below (1).
 template <uint32_t RM> struct RK {
   static_assert(RM == 512 || RM == 1024, "run sizes");
-  static constexpr uint32_t RTAB = 4 * RM, NBUCKET = RM, TAG_BITS = RM == 512 ? 8 : 7, TAG_MASK = (1u << RK<RM>::TAG_BITS) - 1u;
+  using PH = BucketHash<17, RM == 512 ? 9 : 10, 10>;
+  static constexpr uint32_t RTAB = 4 * RM;
   static constexpr int WPB = RM == 512 ? 2 : 1;
 };
 
@@ -39,61 +39,6 @@ struct __align__(16) RunSmem {
   uint16_t rlist[RM];   // roots in digi order
 };
 
-__device__ __forceinline__ uint32_t hmix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
-// 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets
-template <uint32_t RM>
-__device__ __forceinline__ uint32_t hinsert(RunSmem<RM>& s, uint32_t key, uint32_t t, uint32_t below) {
-  const uint32_t h = hmix(key), tag = h & RK<RM>::TAG_MASK;
-  uint32_t p = (h >> RK<RM>::TAG_BITS) * 4u, res = 2u;
-#pragma unroll 1
-  for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u) && res == 2u; ++i, p = (p + 1u) & (RK<RM>::RTAB - 1u)) {
-    const uint32_t want = ((i >> 2) << RK<RM>::TAG_BITS) | tag, mine = (want << 11) | (t << 1) | below;
-    const uint32_t old = atomicCAS(&s.tab[p], EMPTY, mine);
-    if (old == EMPTY) res = 0u;
-    else if ((old >> 11) == want) { atomicMin(&s.tab[p], mine); res = 1u; }  // same pixel: the lowest digi owns it
-  }
-  return res;
-}
-__device__ __forceinline__ uint32_t half_match(const uint4& e, uint32_t want) {
-  uint32_t r = EMPTY;
-  if ((e.w >> 11) == want) r = e.w;
-  if ((e.z >> 11) == want) r = e.z;
-  if ((e.y >> 11) == want) r = e.y;
-  if ((e.x >> 11) == want) r = e.x;
-  return r;
-}
-template <uint32_t RM>
-__device__ __noinline__ uint32_t hfind_slow(const RunSmem<RM>& s, uint32_t h) {
-  const uint32_t tag = h & RK<RM>::TAG_MASK;
-  uint32_t b = h >> RK<RM>::TAG_BITS, r = EMPTY;
-  for (uint32_t i = 1; i <= MAX_DISP && r == EMPTY; ++i) {
-    b = (b + 1u) & (RK<RM>::NBUCKET - 1u);
-    const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[b * 4u]);
-    r = half_match(e, (i << RK<RM>::TAG_BITS) | tag);
-    if (e.w == EMPTY) break;
-  }
-  return r;
-}
-template <uint32_t RM>
-__device__ __forceinline__ uint32_t hfind(const RunSmem<RM>& s, uint32_t h) {
-  const uint4 e = *reinterpret_cast<const uint4*>(&s.tab[(h >> RK<RM>::TAG_BITS) * 4u]);
-  uint32_t r = half_match(e, h & RK<RM>::TAG_MASK);
-  if (r == EMPTY && e.w != EMPTY) r = hfind_slow<RM>(s, h);
-  return r;
-}
-__device__ __forceinline__ uint32_t slot_digi(uint32_t e) { return (e >> 1) & 0x3FFu; }
-__device__ __forceinline__ bool slot_live(uint32_t e) { return e != EMPTY && !(e & 1u); }
-
-// hook-and-descend union (see findclus.cu): one atomicMin per step, no root searches
-__device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
-  bool done = a == b;  // single exit: the lanes of a warp reconverge after the loop
-  while (!done) {
-    const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
-    const uint32_t p = atomicMin(L + hi, lo);
-    if (p == hi || p == lo) done = true;
-    else { a = p; b = lo; }
-  }
-}
 template <uint32_t RM>
 __device__ __forceinline__ void unite_edges(RunSmem<RM>& s, uint32_t ne, uint32_t lane) {
   for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count
@@ -104,11 +49,6 @@ __device__ __forceinline__ void unite_edges(RunSmem<RM>& s, uint32_t ne, uint32_
     __syncwarp();
   }
 }
-__device__ __forceinline__ void push_block(const Chunk& c, uint32_t task) {
-  const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u);
-  if (i < c.ovf_cap) c.ovf_list[i] = task;
-}
-
 template <uint32_t RM>
 __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_constant__ Chunk c, const uint32_t* __restrict__ in_list, uint32_t ctl_count,
                                                                    uint32_t ctl_ticket, uint32_t* __restrict__ long_list, uint32_t ctl_long) {
@@ -116,13 +56,14 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   RunSmem<RM>& s = reinterpret_cast<RunSmem<RM>*>(smem_raw)[warp];
   constexpr uint32_t RMAX = RM, RTAB = RK<RM>::RTAB;
+  using PH = typename RK<RM>::PH;
   const uint32_t lt_mask = (1u << lane) - 1u;
   constexpr uint32_t FULL = 0xFFFFFFFFu, NO_ID = 0xFFFFu;
   uint32_t* const q = s.tab; uint32_t* const np = s.tab + RMAX; uint32_t* const sx = s.tab + 2 * RMAX;
   uint32_t* const sy = s.tab + 3 * RMAX;
   uint16_t* const lid = s.chg;
   uint32_t count = c.ctl[ctl_count];
-  count = count < c.ovf_cap ? count : c.ovf_cap;
+  count = count < c.list_cap ? count : c.list_cap;
   const uint32_t gBeg = c.segB[0];
 
   while (true) {
@@ -138,7 +79,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
     if (n > RMAX) {  // too long for this size of the kernel: the next one takes it
       if (lane == 0) {
         const uint32_t i = atomicAdd(c.ctl + ctl_long, 1u);
-        if (i < c.ovf_cap) long_list[i] = task;
+        if (i < c.list_cap) long_list[i] = task;  // a task moves down the lists at most once: they never overflow
       }
       continue;
     }
@@ -165,20 +106,20 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
       s.label[t] = (dec && !below) ? t : MARK_BELOW;
       s.chg[t] = (uint16_t)e;
       if (dec) {
-        const uint32_t ins = hinsert(s, dk, t, below ? 1u : 0u);
+        const uint32_t ins = PH::insert(s.tab, dk, t, below ? 1u : 0u);
         dup_seen |= ins == 1u; full_seen |= ins == 2u;
       }
     }
     __syncwarp();
     if (__any_sync(FULL, full_seen)) {  // no room near a home bucket (dense run): the block kernel takes it
-      if (lane == 0) push_block(c, task);
+      if (lane == 0) { const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u); if (i < c.list_cap) c.ovf_list[i] = task; }
       continue;
     }
     // ---- duplicates (S10): the digi that is not in the slot
     if (__any_sync(FULL, dup_seen)) {
       for (uint32_t k = 0; k < nk; ++k) {
         const uint32_t t = 32u * k + lane, key = s.dkey[t];
-        if (key != INVALID && slot_digi(hfind(s, hmix(key))) != t) s.label[t] = MARK_DUP;
+        if (key != INVALID && PH::digi(PH::find(s.tab, PH::mix(key))) != t) s.label[t] = MARK_DUP;
       }
       __syncwarp();
     }
@@ -196,13 +137,13 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
       bool f0 = false, f1 = false, f2 = false;
       uint32_t n0 = 0, n1 = 0, n2 = 0;
       if (live) {
-        const uint32_t h = hmix(key);
-        const uint32_t eE = hfind(s, (h + HASH_MUL) & KEY_MASK), eS = hfind(s, (h + 512u * HASH_MUL) & KEY_MASK);
-        const uint32_t eSW = hfind(s, (h + 511u * HASH_MUL) & KEY_MASK), eSE = hfind(s, (h + 513u * HASH_MUL) & KEY_MASK);
-        const bool hS = slot_live(eS);
-        f0 = slot_live(eE); n0 = slot_digi(eE);
-        f1 = hS || slot_live(eSW); n1 = slot_digi(hS ? eS : eSW);
-        f2 = !hS && !f0 && slot_live(eSE); n2 = slot_digi(eSE);  // with E live, SE is E's S: E joins it
+        const uint32_t h = PH::mix(key);
+        const uint32_t eE = PH::find(s.tab, PH::step(h, 1u)), eS = PH::find(s.tab, PH::step(h, 512u));
+        const uint32_t eSW = PH::find(s.tab, PH::step(h, 511u)), eSE = PH::find(s.tab, PH::step(h, 513u));
+        const bool hS = PH::live(eS);
+        f0 = PH::live(eE); n0 = PH::digi(eE);
+        f1 = hS || PH::live(eSW); n1 = PH::digi(hS ? eS : eSW);
+        f2 = !hS && !f0 && PH::live(eSE); n2 = PH::digi(eSE);  // with E live, SE is E's S: E joins it
       }
       const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
       if (f0) s.edge[ne + __popc(m0 & lt_mask)] = t | (n0 << 16);
@@ -267,7 +208,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
       if (valid) {
         if (surv) {
           const float fq = (float)Q;
-          put_temp(c.t_rec + ((gb - gBeg) + id), first + t, np[t], Q, __fdividef((float)sx[t], fq), __fdividef((float)sy[t], fq));
+          put_temp(c, (gb - gBeg) + id, first + t, np[t], Q, __fdividef((float)sx[t], fq), __fdividef((float)sy[t], fq));
         }
         lid[t] = surv ? (uint16_t)id : (uint16_t)NO_ID;
       }
@@ -275,7 +216,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
     }
     __syncwarp();
     if (__any_sync(FULL, wrapped)) {  // 32-bit weighted sums may have wrapped: the block kernel redoes the run
-      if (lane == 0) push_block(c, task);
+      if (lane == 0) { const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u); if (i < c.list_cap) c.ovf_list[i] = task; }
       continue;
     }
     // ---- final status and clus, counters

@@ -1,0 +1,514 @@
+// fused.cu -- the fused warp kernel of the Clusters path ("unpacks them, calibrates the individual
+// pixels, and clusters the pixels on each detector module"): a1 decode (S1-S6), a2 calibrate (S7-S9),
+// a3 module boundaries (S11, S12), a4 findClus (S10, S13) and a5 sums / charge cut / renumber / temp records
+// (S9, S14, S18) in one pass over the raw words.  SURVEY 8f NEXT-3.
+//
+// The word stream is cut into chunks of 128 words.  A warp takes a range of consecutive chunks (a ticket) and walks
+// it with a two-chunk ring in shared memory: while chunk i is clustered, chunk i+1 is already decoded (one word per
+// lane and round, four rounds), so
+//   - the "previous decodable word" that decides whether a word starts a module run is carried in registers from
+//     chunk to chunk (a look-back into memory happens once per range, bounded by the start of the event),
+//   - the look-ahead a window needs (a run belongs to the warp whose chunk holds its first word; the last run of a
+//     chunk may end in the next chunk) is the next chunk's own decode, done once,
+//   - per-event counters live in registers and are flushed when the range ends or the event changes.
+// Per window (the runs that start in chunk i, up to the first run start of chunk i+1; at most 256 slots):
+//   B  clear the position hash; give every digi its run, insert it keyed by (run, row, col); equal keys keep the
+//      lowest digi (S10)
+//   D  forward-neighbour lookups -> dense edge list -> unions (lock-free hook-and-descend, pix_device.cuh)
+//   E  every live digi adds charge | 1 << 24, charge*col, charge*row into its root's accumulators
+//   F  in slot order: roots with Q >= cut are numbered per run (ballot/popc), temp records written
+//   G  final status and clus of every word of the chunk (undecodable words included), counters
+// Warps never wait for each other (no block barrier); all tables are per-warp shared memory.  Runs that do not fit
+// the window, chunks with more than RC runs, hash buckets that overflow and charge sums that could overflow 32 bits go
+// to the warp-per-run kernel (findrun.cu).  Nothing here is shared with oracle/.
+#include "pix_common.cuh"
+#include "pix_device.cuh"
+
+namespace pix {
+
+namespace {
+
+constexpr int WPB = 4;                    // warps per block (they share nothing but the block)
+constexpr int FT = WPB * 32;
+constexpr int BLOCKS_PER_SM = 7;
+constexpr uint32_t HC = CHUNK_WORDS;      // words of a chunk (rounds 0-3 of a window)
+constexpr uint32_t MAXT = 256;            // window: home chunk + up to 4 rounds of the next chunk
+constexpr uint32_t RC = 62;               // runs a window can own
+constexpr uint32_t ECAP = 256;            // edge list; flushed (united) when a round might not fit
+constexpr uint32_t GMAX = 32;             // chunks per ticket, at most
+constexpr uint32_t NOKEY = 0xFFFFFFFFu, FULL = 0xFFFFFFFFu;
+constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
+constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
+constexpr uint32_t NO_ID = 0xFFFFu;
+using PH = BucketHash<23, 8, 8>;          // key: run (6 bits) | row (8) | col (9); 256 buckets of 4; digi = window slot
+constexpr uint32_t WTAB = PH::SLOTS;
+
+// Staged word (ring entry).  Decode writes pos | below; phase B adds the run and the start flag for the slots of the
+// window.  Neighbour keys are key+1 (col+1) and key+512-1, +512, +512+1 (row+1): col 416..511 and row 160..255 never
+// occur, so no bounds checks (S13).
+constexpr uint32_t SK_NONE = 0xFFFFFFFFu;   // no such word (outside the launch group)
+constexpr uint32_t SK_BAD = 0xFFFFFF00u;    // >= SK_BAD: undecodable word, status in the low byte
+constexpr uint32_t SK_POS = 0x1FFFFu;       // row << 9 | col
+constexpr uint32_t SK_RUN_SHIFT = 17, SK_KEY = 0x7FFFFFu;  // run in bits 17-22; hash key = sk & SK_KEY
+constexpr uint32_t SK_BELOW = 1u << 23, SK_START = 1u << 24;
+static_assert(RC + 1u < 64u && MAXT <= 256u && 3u * MAXT <= WTAB, "run field, slot field, sums fit the hash memory");
+
+struct __align__(16) WarpSmem {
+  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D: qn = tab, sx = tab + 256, sy = tab + 512
+  uint32_t label[MAXT];    // union-find parent of window slot t, or MARK_*
+  uint32_t skey[MAXT];     // ring of two chunks: staged words (lane-private: slot t belongs to lane t & 31)
+  uint16_t chg[MAXT];      // ring: charges
+  uint16_t edge[ECAP];     // a | b << 8; after the unions: local id of a root, or NO_ID
+  uint32_t run_ifirst[RC + 2];  // event-relative index of the run's first digi
+  uint32_t run_key[RC + 2];     // event_rel << 16 | module
+  uint16_t run_first[RC + 2];   // window slot of the run's first digi
+  uint16_t run_base[RC + 2];    // survivors before the run
+  uint8_t run_bad[RC + 2];      // the run is left to the warp-per-run kernel
+};
+static_assert(sizeof(WarpSmem) % 16 == 0, "per-warp slices stay 16-byte aligned");
+
+struct Dec {          // what the decode of a chunk leaves in registers for its turn as home chunk
+  uint32_t key[4];    // per lane: event_rel << 16 | module of its word in round j, NOKEY if undecodable
+  uint32_t sb[4];     // warp-uniform: run-start bits of round j
+  uint32_t ebase0;    // global index of word 0 of the event of the chunk's first word
+  uint32_t er0;       // that event
+  bool one_event;     // all 128 words exist and belong to event er0
+};
+
+__global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  WarpSmem& s = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
+  const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
+  const uint32_t* __restrict__ segB = c.segB;
+  const uint32_t gBeg = segB[0], gEnd = segB[S];
+  if (gBeg >= gEnd) return;
+  const uint32_t T0 = gBeg & ~(HC - 1u);
+  const uint32_t n_chunks = (gEnd - T0 + HC - 1u) / HC;
+  const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
+  uint32_t* const qn = s.tab; uint32_t* const sx = s.tab + MAXT; uint32_t* const sy = s.tab + 2 * MAXT;
+  uint16_t* const lid = s.edge;
+  uint32_t G = n_chunks / (gridDim.x * WPB * 4u);  // about four tickets per warp
+  G = G < 1u ? 1u : (G > GMAX ? GMAX : G);
+
+  // per-event counters of the digis this lane has finished: dup | below << 16, ok | cut << 16, roots
+  uint32_t acc_ev = NOKEY, accA = 0u, accB = 0u, accP = 0u;
+  auto flush = [&]() {
+    if (acc_ev != NOKEY) {
+      const uint32_t a = __reduce_add_sync(FULL, accA), bb = __reduce_add_sync(FULL, accB), p = __reduce_add_sync(FULL, accP);
+      if (lane == 0) {
+        uint32_t* ec = c.ev_cnt + (size_t)acc_ev * EC_STRIDE;
+        if (a & 0xFFFFu) atomicAdd(ec + EC_DUP, a & 0xFFFFu);
+        if (a >> 16) atomicAdd(ec + EC_BELOW, a >> 16);
+        if (bb & 0xFFFFu) atomicAdd(ec + EC_OK, bb & 0xFFFFu);
+        if (bb >> 16) atomicAdd(ec + EC_CUT, bb >> 16);
+        if (p) atomicAdd(ec + EC_PRECUT, p);
+      }
+    }
+    accA = accB = accP = 0u;
+  };
+
+  while (true) {
+    uint32_t ri = 0u;
+    if (lane == 0) ri = atomicAdd(c.ctl + CTL_RANGE_TICKET, 1u);
+    ri = __shfl_sync(FULL, ri, 0);
+    const uint32_t c0 = ri * G;
+    if (c0 >= n_chunks) break;
+    const uint32_t c1 = c0 + G < n_chunks ? c0 + G : n_chunks;
+
+    // ---- the last decodable word before the range, inside the event of the range's first word (an earlier event's
+    // word never continues a run; segfill_kernel closes every event's last run)
+    uint32_t carry_key = NOKEY, carry_g = 0u;
+    {
+      const uint32_t b = T0 + c0 * HC, gw = b < gBeg ? gBeg : b;
+      const uint32_t sg0 = c.chunk_seg[c0], er = div_F(c, sg0), evb = segB[er * F];
+      uint32_t g = gw;  // words [evb, g) are still to be searched, backwards
+      while (g > evb) {
+        const bool in = lane < g - evb;
+        const uint32_t gi = g - 1u - lane;
+        uint32_t key = NOKEY;
+        if (in) {
+          uint32_t sg = sg0;
+          while (segB[sg] > gi) --sg;
+          uint32_t m, r, cc;
+          if (decode_word(c.cab, __ldg(c.words + gi), (sg - er * F) << 11, m, r, cc) == ST_OK) key = (er << 16) | m;
+        }
+        const uint32_t bal = __ballot_sync(FULL, key != NOKEY);
+        if (bal) {
+          const int src = __ffs(bal) - 1;
+          carry_key = __shfl_sync(FULL, key, src);
+          carry_g = g - 1u - (uint32_t)src;
+          break;
+        }
+        g = (g - evb > 32u) ? g - 32u : evb;
+      }
+    }
+
+    Dec cur, nxt;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { cur.key[j] = NOKEY; cur.sb[j] = 0u; }
+    cur.ebase0 = 0u; cur.er0 = 0u; cur.one_event = false;
+
+    for (uint32_t ci = c0;; ++ci) {
+      const uint32_t hn = ((ci - c0) & 1u) * HC;  // ring half of chunk ci; chunk ci-1 sits in the other half
+      // ================================================================== decode chunk ci (a1, a2, a3)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { nxt.key[j] = NOKEY; nxt.sb[j] = 0u; }
+      nxt.ebase0 = 0u; nxt.er0 = 0u; nxt.one_event = false;
+      if (ci < n_chunks) {
+        const bool owner = ci < c1;  // else: the look-ahead of the range's last window, nothing is written
+        const uint32_t b = T0 + ci * HC;
+        const uint32_t sg0 = c.chunk_seg[ci];
+        const uint32_t er0 = div_F(c, sg0), fed0 = sg0 - er0 * F;
+        const uint32_t nextB0 = segB[sg0 + 1u], evend0 = segB[(er0 + 1u) * F];
+        const bool all_in = b >= gBeg && b + HC <= gEnd;
+        const bool one_seg = all_in && b + HC <= nextB0;
+        nxt.ebase0 = segB[er0 * F]; nxt.er0 = er0; nxt.one_event = all_in && b + HC <= evend0;
+        uint32_t w[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t g = b + 32u * j + lane;
+          w[j] = (all_in || (g >= gBeg && g < gEnd)) ? __ldg(c.words + g) : 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t g = b + 32u * j + lane;
+          const bool exists = all_in || (g >= gBeg && g < gEnd);
+          uint32_t er = er0, fed = fed0;
+          if (!one_seg && exists) {  // rare: a FED / event boundary inside the chunk
+            uint32_t sg = sg0;
+            while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
+            er = div_F(c, sg); fed = sg - er * F;
+          }
+          uint32_t m, row, col;
+          const uint32_t st = decode_word(c.cab, w[j], fed << 11, m, row, col);
+          const bool ok = exists && st == ST_OK;
+          int32_t e = 0;
+          if (ok) e = calibrate(c, w[j] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
+          const uint32_t sk = ok ? ((row << 9) | col | (e < c.thr ? SK_BELOW : 0u)) : (exists ? (SK_BAD | st) : SK_NONE);
+          s.skey[hn + 32u * j + lane] = sk;
+          s.chg[hn + 32u * j + lane] = (uint16_t)e;
+          if (owner && exists) {
+            c.d_module[g] = (uint16_t)(ok ? m : 0xFFFFu); c.d_row[g] = (uint16_t)(ok ? row : 0xFFFFu);
+            c.d_col[g] = (uint16_t)(ok ? col : 0xFFFFu); c.d_charge[g] = e;
+            if (!ok) atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
+          }
+          nxt.key[j] = ok ? ((er << 16) | m) : NOKEY;
+        }
+        // a3: a word starts a run when its (event, module) differs from the previous decodable word's
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const bool valid = nxt.key[j] != NOKEY;
+          const uint32_t has = __ballot_sync(FULL, valid);
+          const uint32_t below_l = has & lt_mask;
+          const int src = below_l ? 31 - __clz(below_l) : 0;
+          uint32_t pkey = __shfl_sync(FULL, nxt.key[j], src), pg = b + 32u * j + (uint32_t)src;
+          if (!below_l) { pkey = carry_key; pg = carry_g; }
+          const bool start = valid && nxt.key[j] != pkey;
+          nxt.sb[j] = __ballot_sync(FULL, start);
+          if (owner && start) {
+            run_start(c, nxt.key[j], b + 32u * j + lane);
+            if (pkey != NOKEY) run_end(c, pkey, pg);
+          }
+          if (has) {
+            const int top = 31 - __clz(has);
+            carry_key = __shfl_sync(FULL, nxt.key[j], top); carry_g = b + 32u * j + (uint32_t)top;
+          }
+        }
+      }
+
+      // ================================================================== cluster the window of chunk ci - 1
+      if (ci > c0) {
+        const uint32_t hb = hn ^ HC;                 // ring half of the home chunk
+        const uint32_t b = T0 + (ci - 1u) * HC;      // global index of window slot 0
+        uint32_t rb[4];                              // runs started before round k
+        uint32_t R = 0u;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { rb[k] = R; R += __popc(cur.sb[k]); }
+        uint32_t f_t = MAXT, e_t = 0u;               // window = slots [f_t, e_t); empty when nothing is owned
+        uint32_t Rown = R;                           // runs of the window (the last run may be left to findrun)
+        if (R) {
+          const uint32_t kf = cur.sb[0] ? 0u : (cur.sb[1] ? 1u : (cur.sb[2] ? 2u : 3u));
+          f_t = 32u * kf + (uint32_t)__ffs(kf == 0u ? cur.sb[0] : (kf == 1u ? cur.sb[1] : (kf == 2u ? cur.sb[2] : cur.sb[3]))) - 1u;
+          // end of the last run: the first run start of the next chunk, the end of the data, or "does not fit"
+          if (nxt.sb[0] | nxt.sb[1] | nxt.sb[2] | nxt.sb[3]) {
+            const uint32_t ke = nxt.sb[0] ? 0u : (nxt.sb[1] ? 1u : (nxt.sb[2] ? 2u : 3u));
+            e_t = HC + 32u * ke + (uint32_t)__ffs(ke == 0u ? nxt.sb[0] : (ke == 1u ? nxt.sb[1] : (ke == 2u ? nxt.sb[2] : nxt.sb[3]))) - 1u;
+          } else if (b + MAXT >= gEnd) {
+            e_t = gEnd - b;
+          } else {  // the last run does not end inside the next chunk: the warp-per-run kernel takes it
+            const uint32_t kz = cur.sb[3] ? 3u : (cur.sb[2] ? 2u : (cur.sb[1] ? 1u : 0u));
+            const uint32_t sbz = kz == 3u ? cur.sb[3] : (kz == 2u ? cur.sb[2] : (kz == 1u ? cur.sb[1] : cur.sb[0]));
+            const uint32_t lz = 31u - (uint32_t)__clz(sbz);
+            e_t = 32u * kz + lz;
+            uint32_t keyz = kz == 3u ? cur.key[3] : (kz == 2u ? cur.key[2] : (kz == 1u ? cur.key[1] : cur.key[0]));
+            if (lane == lz) push_run(c, c.mid_list, CTL_MID_COUNT, keyz >> 16, keyz & 0xFFFFu);
+            Rown = R - 1u;
+            if (e_t == f_t) { f_t = MAXT; e_t = 0u; }  // it was the only run
+          }
+        }
+        const bool owns = e_t > f_t;
+        if (owns) {
+          // ============================================================== B: clear; runs; insert
+          {
+            uint4* t4 = reinterpret_cast<uint4*>(s.tab);
+            const uint4 e4 = make_uint4(PH::EMPTY, PH::EMPTY, PH::EMPTY, PH::EMPTY);
+#pragma unroll
+            for (int k = 0; k < (int)(WTAB / 4 / 32); ++k) t4[lane + 32 * k] = e4;
+            if (lane < (RC + 2u) / 4u) reinterpret_cast<uint32_t*>(s.run_bad)[lane] = 0u;
+          }
+          __syncwarp();  // the cleared hash is visible
+          if (Rown > RC && lane == 0) s.run_bad[RC + 1u] = 1;  // the runs beyond RC are all "run 63"
+          bool dup_seen = false;
+          const uint32_t k0 = f_t >> 5, kl = (e_t + 31u) >> 5;  // rounds k0 .. kl-1 hold the window
+#pragma unroll
+          for (uint32_t k = 0; k < 4; ++k) {
+            if (k < k0 || k >= kl) continue;  // warp-uniform
+            const uint32_t t = 32u * k + lane;
+            const uint32_t sk = s.skey[hb + t];
+            const bool start = (cur.sb[k] >> lane) & 1u;
+            const uint32_t r = rb[k] + __popc(cur.sb[k] & le_mask);
+            const bool inw = t >= f_t && t < e_t;
+            const bool dec = inw && sk < SK_BAD;
+            if (start && inw) {
+              const uint32_t key = cur.key[k];
+              if (r <= RC) {
+                s.run_first[r] = (uint16_t)t; s.run_key[r] = key;
+                s.run_ifirst[r] = b + t - (cur.one_event ? cur.ebase0 : segB[(key >> 16) * F]);
+              } else {
+                push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);  // too many runs: left to findrun
+              }
+            }
+            const uint32_t rr = r <= RC ? r : RC + 1u;
+            const uint32_t nsk = (sk & (SK_POS | SK_BELOW)) | (rr << SK_RUN_SHIFT) | (start ? SK_START : 0u);
+            const bool live = dec && !(sk & SK_BELOW) && r <= RC;
+            if (dec) s.skey[hb + t] = nsk;
+            s.label[t] = live ? t : MARK_BELOW;
+            if (dec && r <= RC) {
+              const uint32_t ins = PH::insert(s.tab, nsk & SK_KEY, t, (sk & SK_BELOW) ? 1u : 0u);
+              dup_seen |= ins == 1u;
+              if (ins == 2u) s.run_bad[r] = 1;  // no room near the home bucket: findrun takes the run
+            }
+          }
+          {
+            const uint32_t rr = R <= RC ? R : RC + 1u;
+#pragma unroll 1
+            for (uint32_t k = 4; k < kl; ++k) {  // the head of the next chunk: the rest of run R
+              const uint32_t t = 32u * k + lane;
+              const uint32_t sk = s.skey[hn + t - HC];
+              const bool dec = t < e_t && sk < SK_BAD;
+              const uint32_t nsk = (sk & (SK_POS | SK_BELOW)) | (rr << SK_RUN_SHIFT);
+              const bool live = dec && !(sk & SK_BELOW) && R <= RC;
+              if (dec) s.skey[hn + t - HC] = nsk;
+              s.label[t] = live ? t : MARK_BELOW;
+              if (dec && R <= RC) {
+                const uint32_t ins = PH::insert(s.tab, nsk & SK_KEY, t, (sk & SK_BELOW) ? 1u : 0u);
+                dup_seen |= ins == 1u;
+                if (ins == 2u) s.run_bad[R] = 1;
+              }
+            }
+          }
+          __syncwarp();  // hash, labels, run tables complete
+          const uint32_t Rw = Rown < RC ? Rown : RC;  // runs of this window that are numbered here
+
+          // ============================================================== D: duplicates; neighbours -> edges -> unions
+          if (__any_sync(FULL, dup_seen)) {  // rare: some pixel appears twice; the digi not in the slot is a DUPLICATE (S10)
+            for (uint32_t k = k0; k < kl; ++k) {
+              const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
+              const bool dec = t >= f_t && t < e_t && sk < SK_BAD && ((sk >> SK_RUN_SHIFT) & 63u) <= RC;
+              if (dec && PH::digi(PH::find(s.tab, PH::mix(sk & SK_KEY))) != t) s.label[t] = MARK_DUP;
+            }
+            __syncwarp();
+          }
+          // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE
+          // are joined to it by their own E edges, so d-S alone is enough; when E is live, SE is E's S neighbour.
+          uint32_t ne = 0u;
+#pragma unroll 1
+          for (uint32_t k = k0; k < kl; ++k) {
+            const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
+            if (ne + 96u > ECAP) {  // the round's edges might not fit: unite what is listed (warp-uniform)
+              __syncwarp();
+              for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
+                if (i0 + lane < ne) {
+                  const uint32_t e = s.edge[i0 + lane];
+                  hook(s.label, e & 0xFFu, e >> 8);
+                }
+                __syncwarp();
+              }
+              ne = 0u;
+            }
+            const bool live = t >= f_t && t < e_t && sk < SK_BAD && s.label[t] < MAXT;
+            bool f0 = false, f1 = false, f2 = false;
+            uint32_t n0 = 0, n1 = 0, n2 = 0;
+            if (live) {
+              const uint32_t h = PH::mix(sk & SK_KEY);
+              const uint32_t eE = PH::find(s.tab, PH::step(h, 1u)), eS = PH::find(s.tab, PH::step(h, 512u));
+              const uint32_t eSW = PH::find(s.tab, PH::step(h, 511u)), eSE = PH::find(s.tab, PH::step(h, 513u));
+              const bool hS = PH::live(eS);
+              f0 = PH::live(eE); n0 = PH::digi(eE);
+              f1 = hS || PH::live(eSW); n1 = PH::digi(hS ? eS : eSW);
+              f2 = !hS && !f0 && PH::live(eSE); n2 = PH::digi(eSE);  // with E live, SE is E's S: E joins it
+            }
+            const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
+            if (f0) s.edge[ne + __popc(m0 & lt_mask)] = (uint16_t)(t | (n0 << 8));
+            ne += __popc(m0);
+            if (f1) s.edge[ne + __popc(m1 & lt_mask)] = (uint16_t)(t | (n1 << 8));
+            ne += __popc(m1);
+            if (f2) s.edge[ne + __popc(m2 & lt_mask)] = (uint16_t)(t | (n2 << 8));
+            ne += __popc(m2);
+          }
+          __syncwarp();
+          for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
+            if (i0 + lane < ne) {
+              const uint32_t e = s.edge[i0 + lane];
+              hook(s.label, e & 0xFFu, e >> 8);
+            }
+            __syncwarp();
+          }
+#pragma unroll 1
+          for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: the chains shrink 4x before the sums
+            for (uint32_t k = k0; k < kl; ++k) {
+              const uint32_t t = 32u * k + lane;
+              const uint32_t l = s.label[t];
+              if (l < MAXT) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
+            }
+            __syncwarp();
+          }
+
+          // ============================================================== E: cluster sums (the hash is dead: qn / sx / sy)
+          {
+            uint4* t4 = reinterpret_cast<uint4*>(s.tab);
+            const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+            for (int k = 0; k < (int)(3 * MAXT / 4 / 32); ++k) t4[lane + 32 * k] = z4;
+          }
+          __syncwarp();
+#pragma unroll 1
+          for (uint32_t k = k0; k < kl; ++k) {
+            const uint32_t t = 32u * k + lane;
+            volatile uint32_t* L = s.label;
+            uint32_t r = L[t];
+            if (r < MAXT) {  // live (else MARK_*); labels outside the window are never read: k0 <= k < kl and MARK_BELOW there
+              while (true) { const uint32_t n = L[r]; if (n == r) break; r = n; }
+              L[t] = r;  // flatten: r is the root, so other walkers through t stay correct
+              const uint32_t ph = (hb + t) & (MAXT - 1u);
+              const uint32_t sk = s.skey[ph], e = s.chg[ph];
+              atomicAdd(&qn[r], e | (1u << 24));  // charge sum (< 2^24: 256 * 65535) | pixel count (256 wraps to 0)
+              atomicAdd(&sx[r], e * (sk & 511u));
+              atomicAdd(&sy[r], e * ((sk >> 9) & 255u));
+            }
+          }
+          __syncwarp();
+
+          // ============================================================== F: cut, renumber, temp records, in slot order
+          {
+            uint32_t cnt = 0u;               // surviving roots before this round
+            uint32_t base_c = 0u, rf_c = 0u; // of the run that is open when the round starts: survivors before it, its first slot
+            const uint32_t relb = b - gBeg;  // may wrap for the first chunk; only used added to a slot >= gBeg - b
+#pragma unroll 1
+            for (uint32_t k = k0; k < kl; ++k) {
+              const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
+              const bool dec = t >= f_t && t < e_t && sk < SK_BAD;
+              const uint32_t r = (sk >> SK_RUN_SHIFT) & 63u;
+              const bool root = dec && s.label[t] == t;
+              uint32_t Q = 0u, np = 0u;
+              if (root) {
+                const uint32_t v = qn[t];
+                Q = v & 0xFFFFFFu; np = v >> 24;
+                if (np == 0u) np = 256u;
+                if (Q > Q_SAFE) s.run_bad[r] = 1;  // 32-bit weighted sums may have wrapped
+              }
+              const bool surv = root && (int32_t)Q >= c.cut;  // S9: equality keeps
+              const uint32_t sm = __ballot_sync(FULL, surv);
+              const uint32_t rank = cnt + __popc(sm & lt_mask);
+              const bool isstart = dec && (sk & SK_START);
+              const uint32_t stm = __ballot_sync(FULL, isstart);
+              const uint32_t mine = stm & le_mask;
+              const int sl = mine ? 31 - __clz(mine) : 0;
+              uint32_t base = __shfl_sync(FULL, rank, sl), rf = 32u * k + (uint32_t)sl;
+              if (!mine) { base = base_c; rf = rf_c; }
+              if (isstart) s.run_base[r] = (uint16_t)rank;  // survivors before the run
+              if (root) {
+                uint32_t id = NO_ID;
+                if (surv) {
+                  id = rank - base;
+                  // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
+                  const float fq = (float)Q;
+                  put_temp(c, relb + rf + id, s.run_ifirst[r] + (t - rf), np, Q, __fdividef((float)sx[t], fq),
+                           __fdividef((float)sy[t], fq));
+                }
+                lid[t] = (uint16_t)id;
+              }
+              if (stm) {
+                const int top = 31 - __clz(stm);
+                base_c = __shfl_sync(FULL, rank, top); rf_c = 32u * k + (uint32_t)top;
+              }
+              cnt += __popc(sm);
+            }
+            if (lane == 0) s.run_base[Rw + 1u] = (uint16_t)cnt;
+          }
+          __syncwarp();  // run_base, run_bad, local ids final
+          for (uint32_t r = 1u + lane; r <= Rw; r += 32u) {
+            const uint32_t key = s.run_key[r];
+            if (s.run_bad[r]) push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);
+            else c.n_clus[(key >> 16) * c.M + (key & 0xFFFFu)] = (uint32_t)s.run_base[r + 1u] - s.run_base[r];
+          }
+        }
+
+        // ================================================================== G: final status and clus, counters
+        {
+          const uint32_t kl = owns ? (e_t + 31u) >> 5 : 0u;
+          const uint32_t kg = kl > 4u ? kl : 4u;
+          uint32_t cntA = 0u, cntB = 0u, n_pre = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
+#pragma unroll 1
+          for (uint32_t k = 0; k < kg; ++k) {
+            const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
+            if (sk >= SK_BAD) {
+              if (k < 4u && sk != SK_NONE) { c.d_status[b + t] = (uint8_t)(sk & 0xFFu); c.d_clus[b + t] = -1; }  // undecodable: finished here
+            } else if (t >= f_t && t < e_t && !s.run_bad[(sk >> SK_RUN_SHIFT) & 63u]) {
+              const uint32_t lab = s.label[t];
+              uint32_t so; int32_t cl = -1;
+              if (lab == MARK_DUP) { so = ST_DUP; cntA += 1u; }
+              else if (lab == MARK_BELOW) { so = ST_BELOW; cntA += 0x10000u; }
+              else {
+                const uint32_t id = lid[lab];
+                if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
+                n_pre += lab == t ? 1u : 0u;
+              }
+              c.d_status[b + t] = (uint8_t)so; c.d_clus[b + t] = cl;
+              if (!cur.one_event) {  // rare: an event boundary inside the chunk; every digi counts for its own event
+                uint32_t* ec = c.ev_cnt + (size_t)(s.run_key[(sk >> SK_RUN_SHIFT) & 63u] >> 16) * EC_STRIDE;
+                atomicAdd(ec + (so == ST_DUP ? EC_DUP : (so == ST_BELOW ? EC_BELOW : (so == ST_OK ? EC_OK : EC_CUT))), 1u);
+                if (lab == t) atomicAdd(ec + EC_PRECUT, 1u);
+              }
+            }
+          }
+          if (cur.one_event) {
+            if (cur.er0 != acc_ev) { flush(); acc_ev = cur.er0; }
+            accA += cntA; accB += cntB; accP += n_pre;
+          }
+        }
+        __syncwarp();  // shared state is rewritten by the next window
+      }
+      if (ci >= c1) break;
+      cur = nxt;
+    }
+    flush();
+    acc_ev = NOKEY;
+  }
+}
+
+}  // namespace
+
+cudaError_t configure_fused_kernel() {
+  return cudaFuncSetAttribute(fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WPB * sizeof(WarpSmem)));
+}
+
+void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
+  uint64_t nb = ((uint64_t)words_bound + 2 * HC + WPB * HC - 1) / (WPB * HC);
+  if (nb < 1) nb = 1;
+  if (nb > (uint64_t)n_sm * BLOCKS_PER_SM) nb = (uint64_t)n_sm * BLOCKS_PER_SM;
+  fused_kernel<<<(int)nb, FT, WPB * sizeof(WarpSmem), stream>>>(c);
+}
+
+}  // namespace pix

@@ -5,11 +5,11 @@
 // (lines 76-81).  Readings S1..S24 of DESIGN.md fix what the paper leaves open.
 //
 // Kernel chain for one chunk of events:
-//   init      -> segment table, range sentinels, zeroed counters; segfill -> segment of every 128-word chunk
-//   decode    -> a1 decode + a2 calibrate + a3 run boundaries, streaming, 4 words per thread; one start bit per word
-//   findclus  -> a4 findClus + a5 sums/cut/renumber for every module run that fits a warp's 256-word window
-//                (home chunk of 128 words + look-ahead)
-//   findrun   -> a4 + a5 for runs that do not fit a findclus window: one warp per run, two sizes (512 / 1024 words)
+//   init      -> segment table, range sentinels, zeroed counters; segfill -> segment of every 128-word chunk,
+//                end of every event's last run
+//   fused     -> a1 decode + a2 calibrate + a3 run boundaries + a4 findClus + a5 sums/cut/renumber for every module
+//                run that fits a warp's 256-word window (home chunk of 128 words + the head of the next chunk)
+//   findrun   -> a4 + a5 for runs that do not fit a window: one warp per run, two sizes (512 / 1024 words)
 //   overflow  -> a4 + a5 for the runs neither could take (longer than the window, pathological
 //                charge sums): generic block-per-run kernel, tables in global workspace
 //   offsets   -> a6 clamp + prefix scan (Fig. 3), summary, scatter work list
@@ -35,9 +35,9 @@ constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus;
 
 // per-event counters (integer atomics only), one row of EC_STRIDE per event of the chunk
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
-       EC_PRECUT, EC_STRIDE = 16 };
+       EC_PRECUT, EC_PUSHED /* runs the event has put on the task lists (at most M) */, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_WORDS = 16 };
 
 // Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
 //   x = module | bad << 16 | scol << 24     bad: 0, ST_ERR_LINK or ST_ERR_ROC; scol = +1 / -1 (int8)
@@ -45,11 +45,6 @@ enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT
 // so that row = row0 + srow * (pxid >> 1), col = col0 + scol * (2*dcol + (pxid & 1)).
 typedef uint2 CabEntry;
 
-// temp cluster record (one 128-bit store + one 32-bit store; 32-byte stride)
-struct __align__(16) TempRec { uint4 a; float y; uint32_t pad[3]; };  // a = first_digi, n_pix, charge, x_col bits
-__device__ __forceinline__ void put_temp(TempRec* r, uint32_t first, uint32_t npix, uint32_t charge, float x, float y) {
-  r->a = make_uint4(first, npix, charge, __float_as_uint(x)); r->y = y;
-}
 
 // Everything a kernel needs for one chunk of events [e0, e1).  Passed by value (__grid_constant__).
 struct Chunk {
@@ -78,16 +73,16 @@ struct Chunk {
   uint32_t* segB;           // [(e1-e0)*F + 1] global word index where segment (event, fed) starts
   uint32_t* ev_cnt;         // [(e1-e0)*EC_STRIDE]
   uint32_t* ctl;            // [CTL_WORDS]
-  uint32_t* mid_list;       // [(e1-e0)*M] task ids left by findclus to the warp-per-run kernel (findrun)
+  uint32_t* mid_list;       // [(e1-e0)*M] task ids left by the fused kernel to the warp-per-run kernel (findrun)
   uint32_t* big_list;       // [(e1-e0)*M] runs of 513..1024 words, left by findrun<512> to findrun<1024>
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
-  uint32_t ovf_cap;
-  uint32_t* startbits;      // [cap_words/32 + 8] bit (g - T0): word g starts a module run (decode -> findclus)
+  uint32_t list_cap;        // (e1-e0)*M: every event lists at most M runs (push_run)
   uint32_t* chunk_seg;      // [cap_words/128 + 2] segment (event_rel*F + fed) of the chunk's first word
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
-  // temp cluster records, indexed by chunk-relative word index (run first + local id)
-  TempRec* t_rec;
+  // temp cluster records, indexed by chunk-relative word index (run first + local id): dense 16 + 4 bytes
+  uint4* t_a;               // first_digi, n_pix, charge, x_col bits
+  float* t_y;
   // overflow-kernel scratch, indexed by chunk-relative word index
   unsigned long long* g_hash;  // [2*cap_words]
   uint32_t* g_pos; uint32_t* g_q; uint32_t* g_npix; unsigned long long* g_sx; unsigned long long* g_sy;
@@ -96,20 +91,22 @@ struct Chunk {
 __device__ __forceinline__ uint32_t ev_offset(const Chunk& c, uint32_t e) {
   return c.ev_off ? c.ev_off[e] : (e ? c.n_single : 0u);
 }
+__device__ __forceinline__ void put_temp(const Chunk& c, uint32_t i, uint32_t first, uint32_t npix, uint32_t charge, float x, float y) {
+  c.t_a[i] = make_uint4(first, npix, charge, __float_as_uint(x)); c.t_y[i] = y;
+}
 
 // launchers (host), one per kernel; all asynchronous on `stream`
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream);
-void launch_decode(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
-void launch_findclus(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
+void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
 void launch_findrun(const Chunk& c, int n_sm, cudaStream_t stream);
 
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);
-cudaError_t configure_findclus_kernel();
+cudaError_t configure_fused_kernel();
 cudaError_t configure_findrun_kernel();
 cudaError_t configure_finalize_kernel();
 cudaError_t configure_overflow_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 9;    // init, segfill, decode, findclus, findrun x2, overflow, offsets, scatter
+constexpr int LAUNCHES_PER_CHUNK = 8;    // init, segfill, fused, findrun x2, overflow, offsets, scatter
 
 }  // namespace pix
