@@ -28,14 +28,39 @@ namespace pix {
 
 namespace {
 
-constexpr int WPB = 4;                    // warps per block (they share nothing but the block)
+#ifndef PIX_WPB
+#define PIX_WPB 4
+#endif
+#ifndef PIX_BPS
+#define PIX_BPS 7
+#endif
+#ifndef PIX_JUMPS
+#define PIX_JUMPS 2
+#endif
+#ifndef PIX_UD
+#define PIX_UD 1
+#endif
+#ifndef PIX_UE
+#define PIX_UE 1
+#endif
+#ifndef PIX_UF
+#define PIX_UF 1
+#endif
+#ifndef PIX_UG
+#define PIX_UG 1
+#endif
+#ifndef PIX_GMAX
+#define PIX_GMAX 32
+#endif
+constexpr int U_UD = PIX_UD, U_UE = PIX_UE, U_UF = PIX_UF, U_UG = PIX_UG;
+constexpr int WPB = PIX_WPB;              // warps per block (they share nothing but the block)
 constexpr int FT = WPB * 32;
-constexpr int BLOCKS_PER_SM = 7;
+constexpr int BLOCKS_PER_SM = PIX_BPS;
 constexpr uint32_t HC = CHUNK_WORDS;      // words of a chunk (rounds 0-3 of a window)
 constexpr uint32_t MAXT = 256;            // window: home chunk + up to 4 rounds of the next chunk
 constexpr uint32_t RC = 62;               // runs a window can own
 constexpr uint32_t ECAP = 256;            // edge list; flushed (united) when a round might not fit
-constexpr uint32_t GMAX = 32;             // chunks per ticket, at most
+constexpr uint32_t GMAX = PIX_GMAX;             // chunks per ticket, at most
 constexpr uint32_t NOKEY = 0xFFFFFFFFu, FULL = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
@@ -43,37 +68,46 @@ constexpr uint32_t NO_ID = 0xFFFFu;
 using PH = BucketHash<23, 8, 8>;          // key: run (6 bits) | row (8) | col (9); 256 buckets of 4; digi = window slot
 constexpr uint32_t WTAB = PH::SLOTS;
 
-// Staged word (ring entry).  Decode writes pos | below; phase B adds the run and the start flag for the slots of the
-// window.  Neighbour keys are key+1 (col+1) and key+512-1, +512, +512+1 (row+1): col 416..511 and row 160..255 never
+// Staged word (ring entry), written by the decode in its final form: pos | run | below | start, where run is the
+// word's run counted inside its own chunk (0: it continues a run begun in an earlier chunk; RC+1: too many runs).
+// As the head of the next window's... previous window such a word joins that window's last run (phase B writes the run
+// back).  Neighbour keys are key+1 (col+1) and key+512-1, +512, +512+1 (row+1): col 416..511 and row 160..255 never
 // occur, so no bounds checks (S13).
 constexpr uint32_t SK_NONE = 0xFFFFFFFFu;   // no such word (outside the launch group)
 constexpr uint32_t SK_BAD = 0xFFFFFF00u;    // >= SK_BAD: undecodable word, status in the low byte
 constexpr uint32_t SK_POS = 0x1FFFFu;       // row << 9 | col
 constexpr uint32_t SK_RUN_SHIFT = 17, SK_KEY = 0x7FFFFFu;  // run in bits 17-22; hash key = sk & SK_KEY
 constexpr uint32_t SK_BELOW = 1u << 23, SK_START = 1u << 24;
-static_assert(RC + 1u < 64u && MAXT <= 256u && 3u * MAXT <= WTAB, "run field, slot field, sums fit the hash memory");
+static_assert(RC + 1u < 64u && MAXT <= 256u && 3u * MAXT + MAXT / 4u <= WTAB, "run field, slot field; sums + root list fit the hash memory");
 
 struct __align__(16) WarpSmem {
-  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D: qn = tab, sx = tab + 256, sy = tab + 512
+  uint32_t tab[WTAB];      // position hash, EMPTY-filled.  After phase D: qn = tab, sx = tab + 256, sy = tab + 512, root list
   uint32_t label[MAXT];    // union-find parent of window slot t, or MARK_*
-  uint32_t skey[MAXT];     // ring of two chunks: staged words (lane-private: slot t belongs to lane t & 31)
+  uint32_t skey[MAXT];     // ring of two chunks: staged words (lane-private while staged: slot t belongs to lane t & 31)
   uint16_t chg[MAXT];      // ring: charges
   uint16_t edge[ECAP];     // a | b << 8; after the unions: local id of a root, or NO_ID
   uint32_t run_ifirst[RC + 2];  // event-relative index of the run's first digi
   uint32_t run_key[RC + 2];     // event_rel << 16 | module
   uint16_t run_first[RC + 2];   // window slot of the run's first digi
-  uint16_t run_base[RC + 2];    // survivors before the run
+  uint16_t run_cnt[RC + 2];     // clusters of the run that survive the cut
   uint8_t run_bad[RC + 2];      // the run is left to the warp-per-run kernel
 };
 static_assert(sizeof(WarpSmem) % 16 == 0, "per-warp slices stay 16-byte aligned");
 
-struct Dec {          // what the decode of a chunk leaves in registers for its turn as home chunk
-  uint32_t key[4];    // per lane: event_rel << 16 | module of its word in round j, NOKEY if undecodable
-  uint32_t sb[4];     // warp-uniform: run-start bits of round j
+struct Dec {          // what the decode of a chunk leaves in (warp-uniform) registers for its turn as home chunk
+  uint32_t R;         // runs that start in the chunk
+  uint32_t fs, ls;    // slot of the first / last run start (fs = HC: none)
   uint32_t ebase0;    // global index of word 0 of the event of the chunk's first word
   uint32_t er0;       // that event
   bool one_event;     // all 128 words exist and belong to event er0
 };
+
+// rare: event of word g (a FED / event boundary inside the chunk whose first word lies in segment sg0)
+__device__ __noinline__ uint32_t event_of(const Chunk& c, uint32_t S, uint32_t sg0, uint32_t g) {
+  uint32_t sg = sg0;
+  while (sg + 1u < S && c.segB[sg + 1u] <= g) ++sg;
+  return div_F(c, sg);
+}
 
 __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -87,6 +121,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
   const uint32_t n_chunks = (gEnd - T0 + HC - 1u) / HC;
   const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
   uint32_t* const qn = s.tab; uint32_t* const sx = s.tab + MAXT; uint32_t* const sy = s.tab + 2 * MAXT;
+  uint8_t* const rlist = reinterpret_cast<uint8_t*>(s.tab + 3 * MAXT);  // roots in digi order (after phase D)
   uint16_t* const lid = s.edge;
   uint32_t G = n_chunks / (gridDim.x * WPB * 4u);  // about four tickets per warp
   G = G < 1u ? 1u : (G > GMAX ? GMAX : G);
@@ -145,16 +180,20 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
     }
 
     Dec cur, nxt;
+    cur.R = 0u; cur.fs = HC; cur.ls = 0u; cur.ebase0 = 0u; cur.er0 = 0u; cur.one_event = false;
+    uint32_t sgc = 0u;   // segment of the home chunk's first word
+    uint32_t wn[4];      // the raw words of the chunk that is decoded next (loaded one iteration ahead)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) { cur.key[j] = NOKEY; cur.sb[j] = 0u; }
-    cur.ebase0 = 0u; cur.er0 = 0u; cur.one_event = false;
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t g = T0 + c0 * HC + 32u * j + lane;
+      wn[j] = (g >= gBeg && g < gEnd) ? __ldg(c.words + g) : 0u;
+    }
 
     for (uint32_t ci = c0;; ++ci) {
       const uint32_t hn = ((ci - c0) & 1u) * HC;  // ring half of chunk ci; chunk ci-1 sits in the other half
       // ================================================================== decode chunk ci (a1, a2, a3)
-#pragma unroll
-      for (int j = 0; j < 4; ++j) { nxt.key[j] = NOKEY; nxt.sb[j] = 0u; }
-      nxt.ebase0 = 0u; nxt.er0 = 0u; nxt.one_event = false;
+      nxt.R = 0u; nxt.fs = HC; nxt.ls = 0u; nxt.ebase0 = 0u; nxt.er0 = 0u; nxt.one_event = false;
+      uint32_t sgn = 0u;
       if (ci < n_chunks) {
         const bool owner = ci < c1;  // else: the look-ahead of the range's last window, nothing is written
         const uint32_t b = T0 + ci * HC;
@@ -164,15 +203,19 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
         const bool all_in = b >= gBeg && b + HC <= gEnd;
         const bool one_seg = all_in && b + HC <= nextB0;
         nxt.ebase0 = segB[er0 * F]; nxt.er0 = er0; nxt.one_event = all_in && b + HC <= evend0;
-        uint32_t w[4];
+        sgn = sg0;
+        uint32_t w0 = wn[0], w1 = wn[1], w2 = wn[2], w3 = wn[3];
+        if (owner && ci + 1u < n_chunks) {  // the words of chunk ci + 1: in flight while this chunk is decoded and the window clustered
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint32_t g = b + 32u * j + lane;
-          w[j] = (all_in || (g >= gBeg && g < gEnd)) ? __ldg(c.words + g) : 0u;
+          for (int j = 0; j < 4; ++j) {
+            const uint32_t g = b + HC + 32u * j + lane;
+            wn[j] = g < gEnd ? __ldg(c.words + g) : 0u;
+          }
         }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
+#pragma unroll 1
+        for (uint32_t j = 0; j < 4; ++j) {
           const uint32_t g = b + 32u * j + lane;
+          const uint32_t w = j == 0u ? w0 : (j == 1u ? w1 : (j == 2u ? w2 : w3));
           const bool exists = all_in || (g >= gBeg && g < gEnd);
           uint32_t er = er0, fed = fed0;
           if (!one_seg && exists) {  // rare: a FED / event boundary inside the chunk
@@ -181,38 +224,42 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             er = div_F(c, sg); fed = sg - er * F;
           }
           uint32_t m, row, col;
-          const uint32_t st = decode_word(c.cab, w[j], fed << 11, m, row, col);
+          const uint32_t st = decode_word(c.cab, w, fed << 11, m, row, col);
           const bool ok = exists && st == ST_OK;
           int32_t e = 0;
-          if (ok) e = calibrate(c, w[j] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
-          const uint32_t sk = ok ? ((row << 9) | col | (e < c.thr ? SK_BELOW : 0u)) : (exists ? (SK_BAD | st) : SK_NONE);
-          s.skey[hn + 32u * j + lane] = sk;
-          s.chg[hn + 32u * j + lane] = (uint16_t)e;
+          if (ok) e = calibrate(c, w & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
           if (owner && exists) {
             c.d_module[g] = (uint16_t)(ok ? m : 0xFFFFu); c.d_row[g] = (uint16_t)(ok ? row : 0xFFFFu);
             c.d_col[g] = (uint16_t)(ok ? col : 0xFFFFu); c.d_charge[g] = e;
             if (!ok) atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
           }
-          nxt.key[j] = ok ? ((er << 16) | m) : NOKEY;
-        }
-        // a3: a word starts a run when its (event, module) differs from the previous decodable word's
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const bool valid = nxt.key[j] != NOKEY;
-          const uint32_t has = __ballot_sync(FULL, valid);
+          // a3: a word starts a run when its (event, module) differs from the previous decodable word's
+          const uint32_t key = ok ? ((er << 16) | m) : NOKEY;
+          const uint32_t has = __ballot_sync(FULL, ok);
           const uint32_t below_l = has & lt_mask;
           const int src = below_l ? 31 - __clz(below_l) : 0;
-          uint32_t pkey = __shfl_sync(FULL, nxt.key[j], src), pg = b + 32u * j + (uint32_t)src;
+          uint32_t pkey = __shfl_sync(FULL, key, src), pg = b + 32u * j + (uint32_t)src;
           if (!below_l) { pkey = carry_key; pg = carry_g; }
-          const bool start = valid && nxt.key[j] != pkey;
-          nxt.sb[j] = __ballot_sync(FULL, start);
+          const bool start = ok && key != pkey;
+          const uint32_t sbj = __ballot_sync(FULL, start);
           if (owner && start) {
-            run_start(c, nxt.key[j], b + 32u * j + lane);
+            run_start(c, key, g);
             if (pkey != NOKEY) run_end(c, pkey, pg);
+          }
+          uint32_t r = nxt.R + __popc(sbj & le_mask);
+          r = r <= RC ? r : RC + 1u;
+          const uint32_t sk = ok ? ((row << 9) | col | (r << SK_RUN_SHIFT) | (e < c.thr ? SK_BELOW : 0u) | (start ? SK_START : 0u))
+                                 : (exists ? (SK_BAD | st) : SK_NONE);
+          s.skey[hn + 32u * j + lane] = sk;
+          s.chg[hn + 32u * j + lane] = (uint16_t)e;
+          if (sbj) {
+            if (nxt.fs == HC) nxt.fs = 32u * j + (uint32_t)__ffs(sbj) - 1u;
+            nxt.ls = 32u * j + 31u - (uint32_t)__clz(sbj);
+            nxt.R += __popc(sbj);
           }
           if (has) {
             const int top = 31 - __clz(has);
-            carry_key = __shfl_sync(FULL, nxt.key[j], top); carry_g = b + 32u * j + (uint32_t)top;
+            carry_key = __shfl_sync(FULL, key, top); carry_g = b + 32u * j + (uint32_t)top;
           }
         }
       }
@@ -221,91 +268,65 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
       if (ci > c0) {
         const uint32_t hb = hn ^ HC;                 // ring half of the home chunk
         const uint32_t b = T0 + (ci - 1u) * HC;      // global index of window slot 0
-        uint32_t rb[4];                              // runs started before round k
-        uint32_t R = 0u;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { rb[k] = R; R += __popc(cur.sb[k]); }
+        const uint32_t R = cur.R;
         uint32_t f_t = MAXT, e_t = 0u;               // window = slots [f_t, e_t); empty when nothing is owned
         uint32_t Rown = R;                           // runs of the window (the last run may be left to findrun)
         if (R) {
-          const uint32_t kf = cur.sb[0] ? 0u : (cur.sb[1] ? 1u : (cur.sb[2] ? 2u : 3u));
-          f_t = 32u * kf + (uint32_t)__ffs(kf == 0u ? cur.sb[0] : (kf == 1u ? cur.sb[1] : (kf == 2u ? cur.sb[2] : cur.sb[3]))) - 1u;
+          f_t = cur.fs;
           // end of the last run: the first run start of the next chunk, the end of the data, or "does not fit"
-          if (nxt.sb[0] | nxt.sb[1] | nxt.sb[2] | nxt.sb[3]) {
-            const uint32_t ke = nxt.sb[0] ? 0u : (nxt.sb[1] ? 1u : (nxt.sb[2] ? 2u : 3u));
-            e_t = HC + 32u * ke + (uint32_t)__ffs(ke == 0u ? nxt.sb[0] : (ke == 1u ? nxt.sb[1] : (ke == 2u ? nxt.sb[2] : nxt.sb[3]))) - 1u;
+          if (nxt.fs < HC) {
+            e_t = HC + nxt.fs;
           } else if (b + MAXT >= gEnd) {
             e_t = gEnd - b;
           } else {  // the last run does not end inside the next chunk: the warp-per-run kernel takes it
-            const uint32_t kz = cur.sb[3] ? 3u : (cur.sb[2] ? 2u : (cur.sb[1] ? 1u : 0u));
-            const uint32_t sbz = kz == 3u ? cur.sb[3] : (kz == 2u ? cur.sb[2] : (kz == 1u ? cur.sb[1] : cur.sb[0]));
-            const uint32_t lz = 31u - (uint32_t)__clz(sbz);
-            e_t = 32u * kz + lz;
-            uint32_t keyz = kz == 3u ? cur.key[3] : (kz == 2u ? cur.key[2] : (kz == 1u ? cur.key[1] : cur.key[0]));
-            if (lane == lz) push_run(c, c.mid_list, CTL_MID_COUNT, keyz >> 16, keyz & 0xFFFFu);
+            e_t = cur.ls;
+            if (lane == (e_t & 31u)) {
+              const uint32_t er = cur.one_event ? cur.er0 : event_of(c, S, sgc, b + e_t);
+              push_run(c, c.mid_list, CTL_MID_COUNT, er, c.d_module[b + e_t]);
+            }
             Rown = R - 1u;
             if (e_t == f_t) { f_t = MAXT; e_t = 0u; }  // it was the only run
           }
         }
         const bool owns = e_t > f_t;
         if (owns) {
-          // ============================================================== B: clear; runs; insert
+          // ============================================================== B: clear; run tables; insert
           {
             uint4* t4 = reinterpret_cast<uint4*>(s.tab);
             const uint4 e4 = make_uint4(PH::EMPTY, PH::EMPTY, PH::EMPTY, PH::EMPTY);
 #pragma unroll
             for (int k = 0; k < (int)(WTAB / 4 / 32); ++k) t4[lane + 32 * k] = e4;
             if (lane < (RC + 2u) / 4u) reinterpret_cast<uint32_t*>(s.run_bad)[lane] = 0u;
+            reinterpret_cast<uint32_t*>(s.run_cnt)[lane] = 0u;
           }
           __syncwarp();  // the cleared hash is visible
-          if (Rown > RC && lane == 0) s.run_bad[RC + 1u] = 1;  // the runs beyond RC are all "run 63"
+          if (Rown > RC && lane == 0) s.run_bad[RC + 1u] = 1;  // the runs beyond RC are all "run RC + 1"
           bool dup_seen = false;
           const uint32_t k0 = f_t >> 5, kl = (e_t + 31u) >> 5;  // rounds k0 .. kl-1 hold the window
-#pragma unroll
-          for (uint32_t k = 0; k < 4; ++k) {
-            if (k < k0 || k >= kl) continue;  // warp-uniform
-            const uint32_t t = 32u * k + lane;
-            const uint32_t sk = s.skey[hb + t];
-            const bool start = (cur.sb[k] >> lane) & 1u;
-            const uint32_t r = rb[k] + __popc(cur.sb[k] & le_mask);
-            const bool inw = t >= f_t && t < e_t;
-            const bool dec = inw && sk < SK_BAD;
-            if (start && inw) {
-              const uint32_t key = cur.key[k];
+          const uint32_t Rr = R <= RC ? R : RC + 1u;             // run of the slots of the next chunk
+#pragma unroll 1
+          for (uint32_t k = k0; k < kl; ++k) {
+            const uint32_t t = 32u * k + lane, ph = (hb + t) & (MAXT - 1u);
+            uint32_t sk = s.skey[ph];
+            const bool dec = t >= f_t && t < e_t && sk < SK_BAD;
+            if (k >= 4u && dec) { sk |= Rr << SK_RUN_SHIFT; s.skey[ph] = sk; }  // the head of the next chunk: the rest of run R
+            const uint32_t r = (sk >> SK_RUN_SHIFT) & 63u;
+            if (dec && (sk & SK_START)) {
+              const uint32_t er = cur.one_event ? cur.er0 : event_of(c, S, sgc, b + t);
+              const uint32_t m = c.d_module[b + t];  // written by this thread when it decoded the word
               if (r <= RC) {
-                s.run_first[r] = (uint16_t)t; s.run_key[r] = key;
-                s.run_ifirst[r] = b + t - (cur.one_event ? cur.ebase0 : segB[(key >> 16) * F]);
+                s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | m;
+                s.run_ifirst[r] = b + t - (cur.one_event ? cur.ebase0 : segB[er * F]);
               } else {
-                push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);  // too many runs: left to findrun
+                push_run(c, c.mid_list, CTL_MID_COUNT, er, m);  // too many runs: left to findrun
               }
             }
-            const uint32_t rr = r <= RC ? r : RC + 1u;
-            const uint32_t nsk = (sk & (SK_POS | SK_BELOW)) | (rr << SK_RUN_SHIFT) | (start ? SK_START : 0u);
             const bool live = dec && !(sk & SK_BELOW) && r <= RC;
-            if (dec) s.skey[hb + t] = nsk;
             s.label[t] = live ? t : MARK_BELOW;
             if (dec && r <= RC) {
-              const uint32_t ins = PH::insert(s.tab, nsk & SK_KEY, t, (sk & SK_BELOW) ? 1u : 0u);
+              const uint32_t ins = PH::insert(s.tab, sk & SK_KEY, t, (sk & SK_BELOW) ? 1u : 0u);
               dup_seen |= ins == 1u;
               if (ins == 2u) s.run_bad[r] = 1;  // no room near the home bucket: findrun takes the run
-            }
-          }
-          {
-            const uint32_t rr = R <= RC ? R : RC + 1u;
-#pragma unroll 1
-            for (uint32_t k = 4; k < kl; ++k) {  // the head of the next chunk: the rest of run R
-              const uint32_t t = 32u * k + lane;
-              const uint32_t sk = s.skey[hn + t - HC];
-              const bool dec = t < e_t && sk < SK_BAD;
-              const uint32_t nsk = (sk & (SK_POS | SK_BELOW)) | (rr << SK_RUN_SHIFT);
-              const bool live = dec && !(sk & SK_BELOW) && R <= RC;
-              if (dec) s.skey[hn + t - HC] = nsk;
-              s.label[t] = live ? t : MARK_BELOW;
-              if (dec && R <= RC) {
-                const uint32_t ins = PH::insert(s.tab, nsk & SK_KEY, t, (sk & SK_BELOW) ? 1u : 0u);
-                dup_seen |= ins == 1u;
-                if (ins == 2u) s.run_bad[R] = 1;
-              }
             }
           }
           __syncwarp();  // hash, labels, run tables complete
@@ -337,7 +358,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
               }
               ne = 0u;
             }
-            const bool live = t >= f_t && t < e_t && sk < SK_BAD && s.label[t] < MAXT;
+            const bool live = s.label[t] < MAXT;  // slots outside the window and undecodable words carry MARK_BELOW
             bool f0 = false, f1 = false, f2 = false;
             uint32_t n0 = 0, n1 = 0, n2 = 0;
             if (live) {
@@ -366,7 +387,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             __syncwarp();
           }
 #pragma unroll 1
-          for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: the chains shrink 4x before the sums
+          for (int pass = 0; pass < PIX_JUMPS; ++pass) {  // pointer jumping: the chains shrink before the sums
             for (uint32_t k = k0; k < kl; ++k) {
               const uint32_t t = 32u * k + lane;
               const uint32_t l = s.label[t];
@@ -375,7 +396,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             __syncwarp();
           }
 
-          // ============================================================== E: cluster sums (the hash is dead: qn / sx / sy)
+          // ============================================================== E: cluster sums (the hash is dead: qn / sx / sy / root list)
           {
             uint4* t4 = reinterpret_cast<uint4*>(s.tab);
             const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
@@ -383,12 +404,14 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             for (int k = 0; k < (int)(3 * MAXT / 4 / 32); ++k) t4[lane + 32 * k] = z4;
           }
           __syncwarp();
+          uint32_t nr = 0u;  // roots so far
 #pragma unroll 1
           for (uint32_t k = k0; k < kl; ++k) {
             const uint32_t t = 32u * k + lane;
             volatile uint32_t* L = s.label;
             uint32_t r = L[t];
-            if (r < MAXT) {  // live (else MARK_*); labels outside the window are never read: k0 <= k < kl and MARK_BELOW there
+            const bool live = r < MAXT;  // else MARK_*
+            if (live) {
               while (true) { const uint32_t n = L[r]; if (n == r) break; r = n; }
               L[t] = r;  // flatten: r is the root, so other walkers through t stay correct
               const uint32_t ph = (hb + t) & (MAXT - 1u);
@@ -397,61 +420,64 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
               atomicAdd(&sx[r], e * (sk & 511u));
               atomicAdd(&sy[r], e * ((sk >> 9) & 255u));
             }
+            const bool root = live && r == t;
+            const uint32_t rm = __ballot_sync(FULL, root);
+            if (root) rlist[nr + __popc(rm & lt_mask)] = (uint8_t)t;  // digi order
+            nr += __popc(rm);
           }
           __syncwarp();
 
-          // ============================================================== F: cut, renumber, temp records, in slot order
+          // ============================================================== F: cut, renumber, temp records (one root per lane)
           {
-            uint32_t cnt = 0u;               // surviving roots before this round
-            uint32_t base_c = 0u, rf_c = 0u; // of the run that is open when the round starts: survivors before it, its first slot
-            const uint32_t relb = b - gBeg;  // may wrap for the first chunk; only used added to a slot >= gBeg - b
+            uint32_t cnt = 0u;                   // surviving roots before this iteration
+            uint32_t run_c = 0u, base_c = 0u;    // the run of the last root so far and the survivors before that run
+            const uint32_t relb = b - gBeg;      // may wrap for the first chunk; only used added to a slot >= gBeg - b
 #pragma unroll 1
-            for (uint32_t k = k0; k < kl; ++k) {
-              const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
-              const bool dec = t >= f_t && t < e_t && sk < SK_BAD;
-              const uint32_t r = (sk >> SK_RUN_SHIFT) & 63u;
-              const bool root = dec && s.label[t] == t;
-              uint32_t Q = 0u, np = 0u;
-              if (root) {
+            for (uint32_t i0 = 0u; i0 < nr; i0 += 32u) {
+              const bool valid = i0 + lane < nr;
+              uint32_t t = 0u, r = 0u, Q = 0u, np = 0u;
+              if (valid) {
+                t = rlist[i0 + lane];
+                r = (s.skey[(hb + t) & (MAXT - 1u)] >> SK_RUN_SHIFT) & 63u;
                 const uint32_t v = qn[t];
                 Q = v & 0xFFFFFFu; np = v >> 24;
                 if (np == 0u) np = 256u;
                 if (Q > Q_SAFE) s.run_bad[r] = 1;  // 32-bit weighted sums may have wrapped
               }
-              const bool surv = root && (int32_t)Q >= c.cut;  // S9: equality keeps
+              const bool surv = valid && (int32_t)Q >= c.cut;  // S9: equality keeps
               const uint32_t sm = __ballot_sync(FULL, surv);
               const uint32_t rank = cnt + __popc(sm & lt_mask);
-              const bool isstart = dec && (sk & SK_START);
-              const uint32_t stm = __ballot_sync(FULL, isstart);
-              const uint32_t mine = stm & le_mask;
-              const int sl = mine ? 31 - __clz(mine) : 0;
-              uint32_t base = __shfl_sync(FULL, rank, sl), rf = 32u * k + (uint32_t)sl;
-              if (!mine) { base = base_c; rf = rf_c; }
-              if (isstart) s.run_base[r] = (uint16_t)rank;  // survivors before the run
-              if (root) {
+              // runs are contiguous in digi order: the first lane of this lane's run in this iteration
+              const uint32_t rprev = __shfl_up_sync(FULL, r, 1);
+              const uint32_t bnd = __ballot_sync(FULL, valid && (lane == 0u || r != rprev));
+              const uint32_t fl = 31u - (uint32_t)__clz(bnd & le_mask);  // bit 0 of bnd is set whenever lane 0 is valid
+              uint32_t base = cnt + __popc(sm & ((1u << fl) - 1u));
+              if (fl == 0u && r == run_c) base = base_c;  // the run began in an earlier iteration
+              if (valid) {
                 uint32_t id = NO_ID;
                 if (surv) {
                   id = rank - base;
+                  const uint32_t rf = s.run_first[r];
                   // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
                   const float fq = (float)Q;
                   put_temp(c, relb + rf + id, s.run_ifirst[r] + (t - rf), np, Q, __fdividef((float)sx[t], fq),
                            __fdividef((float)sy[t], fq));
                 }
                 lid[t] = (uint16_t)id;
+                // the last root of the run in this iteration leaves the run's count so far
+                const bool lastofrun = lane == 31u || i0 + lane + 1u == nr || ((bnd >> (lane + 1u)) & 1u);
+                if (lastofrun) s.run_cnt[r] = (uint16_t)(rank + (surv ? 1u : 0u) - base);
               }
-              if (stm) {
-                const int top = 31 - __clz(stm);
-                base_c = __shfl_sync(FULL, rank, top); rf_c = 32u * k + (uint32_t)top;
-              }
+              const uint32_t lastl = 31u - (uint32_t)__clz(__ballot_sync(FULL, valid));
+              run_c = __shfl_sync(FULL, r, lastl); base_c = __shfl_sync(FULL, base, lastl);
               cnt += __popc(sm);
             }
-            if (lane == 0) s.run_base[Rw + 1u] = (uint16_t)cnt;
           }
-          __syncwarp();  // run_base, run_bad, local ids final
+          __syncwarp();  // run_cnt, run_bad, local ids final
           for (uint32_t r = 1u + lane; r <= Rw; r += 32u) {
             const uint32_t key = s.run_key[r];
             if (s.run_bad[r]) push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);
-            else c.n_clus[(key >> 16) * c.M + (key & 0xFFFFu)] = (uint32_t)s.run_base[r + 1u] - s.run_base[r];
+            else c.n_clus[(key >> 16) * c.M + (key & 0xFFFFu)] = s.run_cnt[r];
           }
         }
 
@@ -491,7 +517,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
         __syncwarp();  // shared state is rewritten by the next window
       }
       if (ci >= c1) break;
-      cur = nxt;
+      cur = nxt; sgc = sgn;
     }
     flush();
     acc_ev = NOKEY;
