@@ -182,94 +182,175 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
     Dec cur, nxt;
     cur.R = 0u; cur.fs = HC; cur.ls = 0u; cur.ebase0 = 0u; cur.er0 = 0u; cur.one_event = false;
     uint32_t sgc = 0u;   // segment of the home chunk's first word
-    uint32_t wn[4];      // the raw words of the chunk that is decoded next (loaded one iteration ahead)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const uint32_t g = T0 + c0 * HC + 32u * j + lane;
-      wn[j] = (g >= gBeg && g < gEnd) ? __ldg(c.words + g) : 0u;
+    uint4 wn = make_uint4(0u, 0u, 0u, 0u);  // the raw words of the chunk that is decoded next (loaded one iteration ahead)
+    {
+      const uint32_t g0 = T0 + c0 * HC + 4u * lane;
+      if (g0 >= gBeg && g0 + 4u <= gEnd) wn = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
+      else {
+        if (g0 >= gBeg && g0 < gEnd) wn.x = __ldg(c.words + g0);
+        if (g0 + 1u >= gBeg && g0 + 1u < gEnd) wn.y = __ldg(c.words + g0 + 1u);
+        if (g0 + 2u >= gBeg && g0 + 2u < gEnd) wn.z = __ldg(c.words + g0 + 2u);
+        if (g0 + 3u >= gBeg && g0 + 3u < gEnd) wn.w = __ldg(c.words + g0 + 3u);
+      }
     }
 
     for (uint32_t ci = c0;; ++ci) {
       const uint32_t hn = ((ci - c0) & 1u) * HC;  // ring half of chunk ci; chunk ci-1 sits in the other half
-      // ================================================================== decode chunk ci (a1, a2, a3)
+      // ================================================================== decode chunk ci (a1, a2, a3): four consecutive words per lane
       nxt.R = 0u; nxt.fs = HC; nxt.ls = 0u; nxt.ebase0 = 0u; nxt.er0 = 0u; nxt.one_event = false;
       uint32_t sgn = 0u;
       if (ci < n_chunks) {
         const bool owner = ci < c1;  // else: the look-ahead of the range's last window, nothing is written
-        const uint32_t b = T0 + ci * HC;
+        const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
         const uint32_t sg0 = c.chunk_seg[ci];
         const uint32_t er0 = div_F(c, sg0), fed0 = sg0 - er0 * F;
-        const uint32_t nextB0 = segB[sg0 + 1u], evend0 = segB[(er0 + 1u) * F];
+        const uint32_t nextB0 = segB[sg0 + 1u], evend0 = segB[(er0 + 1u) * F], ebase0 = segB[er0 * F];
         const bool all_in = b >= gBeg && b + HC <= gEnd;
         const bool one_seg = all_in && b + HC <= nextB0;
-        nxt.ebase0 = segB[er0 * F]; nxt.er0 = er0; nxt.one_event = all_in && b + HC <= evend0;
+        nxt.ebase0 = ebase0; nxt.er0 = er0; nxt.one_event = all_in && b + HC <= evend0;
         sgn = sg0;
-        uint32_t w0 = wn[0], w1 = wn[1], w2 = wn[2], w3 = wn[3];
+        const uint32_t w[4] = {wn.x, wn.y, wn.z, wn.w};
+        wn = make_uint4(0u, 0u, 0u, 0u);
         if (owner && ci + 1u < n_chunks) {  // the words of chunk ci + 1: in flight while this chunk is decoded and the window clustered
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const uint32_t g = b + HC + 32u * j + lane;
-            wn[j] = g < gEnd ? __ldg(c.words + g) : 0u;
+          const uint32_t h0 = g0 + HC;
+          if (h0 + 4u <= gEnd) wn = __ldg(reinterpret_cast<const uint4*>(c.words + h0));
+          else {
+            if (h0 < gEnd) wn.x = __ldg(c.words + h0);
+            if (h0 + 1u < gEnd) wn.y = __ldg(c.words + h0 + 1u);
+            if (h0 + 2u < gEnd) wn.z = __ldg(c.words + h0 + 2u);
           }
         }
-#pragma unroll 1
-        for (uint32_t j = 0; j < 4; ++j) {
-          const uint32_t g = b + 32u * j + lane;
-          const uint32_t w = j == 0u ? w0 : (j == 1u ? w1 : (j == 2u ? w2 : w3));
+        uint32_t st[4], key[4], sk[4];
+        uint32_t mod[4], row[4], col[4];
+        int32_t chg[4];
+        uint32_t exmask = 0u;  // words of the lane that exist
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t g = g0 + j;
           const bool exists = all_in || (g >= gBeg && g < gEnd);
+          exmask |= exists ? 1u << j : 0u;
           uint32_t er = er0, fed = fed0;
           if (!one_seg && exists) {  // rare: a FED / event boundary inside the chunk
             uint32_t sg = sg0;
             while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
             er = div_F(c, sg); fed = sg - er * F;
           }
-          uint32_t m, row, col;
-          const uint32_t st = decode_word(c.cab, w, fed << 11, m, row, col);
-          const bool ok = exists && st == ST_OK;
-          int32_t e = 0;
-          if (ok) e = calibrate(c, w & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
-          if (owner && exists) {
-            c.d_module[g] = (uint16_t)(ok ? m : 0xFFFFu); c.d_row[g] = (uint16_t)(ok ? row : 0xFFFFu);
-            c.d_col[g] = (uint16_t)(ok ? col : 0xFFFFu); c.d_charge[g] = e;
-            if (!ok) atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
-          }
-          // a3: a word starts a run when its (event, module) differs from the previous decodable word's
-          const uint32_t key = ok ? ((er << 16) | m) : NOKEY;
-          const uint32_t has = __ballot_sync(FULL, ok);
-          const uint32_t below_l = has & lt_mask;
-          const int src = below_l ? 31 - __clz(below_l) : 0;
-          uint32_t pkey = __shfl_sync(FULL, key, src), pg = b + 32u * j + (uint32_t)src;
-          if (!below_l) { pkey = carry_key; pg = carry_g; }
-          const bool start = ok && key != pkey;
-          const uint32_t sbj = __ballot_sync(FULL, start);
-          if (owner && start) {
-            run_start(c, key, g);
-            if (pkey != NOKEY) run_end(c, pkey, pg);
-          }
-          uint32_t r = nxt.R + __popc(sbj & le_mask);
-          r = r <= RC ? r : RC + 1u;
-          const uint32_t sk = ok ? ((row << 9) | col | (r << SK_RUN_SHIFT) | (e < c.thr ? SK_BELOW : 0u) | (start ? SK_START : 0u))
-                                 : (exists ? (SK_BAD | st) : SK_NONE);
-          s.skey[hn + 32u * j + lane] = sk;
-          s.chg[hn + 32u * j + lane] = (uint16_t)e;
-          if (sbj) {
-            if (nxt.fs == HC) nxt.fs = 32u * j + (uint32_t)__ffs(sbj) - 1u;
-            nxt.ls = 32u * j + 31u - (uint32_t)__clz(sbj);
-            nxt.R += __popc(sbj);
-          }
-          if (has) {
-            const int top = 31 - __clz(has);
-            carry_key = __shfl_sync(FULL, key, top); carry_g = b + 32u * j + (uint32_t)top;
+          uint32_t m, r, cc;
+          st[j] = decode_word(c.cab, w[j], fed << 11, m, r, cc);
+          const bool ok = exists && st[j] == ST_OK;
+          mod[j] = row[j] = col[j] = 0xFFFFu; chg[j] = 0; key[j] = NOKEY;
+          if (ok) {
+            mod[j] = m; row[j] = r; col[j] = cc;
+            chg[j] = calibrate(c, w[j] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + cc)));  // S8: one pair per (module, col)
+            key[j] = (er << 16) | m;
+          } else if (owner && exists) {
+            atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st[j] - ST_EMPTY), 1u);
           }
         }
+        if (owner) {
+          if (exmask == 15u) {
+            *reinterpret_cast<ushort4*>(c.d_module + g0) = make_ushort4(mod[0], mod[1], mod[2], mod[3]);
+            *reinterpret_cast<ushort4*>(c.d_row + g0) = make_ushort4(row[0], row[1], row[2], row[3]);
+            *reinterpret_cast<ushort4*>(c.d_col + g0) = make_ushort4(col[0], col[1], col[2], col[3]);
+            *reinterpret_cast<int4*>(c.d_charge + g0) = make_int4(chg[0], chg[1], chg[2], chg[3]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              if (!(exmask >> j & 1u)) continue;
+              const uint32_t g = g0 + j;
+              c.d_module[g] = (uint16_t)mod[j]; c.d_row[g] = (uint16_t)row[j]; c.d_col[g] = (uint16_t)col[j];
+              c.d_charge[g] = chg[j];
+            }
+          }
+          // undecodable words are finished here (status, clus = -1)
+          const uint32_t badmask = (key[0] == NOKEY ? 1u : 0u) | (key[1] == NOKEY ? 2u : 0u) | (key[2] == NOKEY ? 4u : 0u) | (key[3] == NOKEY ? 8u : 0u);
+          if (badmask & exmask) {
+            if (badmask == 15u && exmask == 15u) {
+              *reinterpret_cast<uchar4*>(c.d_status + g0) = make_uchar4(st[0], st[1], st[2], st[3]);
+              *reinterpret_cast<int4*>(c.d_clus + g0) = make_int4(-1, -1, -1, -1);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if ((badmask & exmask) >> j & 1u) { c.d_status[g0 + j] = (uint8_t)st[j]; c.d_clus[g0 + j] = -1; }
+            }
+          }
+        }
+        // a3: a word starts a run when its (event, module) differs from the previous decodable word's
+        uint32_t tkey = NOKEY, tj = 0u;  // the lane's last decodable word
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (key[j] != NOKEY) { tkey = key[j]; tj = j; }
+        const uint32_t has = __ballot_sync(FULL, tkey != NOKEY);
+        const uint32_t below_l = has & lt_mask;
+        const int src = below_l ? 31 - __clz(below_l) : 0;
+        uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = b + 4u * (uint32_t)src + __shfl_sync(FULL, tj, src);
+        if (!below_l) { pkey = carry_key; pg = carry_g; }
+        uint32_t startmask = 0u;
+        uint32_t s_key = NOKEY, s_g = 0u, s_pkey = NOKEY, s_pg = 0u;  // the lane's first run start and its predecessor
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (key[j] == NOKEY) continue;
+          if (key[j] != pkey) {
+            if (!startmask) { s_key = key[j]; s_g = g0 + j; s_pkey = pkey; s_pg = pg; }
+            startmask |= 1u << j;
+          }
+          pkey = key[j]; pg = g0 + j;
+        }
+        if (owner) {
+          if (s_key != NOKEY) {  // one copy of the atomics for the usual case of at most one start per lane
+            run_start(c, s_key, s_g);
+            if (s_pkey != NOKEY) run_end(c, s_pkey, s_pg);
+          }
+          if (startmask & (startmask - 1u)) {  // rare: several runs start inside the lane's four words
+            uint32_t pk = NOKEY, pgg = 0u;
+            bool first = true;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              if (key[j] == NOKEY) continue;
+              if (startmask >> j & 1u) {
+                if (!first) { run_start(c, key[j], g0 + j); run_end(c, pk, pgg); }
+                first = false;
+              }
+              pk = key[j]; pgg = g0 + j;
+            }
+          }
+        }
+        if (has) {
+          const int top = 31 - __clz(has);
+          carry_key = __shfl_sync(FULL, tkey, top); carry_g = b + 4u * (uint32_t)top + __shfl_sync(FULL, tj, top);
+        }
+        // runs: the word's run counted inside the chunk; chunk totals
+        const uint32_t anyst = __ballot_sync(FULL, startmask != 0u);
+        uint32_t rbefore = __popc(startmask);  // inclusive scan over the lanes, then made exclusive
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const uint32_t o = __shfl_up_sync(FULL, rbefore, d);
+          if (lane >= (uint32_t)d) rbefore += o;
+        }
+        nxt.R = __shfl_sync(FULL, rbefore, 31);
+        rbefore -= __popc(startmask);
+        if (anyst) {
+          const int fl = __ffs(anyst) - 1, ll = 31 - __clz(anyst);
+          nxt.fs = 4u * (uint32_t)fl + (uint32_t)__ffs(__shfl_sync(FULL, startmask, fl)) - 1u;
+          nxt.ls = 4u * (uint32_t)ll + 31u - (uint32_t)__clz(__shfl_sync(FULL, startmask, ll));
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          uint32_t r = rbefore + __popc(startmask & ((2u << j) - 1u));
+          r = r <= RC ? r : RC + 1u;
+          sk[j] = key[j] != NOKEY ? ((row[j] << 9) | col[j] | (r << SK_RUN_SHIFT) | (chg[j] < c.thr ? SK_BELOW : 0u) | ((startmask >> j & 1u) ? SK_START : 0u))
+                                  : ((exmask >> j & 1u) ? (SK_BAD | st[j]) : SK_NONE);
+        }
+        *reinterpret_cast<uint4*>(&s.skey[hn + 4u * lane]) = make_uint4(sk[0], sk[1], sk[2], sk[3]);
+        *reinterpret_cast<ushort4*>(&s.chg[hn + 4u * lane]) = make_ushort4(chg[0], chg[1], chg[2], chg[3]);
       }
+      __syncwarp();  // the staged chunk is visible to every lane
 
       // ================================================================== cluster the window of chunk ci - 1
       if (ci > c0) {
         const uint32_t hb = hn ^ HC;                 // ring half of the home chunk
-        const uint32_t b = T0 + (ci - 1u) * HC;      // global index of window slot 0
+        const uint32_t b = T0 + (ci - 1u) * HC;      // global index of the home chunk's word 0
         const uint32_t R = cur.R;
-        uint32_t f_t = MAXT, e_t = 0u;               // window = slots [f_t, e_t); empty when nothing is owned
+        uint32_t f_t = MAXT, e_t = 0u;               // window = chunk slots [f_t, e_t); empty when nothing is owned
         uint32_t Rown = R;                           // runs of the window (the last run may be left to findrun)
         if (R) {
           f_t = cur.fs;
@@ -280,7 +361,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             e_t = gEnd - b;
           } else {  // the last run does not end inside the next chunk: the warp-per-run kernel takes it
             e_t = cur.ls;
-            if (lane == (e_t & 31u)) {
+            if (lane == 0) {
               const uint32_t er = cur.one_event ? cur.er0 : event_of(c, S, sgc, b + e_t);
               push_run(c, c.mid_list, CTL_MID_COUNT, er, c.d_module[b + e_t]);
             }
@@ -288,8 +369,10 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             if (e_t == f_t) { f_t = MAXT; e_t = 0u; }  // it was the only run
           }
         }
-        const bool owns = e_t > f_t;
-        if (owns) {
+        if (e_t > f_t) {
+          // window slot t <-> chunk slot f_t + t <-> ring entry (hb + f_t + t) & 255 <-> word wb + t
+          const uint32_t len = e_t - f_t, nk = (len + 31u) >> 5, pb = hb + f_t, wb = b + f_t;
+          const uint32_t nhome = HC - f_t;  // window slots of the home chunk; the rest is the head of the next chunk
           // ============================================================== B: clear; run tables; insert
           {
             uint4* t4 = reinterpret_cast<uint4*>(s.tab);
@@ -302,21 +385,20 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           __syncwarp();  // the cleared hash is visible
           if (Rown > RC && lane == 0) s.run_bad[RC + 1u] = 1;  // the runs beyond RC are all "run RC + 1"
           bool dup_seen = false;
-          const uint32_t k0 = f_t >> 5, kl = (e_t + 31u) >> 5;  // rounds k0 .. kl-1 hold the window
           const uint32_t Rr = R <= RC ? R : RC + 1u;             // run of the slots of the next chunk
 #pragma unroll 1
-          for (uint32_t k = k0; k < kl; ++k) {
-            const uint32_t t = 32u * k + lane, ph = (hb + t) & (MAXT - 1u);
+          for (uint32_t k = 0; k < nk; ++k) {
+            const uint32_t t = 32u * k + lane, ph = (pb + t) & (MAXT - 1u);
             uint32_t sk = s.skey[ph];
-            const bool dec = t >= f_t && t < e_t && sk < SK_BAD;
-            if (k >= 4u && dec) { sk |= Rr << SK_RUN_SHIFT; s.skey[ph] = sk; }  // the head of the next chunk: the rest of run R
+            const bool dec = t < len && sk < SK_BAD;
+            if (t >= nhome && dec) { sk |= Rr << SK_RUN_SHIFT; s.skey[ph] = sk; }  // the head of the next chunk: the rest of run R
             const uint32_t r = (sk >> SK_RUN_SHIFT) & 63u;
             if (dec && (sk & SK_START)) {
-              const uint32_t er = cur.one_event ? cur.er0 : event_of(c, S, sgc, b + t);
-              const uint32_t m = c.d_module[b + t];  // written by this thread when it decoded the word
+              const uint32_t er = cur.one_event ? cur.er0 : event_of(c, S, sgc, wb + t);
+              const uint32_t m = c.d_module[wb + t];  // written by this warp when it decoded the chunk
               if (r <= RC) {
                 s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | m;
-                s.run_ifirst[r] = b + t - (cur.one_event ? cur.ebase0 : segB[er * F]);
+                s.run_ifirst[r] = wb + t - (cur.one_event ? cur.ebase0 : segB[er * F]);
               } else {
                 push_run(c, c.mid_list, CTL_MID_COUNT, er, m);  // too many runs: left to findrun
               }
@@ -334,9 +416,9 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
 
           // ============================================================== D: duplicates; neighbours -> edges -> unions
           if (__any_sync(FULL, dup_seen)) {  // rare: some pixel appears twice; the digi not in the slot is a DUPLICATE (S10)
-            for (uint32_t k = k0; k < kl; ++k) {
-              const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
-              const bool dec = t >= f_t && t < e_t && sk < SK_BAD && ((sk >> SK_RUN_SHIFT) & 63u) <= RC;
+            for (uint32_t k = 0; k < nk; ++k) {
+              const uint32_t t = 32u * k + lane, sk = s.skey[(pb + t) & (MAXT - 1u)];
+              const bool dec = t < len && sk < SK_BAD && ((sk >> SK_RUN_SHIFT) & 63u) <= RC;
               if (dec && PH::digi(PH::find(s.tab, PH::mix(sk & SK_KEY))) != t) s.label[t] = MARK_DUP;
             }
             __syncwarp();
@@ -345,11 +427,10 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           // are joined to it by their own E edges, so d-S alone is enough; when E is live, SE is E's S neighbour.
           uint32_t ne = 0u;
 #pragma unroll 1
-          for (uint32_t k = k0; k < kl; ++k) {
-            const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
-            if (ne + 96u > ECAP) {  // the round's edges might not fit: unite what is listed (warp-uniform)
+          for (uint32_t k = 0; k <= nk; ++k) {
+            if (k == nk || ne + 96u > ECAP) {  // the last round is done, or the next round's edges might not fit: unite what is listed
               __syncwarp();
-              for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {
+              for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
                 if (i0 + lane < ne) {
                   const uint32_t e = s.edge[i0 + lane];
                   hook(s.label, e & 0xFFu, e >> 8);
@@ -357,8 +438,10 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
                 __syncwarp();
               }
               ne = 0u;
+              if (k == nk) break;
             }
-            const bool live = s.label[t] < MAXT;  // slots outside the window and undecodable words carry MARK_BELOW
+            const uint32_t t = 32u * k + lane, sk = s.skey[(pb + t) & (MAXT - 1u)];
+            const bool live = s.label[t] < MAXT;  // slots beyond the window and undecodable words carry MARK_BELOW
             bool f0 = false, f1 = false, f2 = false;
             uint32_t n0 = 0, n1 = 0, n2 = 0;
             if (live) {
@@ -378,17 +461,9 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             if (f2) s.edge[ne + __popc(m2 & lt_mask)] = (uint16_t)(t | (n2 << 8));
             ne += __popc(m2);
           }
-          __syncwarp();
-          for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
-            if (i0 + lane < ne) {
-              const uint32_t e = s.edge[i0 + lane];
-              hook(s.label, e & 0xFFu, e >> 8);
-            }
-            __syncwarp();
-          }
 #pragma unroll 1
           for (int pass = 0; pass < PIX_JUMPS; ++pass) {  // pointer jumping: the chains shrink before the sums
-            for (uint32_t k = k0; k < kl; ++k) {
+            for (uint32_t k = 0; k < nk; ++k) {
               const uint32_t t = 32u * k + lane;
               const uint32_t l = s.label[t];
               if (l < MAXT) { const uint32_t ll = s.label[l]; if (ll != l) s.label[t] = ll; }
@@ -406,7 +481,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           __syncwarp();
           uint32_t nr = 0u;  // roots so far
 #pragma unroll 1
-          for (uint32_t k = k0; k < kl; ++k) {
+          for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane;
             volatile uint32_t* L = s.label;
             uint32_t r = L[t];
@@ -414,7 +489,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             if (live) {
               while (true) { const uint32_t n = L[r]; if (n == r) break; r = n; }
               L[t] = r;  // flatten: r is the root, so other walkers through t stay correct
-              const uint32_t ph = (hb + t) & (MAXT - 1u);
+              const uint32_t ph = (pb + t) & (MAXT - 1u);
               const uint32_t sk = s.skey[ph], e = s.chg[ph];
               atomicAdd(&qn[r], e | (1u << 24));  // charge sum (< 2^24: 256 * 65535) | pixel count (256 wraps to 0)
               atomicAdd(&sx[r], e * (sk & 511u));
@@ -431,14 +506,14 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           {
             uint32_t cnt = 0u;                   // surviving roots before this iteration
             uint32_t run_c = 0u, base_c = 0u;    // the run of the last root so far and the survivors before that run
-            const uint32_t relb = b - gBeg;      // may wrap for the first chunk; only used added to a slot >= gBeg - b
+            const uint32_t relb = wb - gBeg;     // launch-group index of window slot 0
 #pragma unroll 1
             for (uint32_t i0 = 0u; i0 < nr; i0 += 32u) {
               const bool valid = i0 + lane < nr;
               uint32_t t = 0u, r = 0u, Q = 0u, np = 0u;
               if (valid) {
                 t = rlist[i0 + lane];
-                r = (s.skey[(hb + t) & (MAXT - 1u)] >> SK_RUN_SHIFT) & 63u;
+                r = (s.skey[(pb + t) & (MAXT - 1u)] >> SK_RUN_SHIFT) & 63u;
                 const uint32_t v = qn[t];
                 Q = v & 0xFFFFFFu; np = v >> 24;
                 if (np == 0u) np = 256u;
@@ -450,7 +525,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
               // runs are contiguous in digi order: the first lane of this lane's run in this iteration
               const uint32_t rprev = __shfl_up_sync(FULL, r, 1);
               const uint32_t bnd = __ballot_sync(FULL, valid && (lane == 0u || r != rprev));
-              const uint32_t fl = 31u - (uint32_t)__clz(bnd & le_mask);  // bit 0 of bnd is set whenever lane 0 is valid
+              const uint32_t fl = 31u - (uint32_t)__clz(bnd & le_mask);  // bit 0 of bnd is set: lane 0 is valid
               uint32_t base = cnt + __popc(sm & ((1u << fl) - 1u));
               if (fl == 0u && r == run_c) base = base_c;  // the run began in an earlier iteration
               if (valid) {
@@ -479,19 +554,13 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             if (s.run_bad[r]) push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);
             else c.n_clus[(key >> 16) * c.M + (key & 0xFFFFu)] = s.run_cnt[r];
           }
-        }
 
-        // ================================================================== G: final status and clus, counters
-        {
-          const uint32_t kl = owns ? (e_t + 31u) >> 5 : 0u;
-          const uint32_t kg = kl > 4u ? kl : 4u;
+          // ============================================================== G: final status and clus, counters
           uint32_t cntA = 0u, cntB = 0u, n_pre = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
 #pragma unroll 1
-          for (uint32_t k = 0; k < kg; ++k) {
-            const uint32_t t = 32u * k + lane, sk = s.skey[(hb + t) & (MAXT - 1u)];
-            if (sk >= SK_BAD) {
-              if (k < 4u && sk != SK_NONE) { c.d_status[b + t] = (uint8_t)(sk & 0xFFu); c.d_clus[b + t] = -1; }  // undecodable: finished here
-            } else if (t >= f_t && t < e_t && !s.run_bad[(sk >> SK_RUN_SHIFT) & 63u]) {
+          for (uint32_t k = 0; k < nk; ++k) {
+            const uint32_t t = 32u * k + lane, sk = s.skey[(pb + t) & (MAXT - 1u)];
+            if (t < len && sk < SK_BAD && !s.run_bad[(sk >> SK_RUN_SHIFT) & 63u]) {
               const uint32_t lab = s.label[t];
               uint32_t so; int32_t cl = -1;
               if (lab == MARK_DUP) { so = ST_DUP; cntA += 1u; }
@@ -501,7 +570,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
                 if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
                 n_pre += lab == t ? 1u : 0u;
               }
-              c.d_status[b + t] = (uint8_t)so; c.d_clus[b + t] = cl;
+              c.d_status[wb + t] = (uint8_t)so; c.d_clus[wb + t] = cl;
               if (!cur.one_event) {  // rare: an event boundary inside the chunk; every digi counts for its own event
                 uint32_t* ec = c.ev_cnt + (size_t)(s.run_key[(sk >> SK_RUN_SHIFT) & 63u] >> 16) * EC_STRIDE;
                 atomicAdd(ec + (so == ST_DUP ? EC_DUP : (so == ST_BELOW ? EC_BELOW : (so == ST_OK ? EC_OK : EC_CUT))), 1u);
@@ -513,8 +582,8 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             if (cur.er0 != acc_ev) { flush(); acc_ev = cur.er0; }
             accA += cntA; accB += cntB; accP += n_pre;
           }
+          __syncwarp();  // shared state is rewritten by the next window
         }
-        __syncwarp();  // shared state is rewritten by the next window
       }
       if (ci >= c1) break;
       cur = nxt; sgc = sgn;
