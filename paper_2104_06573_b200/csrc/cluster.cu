@@ -245,7 +245,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
   }
   n_dup = g.sum(n_dup); n_below = g.sum(n_below); n_ok = g.sum(n_ok); n_cut = g.sum(n_cut);
   if (rk == 0) {
-    c.n_clus[task] = n_post;
+    if (n_post) atomicAdd(c.n_clus + task, n_post);
     uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
     atomicAdd(ec + EC_PRECUT, n_pre); atomicAdd(ec + EC_DUP, n_dup); atomicAdd(ec + EC_BELOW, n_below);
     atomicAdd(ec + EC_OK, n_ok); atomicAdd(ec + EC_CUT, n_cut);
@@ -287,7 +287,7 @@ __global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_cons
     if (t >= count) break;
     const uint32_t task = c.ovf_list[t];
     const uint32_t er = task / c.M, m = task - er * c.M;
-    if (c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] & FLAG_NONCONTIGUOUS) continue;  // S11: not clustered
+    if (module_split(c, er, m)) continue;  // S11: the module has several runs; the event is not clustered
     const uint32_t first = c.module_first[(size_t)(c.e0 + er) * c.M + m];
     if (c.module_end[(size_t)(c.e0 + er) * c.M + m] - first <= SMEM_CAP) {
       cluster_task<BlockGroup<OVF_THREADS>, uint32_t, true>(c, g, carve(ovf_smem, SMEM_CAP), task);

@@ -7,6 +7,7 @@
 // scatter: a persistent grid takes slices from the list; a block stages the event's offsets in shared memory
 // and copies its records, one thread per output record, module found by binary search in the shared offsets.
 #include "pix_common.cuh"
+#include "pix_device.cuh"
 
 namespace pix {
 
@@ -31,16 +32,20 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
   __shared__ uint32_t s_red[8];
   const uint32_t er = blockIdx.x, e = c.e0 + er, M = c.M;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  const uint32_t flags = c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS];
-  const bool skip = (flags & FLAG_NONCONTIGUOUS) != 0;  // S11: clustering is not defined for such an event
-  const uint32_t* n_clus = c.n_clus + (size_t)er * M;
+  const uint32_t* n_clus_raw = c.n_clus + (size_t)er * M;  // runs << 24 | clusters surviving the cut
+  // S11: a module with two or more runs makes the event NONCONTIGUOUS; clustering is not defined for such an event
+  bool split = false;
+  for (uint32_t m = tid; m < M; m += FIN_THREADS) split |= n_clus_raw[m] >= 2u * NCLUS_RUN;
+  const bool skip = __syncthreads_or(split);
+  const uint32_t flags = c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] | (skip ? FLAG_NONCONTIGUOUS : 0u);
+  auto n_clus = [&](uint32_t m) { return n_clus_raw[m] & NCLUS_MASK; };
 
   // ---- Fig. 3 clamp + exclusive prefix sum over the M modules
   const uint32_t ipt = (M + FIN_THREADS - 1) / FIN_THREADS;
   const uint32_t m0 = tid * ipt, m1 = (m0 + ipt < M) ? m0 + ipt : M;
   uint32_t local = 0;
   for (uint32_t m = m0; m < m1; ++m) {
-    const uint32_t n = skip ? 0u : n_clus[m];
+    const uint32_t n = skip ? 0u : n_clus(m);
     local += n < c.cap_mod ? n : c.cap_mod;
   }
   const uint32_t incl = warp_inclusive_scan(local, lane);
@@ -51,7 +56,7 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
   for (uint32_t w = 0; w < warp; ++w) base += s_warp[w];
   for (uint32_t m = m0; m < m1; ++m) {
     s_start[m] = base;
-    const uint32_t n = skip ? 0u : n_clus[m];
+    const uint32_t n = skip ? 0u : n_clus(m);
     base += n < c.cap_mod ? n : c.cap_mod;
   }
   if (m0 < M && m1 == M) s_start[M] = base;
@@ -83,7 +88,7 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
     const bool present = c.module_end[(size_t)e * M + m] > 0u;
     if (!present) c.module_first[(size_t)e * M + m] = 0u;  // S12: absent -> 0,0 (init left the atomicMin sentinel)
     acc[0] += present ? 1u : 0u;
-    acc[1] += skip ? 0u : n_clus[m];
+    acc[1] += skip ? 0u : n_clus(m);
   }
 #pragma unroll
   for (int k = 0; k < 4; ++k) {

@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
     if (ti >= count) break;
     const uint32_t task = in_list[ti];
     const uint32_t er = task / c.M, m = task - er * c.M;
-    if (c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] & FLAG_NONCONTIGUOUS) continue;  // S11: not clustered
+    if (module_split(c, er, m)) continue;  // S11: the module has several runs; the event is not clustered
     const size_t mo = (size_t)(c.e0 + er) * c.M + m;
     const uint32_t first = c.module_first[mo], n = c.module_end[mo] - first;
     if (n > RMAX) {  // too long for this size of the kernel: the next one takes it
@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
     }
     const uint32_t a = __reduce_add_sync(FULL, cntA), bb = __reduce_add_sync(FULL, cntB);
     if (lane == 0) {
-      c.n_clus[task] = cnt;
+      if (cnt) atomicAdd(c.n_clus + task, cnt);
       uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
       if (a & 0xFFFFu) atomicAdd(ec + EC_DUP, a & 0xFFFFu);
       if (a >> 16) atomicAdd(ec + EC_BELOW, a >> 16);
