@@ -35,7 +35,10 @@ namespace {
 #define PIX_BPS 7
 #endif
 #ifndef PIX_JUMPS
-#define PIX_JUMPS 1
+#define PIX_JUMPS 2
+#endif
+#ifndef PIX_UB
+#define PIX_UB 1
 #endif
 #ifndef PIX_UD
 #define PIX_UD 1
@@ -52,7 +55,7 @@ namespace {
 #ifndef PIX_GMAX
 #define PIX_GMAX 32
 #endif
-constexpr int U_UD = PIX_UD, U_UE = PIX_UE, U_UF = PIX_UF, U_UG = PIX_UG;
+constexpr int U_UB = PIX_UB, U_UD = PIX_UD, U_UE = PIX_UE, U_UG = PIX_UG;
 constexpr int WPB = PIX_WPB;              // warps per block (they share nothing but the block)
 constexpr int FT = WPB * 32;
 constexpr int BLOCKS_PER_SM = PIX_BPS;
@@ -123,7 +126,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
   uint32_t* const qn = s.tab; uint32_t* const sx = s.tab + MAXT; uint32_t* const sy = s.tab + 2 * MAXT;
   uint8_t* const rlist = reinterpret_cast<uint8_t*>(s.tab + 3 * MAXT);  // roots in digi order (after phase D)
   uint16_t* const lid = s.edge;
-  uint32_t G = n_chunks / (gridDim.x * WPB * 4u);  // about four tickets per warp
+  uint32_t G = n_chunks / (gridDim.x * WPB * 6u);  // about six tickets per warp
   G = G < 1u ? 1u : (G > GMAX ? GMAX : G);
 
   // per-event counters of the digis this lane has finished: dup | below << 16, ok | cut << 16, roots
@@ -386,7 +389,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           if (Rown > RC && lane == 0) s.run_bad[RC + 1u] = 1;  // the runs beyond RC are all "run RC + 1"
           bool dup_seen = false;
           const uint32_t Rr = R <= RC ? R : RC + 1u;             // run of the slots of the next chunk
-#pragma unroll 1
+#pragma unroll U_UB
           for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane, ph = (pb + t) & (MAXT - 1u);
             uint32_t sk = s.skey[ph];
@@ -426,7 +429,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE
           // are joined to it by their own E edges, so d-S alone is enough; when E is live, SE is E's S neighbour.
           uint32_t ne = 0u;
-#pragma unroll 1
+#pragma unroll U_UD
           for (uint32_t k = 0; k <= nk; ++k) {
             if (k == nk || ne + 96u > ECAP) {  // the last round is done, or the next round's edges might not fit: unite what is listed
               __syncwarp();
@@ -446,8 +449,15 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             uint32_t n0 = 0, n1 = 0, n2 = 0;
             if (live) {
               const uint32_t h = PH::mix(sk & SK_KEY);
-              const uint32_t eE = PH::find(s.tab, PH::step(h, 1u)), eS = PH::find(s.tab, PH::step(h, 512u));
-              const uint32_t eSW = PH::find(s.tab, PH::step(h, 511u)), eSE = PH::find(s.tab, PH::step(h, 513u));
+              bool o0, o1, o2, o3;  // one branch for the four lookups: a full home bucket without a match is rare
+              uint32_t eE = PH::find_home(s.tab, PH::step(h, 1u), o0), eS = PH::find_home(s.tab, PH::step(h, 512u), o1);
+              uint32_t eSW = PH::find_home(s.tab, PH::step(h, 511u), o2), eSE = PH::find_home(s.tab, PH::step(h, 513u), o3);
+              if (o0 | o1 | o2 | o3) {
+                if (o0) eE = PH::find_slow(s.tab, PH::step(h, 1u));
+                if (o1) eS = PH::find_slow(s.tab, PH::step(h, 512u));
+                if (o2) eSW = PH::find_slow(s.tab, PH::step(h, 511u));
+                if (o3) eSE = PH::find_slow(s.tab, PH::step(h, 513u));
+              }
               const bool hS = PH::live(eS);
               f0 = PH::live(eE); n0 = PH::digi(eE);
               f1 = hS || PH::live(eSW); n1 = PH::digi(hS ? eS : eSW);
@@ -480,7 +490,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           }
           __syncwarp();
           uint32_t nr = 0u;  // roots so far
-#pragma unroll 1
+#pragma unroll U_UE
           for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane;
             volatile uint32_t* L = s.label;
@@ -557,7 +567,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
 
           // ============================================================== G: final status and clus, counters
           uint32_t cntA = 0u, cntB = 0u, n_pre = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
-#pragma unroll 1
+#pragma unroll U_UG
           for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane, sk = s.skey[(pb + t) & (MAXT - 1u)];
             if (t < len && sk < SK_BAD && !s.run_bad[(sk >> SK_RUN_SHIFT) & 63u]) {

@@ -105,6 +105,7 @@ struct BucketHash {
   static __device__ __forceinline__ uint32_t step(uint32_t h, uint32_t d) { return (h + d * HASH_MUL) & KEY_MASK; }
 
   // 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets.
+  // (Looking at the bucket first and aiming one atomicCAS at its first free slot was measured slower.)
   static __device__ __noinline__ uint32_t insert(uint32_t* tab, uint32_t key, uint32_t t, uint32_t below) {
     const uint32_t h = mix(key), tag = h & TAG_MASK;
     uint32_t p = (h >> TAG_BITS) * 4u, res = 2u;
@@ -141,6 +142,13 @@ struct BucketHash {
     const uint4 e = *reinterpret_cast<const uint4*>(&tab[(h >> TAG_BITS) * 4u]);
     uint32_t r = match4(e, h & TAG_MASK);
     if (r == EMPTY && e.w != EMPTY) r = find_slow(tab, h);  // home bucket full, no match (rare): displaced keys
+    return r;
+  }
+  // the home bucket only; full = the bucket has no free slot, so a key that is not in it may sit in the next buckets
+  static __device__ __forceinline__ uint32_t find_home(const uint32_t* tab, uint32_t h, bool& full) {
+    const uint4 e = *reinterpret_cast<const uint4*>(&tab[(h >> TAG_BITS) * 4u]);
+    const uint32_t r = match4(e, h & TAG_MASK);
+    full = r == EMPTY && e.w != EMPTY;
     return r;
   }
   static __device__ __forceinline__ uint32_t digi(uint32_t e) { return (e >> 1) & DIGI_MASK; }
