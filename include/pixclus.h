@@ -61,9 +61,18 @@ enum {
   PIX_SUM_N_CUT_DIGIS, PIX_SUM_N_MODULES_PRESENT, PIX_SUM_N_CLUSTERS_PRECUT, PIX_SUM_N_CLUSTERS,
   PIX_SUM_N_CLUSTERS_EMITTED, PIX_SUM_FLAGS
 };
-#define PIX_FLAG_NONCONTIGUOUS 1u             /* some module's words form more than one run (S11) */
+#define PIX_FLAG_NONCONTIGUOUS 1u             /* some module's words form more than one run (S11): the event is not clustered.
+                                                 Every decodable word gets status BELOW_THRESHOLD or CUT and clus = -1, the
+                                                 counters follow (no duplicates, no OK digis, no clusters); decode fields,
+                                                 module_first / module_end and n_modules_present are as for any event */
 #define PIX_FLAG_CLUSTER_CAPACITY_OVERFLOW 2u /* more clusters than max_clusters_per_event; the rest are dropped */
-#define PIX_FLAG_EVENT_TOO_LARGE 4u           /* batch only: event longer than max_words_per_event, skipped */
+#define PIX_FLAG_EVENT_TOO_LARGE 4u           /* batch only: the event is longer than max_words_per_event, its offsets are not
+                                                 ascending, or it reaches beyond the word capacity of its launch group
+                                                 (chunk_events x max_words_per_event words counted from the group's first
+                                                 word).  The words inside the capacity are processed as usual -- a long
+                                                 event that fits its group is complete -- and the outputs of the words beyond
+                                                 it are NOT written (the one exception to "every element is written").
+                                                 A batch whose events all respect max_words_per_event never raises it. */
 
 typedef struct pix_handle pix_handle;
 
@@ -144,7 +153,11 @@ int pix_process_batch(pix_handle* h, void* cuda_stream, uint32_t n_events, const
 
 /* Same as pix_process_batch but every pointer is a HOST pointer (pinned memory recommended): copies the
  * inputs to library-owned device staging, runs the path, copies every non-NULL output array back and
- * synchronises cuda_stream before returning.  Staging is allocated on first use (sized by the capacities). */
+ * synchronises cuda_stream before returning (on an error too: nothing is in flight when the call returns).
+ * Any output array pointer may be NULL: that array is not copied (e.g. all digi arrays NULL: clusters only).
+ * Cluster records travel as rows of max(n_clusters_emitted) over the events of a launch group, so record
+ * elements at and beyond an event's n_clusters_emitted are UNSPECIFIED after this call (not "untouched").
+ * Staging is allocated on first use (sized by the capacities). */
 int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* raw_words,
                            uint32_t n_words_total, const uint32_t* event_word_offsets, const uint32_t* fed_offsets,
                            const pix_digis* out_digis, const pix_clusters* out_clusters);
@@ -174,13 +187,16 @@ int pix_rechits(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint3
 /* Number of CUDA kernels this handle has launched so far (for launch accounting). */
 uint64_t pix_kernel_launches(const pix_handle* h);
 
+/* Device->host bytes the last pix_process_batch_host call on this handle copied (for transfer accounting). */
+uint64_t pix_host_bytes_out(const pix_handle* h);
+
 /* Diagnostic: module runs the LAST internal chunk of the last call left to the overflow kernel (runs longer than the
  * warp kernels' windows, pathological charge sums).  Synchronises the device; not for the hot path. */
 int pix_overflow_runs(pix_handle* h, uint32_t* out);
 
 /* Optional per-kernel timing for benchmarks (not legal during stream capture).  While enabled, every chunk
  * records CUDA events between its kernels on the caller's stream.  pix_read_profile waits for them and adds up
- * the device time per kernel since the last read: ms_out[8] = {init, decode, findclus, findrun, overflow, finalize, 0, 0};
+ * the device time per kernel since the last read: ms_out[8] = {init, fused, findrun, overflow, finalize, 0, 0, 0};
  * *n_chunks_out = chunks covered. */
 int pix_set_profiling(pix_handle* h, int enable);
 int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out);

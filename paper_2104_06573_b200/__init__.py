@@ -25,7 +25,7 @@ SUMMARY = ("n_words", "n_decoded", "n_empty", "n_err_link", "n_err_roc", "n_err_
 FLAG_NONCONTIGUOUS, FLAG_CLUSTER_CAPACITY_OVERFLOW, FLAG_EVENT_TOO_LARGE = 1, 2, 4
 EXPORTS = ("pix_create", "pix_clone", "pix_destroy", "pix_process", "pix_process_batch", "pix_process_batch_host",
            "pix_rechits", "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile",
-           "pix_overflow_runs")
+           "pix_overflow_runs", "pix_host_bytes_out")
 
 _vp, _u32 = ctypes.c_void_p, ctypes.c_uint32
 
@@ -82,6 +82,8 @@ def load() -> ctypes.CDLL:
             getattr(lib, f).restype = ctypes.c_int
         lib.pix_kernel_launches.argtypes = [_vp]
         lib.pix_kernel_launches.restype = ctypes.c_uint64
+        lib.pix_host_bytes_out.argtypes = [_vp]
+        lib.pix_host_bytes_out.restype = ctypes.c_uint64
         lib.pix_set_profiling.argtypes = [_vp, ctypes.c_int]
         lib.pix_set_profiling.restype = ctypes.c_int
         lib.pix_read_profile.argtypes = [_vp, pp(ctypes.c_float), pp(_u32)]
@@ -169,6 +171,10 @@ def pix_last_error(h: Handle) -> str:
 
 def pix_kernel_launches(h: Handle) -> int:
     return int(load().pix_kernel_launches(h.ptr))
+
+
+def pix_host_bytes_out(h: Handle) -> int:
+    return int(load().pix_host_bytes_out(h.ptr))
 
 
 def pix_overflow_runs(h: Handle) -> int:

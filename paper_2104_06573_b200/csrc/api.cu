@@ -33,7 +33,8 @@ struct HostStage {  // device staging of pix_process_batch_host, allocated on fi
   uint32_t *module_first = nullptr, *module_end = nullptr, *clus_module_start = nullptr, *summary = nullptr;
   std::vector<void*> allocs;
   cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of the pipelined host path
-  std::vector<cudaEvent_t> ev;                   // two per launch group: input landed, group computed
+  std::vector<cudaEvent_t> ev;                   // three per launch group: input landed, group computed, summaries landed
+  uint32_t* h_summary = nullptr;                 // pinned host copy of the summaries (sizes the record copies)
 };
 
 }  // namespace
@@ -48,6 +49,7 @@ struct pix_handle {
   void* ws = nullptr;  // one allocation, carved below
   pix::Chunk proto{};  // tables, params and workspace pointers filled once
   uint64_t launches = 0;
+  uint64_t hs_d2h_bytes = 0;  // device->host bytes of the last pix_process_batch_host call
   std::string err;
   HostStage hs;
   bool profiling = false;
@@ -84,6 +86,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
   c.n_clus = (uint32_t*)take(Ec * M * 4);
+  c.n_runs = (uint32_t*)take(Ec * M * 4);
   c.t_a = (uint4*)take(W * sizeof(uint4));
   c.t_y = (float*)take(W * sizeof(float));
   c.g_hash = (unsigned long long*)take(W * 16);
@@ -224,7 +227,7 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   for (uint32_t sh = 0; sh < 17; ++sh) if ((1u << sh) == F) c.F_shift = sh;
   c.vcal_gain = params->vcal_gain; c.vcal_offset = params->vcal_offset; c.max_e_f = (float)params->max_electrons;
   c.thr = params->pixel_threshold_e; c.cut = params->cluster_charge_cut_e;
-  c.cap_mod = params->max_clusters_per_module; c.cap_ev = params->max_clusters_per_event; c.cap_words = h->cap_words;
+  c.cap_mod = params->max_clusters_per_module; c.cap_ev = params->max_clusters_per_event; c.cap_words = h->cap_words; c.max_wpe = params->max_words_per_event;
   if (make_workspace(h) != PIX_OK) { release_tables(t); delete h; return PIX_ERR_ALLOC; }
   *out = h;
   return PIX_OK;
@@ -247,6 +250,7 @@ int pix_destroy(pix_handle* h) {
   if (!h) return PIX_ERR_INVALID_ARG;
   cudaFree(h->ws);
   for (void* p : h->hs.allocs) cudaFree(p);
+  if (h->hs.h_summary) cudaFreeHost(h->hs.h_summary);
   for (cudaEvent_t x : h->hs.ev) cudaEventDestroy(x);
   if (h->hs.s_in) cudaStreamDestroy(h->hs.s_in);
   if (h->hs.s_out) cudaStreamDestroy(h->hs.s_out);
@@ -307,10 +311,7 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
   if (h->F > 1 && !fed_offsets) return fail(h, PIX_ERR_INVALID_ARG, "fed_offsets is NULL but n_feds > 1");
   if (n_events > h->p.max_events_per_batch) return fail(h, PIX_ERR_CAPACITY, "n_events > max_events_per_batch");
   if ((uint64_t)n_words_total > h->cap_total) return fail(h, PIX_ERR_CAPACITY, "n_words_total > capacity");
-  if (!od->module || !od->row || !od->col || !od->charge || !od->clus || !od->status || !oc->module || !oc->first_digi ||
-      !oc->n_pix || !oc->charge || !oc->x_col || !oc->y_row || !oc->module_first || !oc->module_end ||
-      !oc->clus_module_start || !oc->summary)
-    return fail(h, PIX_ERR_INVALID_ARG, "an output array is NULL");
+  const bool want_rec = oc->module || oc->first_digi || oc->n_pix || oc->charge || oc->x_col || oc->y_row;
   HostStage& s = h->hs;
   const size_t E = h->p.max_events_per_batch, W = (size_t)h->cap_total, M = h->M, F = h->F, K = h->p.max_clusters_per_event;
   if (!s.ready) {
@@ -319,16 +320,18 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
       void* p = nullptr;
       if (!ok) return p;
       if (cudaMalloc(&p, bytes ? bytes : 16) != cudaSuccess) { ok = false; cudaGetLastError(); return (void*)nullptr; }
+      cudaMemset(p, 0, bytes ? bytes : 16);  // record slots beyond n_clusters_emitted may be copied out: never uninitialised memory
       s.allocs.push_back(p);
       return p;
     };
-    s.words = (uint32_t*)dev(W * 4); s.ev_off = (uint32_t*)dev((E + 1) * 4); s.fed_off = (uint32_t*)dev(E * (F + 1) * 4);
-    s.d_module = (uint16_t*)dev(W * 2); s.d_row = (uint16_t*)dev(W * 2); s.d_col = (uint16_t*)dev(W * 2);
-    s.d_charge = (int32_t*)dev(W * 4); s.d_clus = (int32_t*)dev(W * 4); s.d_status = (uint8_t*)dev(W);
+    s.words = (uint32_t*)dev(W * 4 + 64); s.ev_off = (uint32_t*)dev((E + 1) * 4); s.fed_off = (uint32_t*)dev(E * (F + 1) * 4);
+    s.d_module = (uint16_t*)dev(W * 2 + 64); s.d_row = (uint16_t*)dev(W * 2 + 64); s.d_col = (uint16_t*)dev(W * 2 + 64);
+    s.d_charge = (int32_t*)dev(W * 4 + 64); s.d_clus = (int32_t*)dev(W * 4 + 64); s.d_status = (uint8_t*)dev(W + 64);
     s.c_module = (uint16_t*)dev(E * K * 2); s.c_first = (uint32_t*)dev(E * K * 4); s.c_npix = (uint32_t*)dev(E * K * 4);
     s.c_charge = (uint32_t*)dev(E * K * 4); s.c_x = (float*)dev(E * K * 4); s.c_y = (float*)dev(E * K * 4);
     s.module_first = (uint32_t*)dev(E * M * 4); s.module_end = (uint32_t*)dev(E * M * 4);
     s.clus_module_start = (uint32_t*)dev(E * (M + 1) * 4); s.summary = (uint32_t*)dev(E * 16 * 4);
+    if (ok && cudaMallocHost(&s.h_summary, E * 16 * 4) != cudaSuccess) { ok = false; cudaGetLastError(); s.h_summary = nullptr; }
     if (!ok) { for (void* p : s.allocs) cudaFree(p); s.allocs.clear(); return fail(h, PIX_ERR_ALLOC, "staging allocation failed"); }
     s.ready = true;
   }
@@ -347,60 +350,90 @@ int pix_process_batch_host(pix_handle* h, void* cuda_stream, uint32_t n_events, 
   if (ge < 1u) ge = 1u;
   if (ge > h->chunk_events) ge = h->chunk_events;
   const uint32_t n_groups = (n_events + ge - 1u) / ge;
-  while (s.ev.size() < 2 * (size_t)n_groups + 1) {
+  while (s.ev.size() < 3 * (size_t)n_groups + 1) {  // all events exist before the first copy is issued
     cudaEvent_t x;
     if (cudaEventCreateWithFlags(&x, cudaEventDisableTiming) != cudaSuccess) return fail(h, PIX_ERR_ALLOC, "cudaEventCreate");
     s.ev.push_back(x);
   }
   const size_t Ev = n_events;
   cudaError_t e = cudaSuccess;
+  int rc = PIX_OK;
   auto h2d = [&](void* d, const void* src, size_t bytes) { if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, s.s_in); };
   auto d2h = [&](void* dst, const void* d, size_t bytes) { if (e == cudaSuccess && dst && bytes) e = cudaMemcpyAsync(dst, d, bytes, cudaMemcpyDeviceToHost, s.s_out); };
+  // record arrays: rows of `width` elements (the most any event of the group emitted) at the per-event stride K
+  auto d2h_rec = [&](void* dst, const void* d, size_t elem, size_t k0, size_t width, size_t rows) {
+    if (e == cudaSuccess && dst && width && rows)
+      e = cudaMemcpy2DAsync((char*)dst + k0 * elem, K * elem, (const char*)d + k0 * elem, K * elem, width * elem, rows, cudaMemcpyDeviceToHost, s.s_out);
+  };
+  // the record copies of group g, once its summaries have landed in h_summary
+  auto records_of = [&](uint32_t g) {
+    if (!want_rec || e != cudaSuccess) return;
+    const uint32_t e0 = g * ge, e1 = (n_events - e0 > ge) ? e0 + ge : n_events;
+    e = cudaEventSynchronize(s.ev[3 * g + 2]);
+    if (e != cudaSuccess) return;
+    size_t width = 0;
+    for (uint32_t ev = e0; ev < e1; ++ev) { const size_t n = s.h_summary[(size_t)ev * 16 + PIX_SUM_N_CLUSTERS_EMITTED]; width = n > width ? n : width; }
+    if (width > K) width = K;
+    const size_t k0 = (size_t)e0 * K, ne = e1 - e0;
+    d2h_rec(oc->module, s.c_module, 2, k0, width, ne); d2h_rec(oc->first_digi, s.c_first, 4, k0, width, ne);
+    d2h_rec(oc->n_pix, s.c_npix, 4, k0, width, ne); d2h_rec(oc->charge, s.c_charge, 4, k0, width, ne);
+    d2h_rec(oc->x_col, s.c_x, 4, k0, width, ne); d2h_rec(oc->y_row, s.c_y, 4, k0, width, ne);
+    h->hs_d2h_bytes += width * ne * ((oc->module ? 2 : 0) + (oc->first_digi ? 4 : 0) + (oc->n_pix ? 4 : 0) + (oc->charge ? 4 : 0) + (oc->x_col ? 4 : 0) + (oc->y_row ? 4 : 0));
+  };
+  h->hs_d2h_bytes = 0;
   // the copy streams start after whatever the caller's stream holds so far
-  if (e == cudaSuccess) e = cudaEventRecord(s.ev[2 * n_groups], st);
-  if (e == cudaSuccess) e = cudaStreamWaitEvent(s.s_in, s.ev[2 * n_groups], 0);
+  if (e == cudaSuccess) e = cudaEventRecord(s.ev[3 * n_groups], st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s.s_in, s.ev[3 * n_groups], 0);
   h2d(s.ev_off, event_word_offsets, (Ev + 1) * 4);
   if (F > 1) h2d(s.fed_off, fed_offsets, Ev * (F + 1) * 4);
-  if (e != cudaSuccess) return fail_cuda(h, e, "host->device copy");
   pix_digis dd{s.d_module, s.d_row, s.d_col, s.d_charge, s.d_clus, s.d_status};
   pix_clusters dc{s.c_module, s.c_first, s.c_npix, s.c_charge, s.c_x, s.c_y, s.module_first, s.module_end, s.clus_module_start, s.summary};
   pix::Chunk c = h->proto;
   c.words = s.words; c.ev_off = s.ev_off; c.fed_off = F > 1 ? s.fed_off : nullptr; c.n_single = 0;
   bind_outputs(c, &dd, &dc);
-  for (uint32_t g = 0; g < n_groups; ++g) {
+  uint32_t g = 0;
+  for (; g < n_groups && e == cudaSuccess && rc == PIX_OK; ++g) {
     const uint32_t e0 = g * ge, e1 = (n_events - e0 > ge) ? e0 + ge : n_events;
     // host-side view of the group's word range, clamped like the device does
     size_t w0 = event_word_offsets[e0], w1 = event_word_offsets[e1];
     if (w1 > n_words_total) w1 = n_words_total;
     if (w0 > w1) w0 = w1;
     h2d(s.words + w0, raw_words + w0, (w1 - w0) * 4);
-    if (e == cudaSuccess) e = cudaEventRecord(s.ev[2 * g], s.s_in);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s.ev[2 * g], 0);
-    if (e != cudaSuccess) return fail_cuda(h, e, "host->device copy");
+    if (e == cudaSuccess) e = cudaEventRecord(s.ev[3 * g], s.s_in);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s.ev[3 * g], 0);
+    if (e != cudaSuccess) break;
     c.e0 = e0; c.e1 = e1;
     size_t bound = w1 - w0;
     if (bound > h->cap_words) bound = h->cap_words;
-    if (int rc = run_chunk(h, c, n_words_total, (uint32_t)bound, st)) return rc;
-    if (e == cudaSuccess) e = cudaEventRecord(s.ev[2 * g + 1], st);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(s.s_out, s.ev[2 * g + 1], 0);
+    rc = run_chunk(h, c, n_words_total, (uint32_t)bound, st);
+    if (rc != PIX_OK) break;
+    if (e == cudaSuccess) e = cudaEventRecord(s.ev[3 * g + 1], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s.s_out, s.ev[3 * g + 1], 0);
     const size_t nw = w1 - w0, ne = e1 - e0;
-    d2h(od->module + w0, s.d_module + w0, nw * 2); d2h(od->row + w0, s.d_row + w0, nw * 2); d2h(od->col + w0, s.d_col + w0, nw * 2);
-    d2h(od->charge + w0, s.d_charge + w0, nw * 4); d2h(od->clus + w0, s.d_clus + w0, nw * 4); d2h(od->status + w0, s.d_status + w0, nw);
-    const size_t k0 = (size_t)e0 * K;
-    d2h(oc->module + k0, s.c_module + k0, ne * K * 2); d2h(oc->first_digi + k0, s.c_first + k0, ne * K * 4);
-    d2h(oc->n_pix + k0, s.c_npix + k0, ne * K * 4); d2h(oc->charge + k0, s.c_charge + k0, ne * K * 4);
-    d2h(oc->x_col + k0, s.c_x + k0, ne * K * 4); d2h(oc->y_row + k0, s.c_y + k0, ne * K * 4);
-    d2h(oc->module_first + (size_t)e0 * M, s.module_first + (size_t)e0 * M, ne * M * 4);
-    d2h(oc->module_end + (size_t)e0 * M, s.module_end + (size_t)e0 * M, ne * M * 4);
-    d2h(oc->clus_module_start + (size_t)e0 * (M + 1), s.clus_module_start + (size_t)e0 * (M + 1), ne * (M + 1) * 4);
-    d2h(oc->summary + (size_t)e0 * 16, s.summary + (size_t)e0 * 16, ne * 16 * 4);
-    if (e != cudaSuccess) return fail_cuda(h, e, "device->host copy");
+    // the summaries first: the record copies are sized by n_clusters_emitted
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s.h_summary + (size_t)e0 * 16, s.summary + (size_t)e0 * 16, ne * 64, cudaMemcpyDeviceToHost, s.s_out);
+    if (e == cudaSuccess) e = cudaEventRecord(s.ev[3 * g + 2], s.s_out);
+    d2h(od->module ? od->module + w0 : nullptr, s.d_module + w0, nw * 2); d2h(od->row ? od->row + w0 : nullptr, s.d_row + w0, nw * 2);
+    d2h(od->col ? od->col + w0 : nullptr, s.d_col + w0, nw * 2); d2h(od->charge ? od->charge + w0 : nullptr, s.d_charge + w0, nw * 4);
+    d2h(od->clus ? od->clus + w0 : nullptr, s.d_clus + w0, nw * 4); d2h(od->status ? od->status + w0 : nullptr, s.d_status + w0, nw);
+    d2h(oc->module_first ? oc->module_first + (size_t)e0 * M : nullptr, s.module_first + (size_t)e0 * M, ne * M * 4);
+    d2h(oc->module_end ? oc->module_end + (size_t)e0 * M : nullptr, s.module_end + (size_t)e0 * M, ne * M * 4);
+    d2h(oc->clus_module_start ? oc->clus_module_start + (size_t)e0 * (M + 1) : nullptr, s.clus_module_start + (size_t)e0 * (M + 1), ne * (M + 1) * 4);
+    h->hs_d2h_bytes += nw * ((od->module ? 2 : 0) + (od->row ? 2 : 0) + (od->col ? 2 : 0) + (od->charge ? 4 : 0) + (od->clus ? 4 : 0) + (od->status ? 1 : 0)) +
+                       ne * ((oc->module_first ? M * 4 : 0) + (oc->module_end ? M * 4 : 0) + (oc->clus_module_start ? (M + 1) * 4 : 0) + 64);
+    if (g > 0) records_of(g - 1);  // the previous group's summaries have had a whole group's time to land
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s.s_out);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  if (e != cudaSuccess) return fail_cuda(h, e, "device->host copy");
+  if (e == cudaSuccess && rc == PIX_OK && g == n_groups) records_of(n_groups - 1);
+  // every exit waits for what has been issued: the copies write the caller's buffers and read its input
+  const cudaError_t e1 = cudaStreamSynchronize(s.s_in), e2 = cudaStreamSynchronize(st), e3 = cudaStreamSynchronize(s.s_out);
+  if (rc != PIX_OK) return rc;
+  if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+  if (e != cudaSuccess) { cudaGetLastError(); return fail_cuda(h, e, "pix_process_batch_host"); }
+  if (oc->summary) std::memcpy(oc->summary, s.h_summary, Ev * 64);
   return PIX_OK;
 }
+
+uint64_t pix_host_bytes_out(const pix_handle* h) { return h ? h->hs_d2h_bytes : 0; }
 
 int pix_rechits(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* event_word_offsets,
                 const pix_digis* digis, const pix_clusters* clusters, const pix_hits* out_hits) {

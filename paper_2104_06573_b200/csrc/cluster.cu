@@ -245,7 +245,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
   }
   n_dup = g.sum(n_dup); n_below = g.sum(n_below); n_ok = g.sum(n_ok); n_cut = g.sum(n_cut);
   if (rk == 0) {
-    if (n_post) atomicAdd(c.n_clus + task, n_post);
+    c.n_clus[task] = n_post;
     uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
     atomicAdd(ec + EC_PRECUT, n_pre); atomicAdd(ec + EC_DUP, n_dup); atomicAdd(ec + EC_BELOW, n_below);
     atomicAdd(ec + EC_OK, n_ok); atomicAdd(ec + EC_CUT, n_cut);

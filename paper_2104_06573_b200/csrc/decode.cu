@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk
     const uint32_t b = rb < lo ? lo : (rb > hi ? hi : rb);
     const uint32_t en = re < b ? b : (re > hi ? hi : re);
     const uint32_t nw = en - b;
-    const uint32_t flags = (re > hi || rb > hi || re < rb || rb < lo) ? FLAG_TOO_LARGE : 0u;
+    const uint32_t flags = (re > hi || rb > hi || re < rb || rb < lo || re - rb > c.max_wpe) ? FLAG_TOO_LARGE : 0u;
     uint32_t carry = 0;
     for (uint32_t f0 = 0; f0 < c.F; f0 += 32u) {
       const uint32_t f = f0 + lane;
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk
   const uint32_t nmod = Ec * c.M;
   uint32_t* mf = c.module_first + (size_t)c.e0 * c.M;
   uint32_t* me = c.module_end + (size_t)c.e0 * c.M;
-  for (uint32_t t = tid; t < nmod; t += nth) { mf[t] = NO_INDEX; me[t] = 0u; c.n_clus[t] = 0u; }
+  for (uint32_t t = tid; t < nmod; t += nth) { mf[t] = NO_INDEX; me[t] = 0u; c.n_clus[t] = 0u; c.n_runs[t] = 0u; }
 }
 
 // chunk_seg[ci] = segment (event, FED) of the first word of 128-word chunk ci (its first word inside the launch

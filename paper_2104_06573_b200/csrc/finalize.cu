@@ -32,13 +32,13 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
   __shared__ uint32_t s_red[8];
   const uint32_t er = blockIdx.x, e = c.e0 + er, M = c.M;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  const uint32_t* n_clus_raw = c.n_clus + (size_t)er * M;  // runs << 24 | clusters surviving the cut
+  const uint32_t* n_clus_raw = c.n_clus + (size_t)er * M;
   // S11: a module with two or more runs makes the event NONCONTIGUOUS; clustering is not defined for such an event
   bool split = false;
-  for (uint32_t m = tid; m < M; m += FIN_THREADS) split |= n_clus_raw[m] >= 2u * NCLUS_RUN;
+  for (uint32_t m = tid; m < M; m += FIN_THREADS) split |= c.n_runs[(size_t)er * M + m] >= 2u;
   const bool skip = __syncthreads_or(split);
   const uint32_t flags = c.ev_cnt[(size_t)er * EC_STRIDE + EC_FLAGS] | (skip ? FLAG_NONCONTIGUOUS : 0u);
-  auto n_clus = [&](uint32_t m) { return n_clus_raw[m] & NCLUS_MASK; };
+  auto n_clus = [&](uint32_t m) { return n_clus_raw[m]; };
 
   // ---- Fig. 3 clamp + exclusive prefix sum over the M modules
   const uint32_t ipt = (M + FIN_THREADS - 1) / FIN_THREADS;

@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(RK<RM>::WPB * 32) findrun_kernel(const __grid_
     }
     const uint32_t a = __reduce_add_sync(FULL, cntA), bb = __reduce_add_sync(FULL, cntB);
     if (lane == 0) {
-      if (cnt) atomicAdd(c.n_clus + task, cnt);
+      c.n_clus[task] = cnt;
       uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
       if (a & 0xFFFFu) atomicAdd(ec + EC_DUP, a & 0xFFFFu);
       if (a >> 16) atomicAdd(ec + EC_BELOW, a >> 16);

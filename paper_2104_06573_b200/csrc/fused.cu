@@ -562,7 +562,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           for (uint32_t r = 1u + lane; r <= Rw; r += 32u) {
             const uint32_t key = s.run_key[r];
             if (s.run_bad[r]) push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);
-            else if (s.run_cnt[r]) atomicAdd(c.n_clus + ((key >> 16) * c.M + (key & 0xFFFFu)), (uint32_t)s.run_cnt[r]);
+            else c.n_clus[(key >> 16) * c.M + (key & 0xFFFFu)] = s.run_cnt[r];
           }
 
           // ============================================================== G: final status and clus, counters

@@ -64,6 +64,7 @@ struct Chunk {
   int32_t thr, cut;
   uint32_t cap_mod, cap_ev; // max_clusters_per_module, max_clusters_per_event
   uint32_t cap_words;       // word capacity of the chunk workspace
+  uint32_t max_wpe;         // max_words_per_event (longer events are flagged)
   // ---- digi outputs, indexed by global word index
   uint16_t* d_module; uint16_t* d_row; uint16_t* d_col; int32_t* d_charge; int32_t* d_clus; uint8_t* d_status;
   // ---- cluster outputs; per-event strides cap_ev, M, M, M+1, 16 (event index absolute)
@@ -80,6 +81,7 @@ struct Chunk {
   uint32_t* chunk_seg;      // [cap_words/128 + 2] segment (event_rel*F + fed) of the chunk's first word
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
+  uint32_t* n_runs;         // [(e1-e0)*M] runs of the module (more than one: the event is NONCONTIGUOUS, S11)
   // temp cluster records, indexed by chunk-relative word index (run first + local id): dense 16 + 4 bytes
   uint4* t_a;               // first_digi, n_pix, charge, x_col bits
   float* t_y;

@@ -43,19 +43,17 @@ __device__ __forceinline__ int32_t calibrate(const Chunk& c, uint32_t adc, float
 // sg / F (F is a power of two in both detector configurations: a shift)
 __device__ __forceinline__ uint32_t div_F(const Chunk& c, uint32_t sg) { return c.F_shift != 0xFFFFFFFFu ? sg >> c.F_shift : sg / c.F; }
 
-// a3: module_first / module_end are keyed by module id (S12).  Every run start also counts one run of its module in
-// the top byte of n_clus (saturating use: two or more runs make the event NONCONTIGUOUS, S11; offsets_kernel raises
-// the flag); none of the three atomics returns a value, so nothing waits for them.
-// key = event_rel << 16 | module, g = global word index.
-constexpr uint32_t NCLUS_RUN = 1u << 24, NCLUS_MASK = NCLUS_RUN - 1u;  // n_clus: runs << 24 | clusters surviving the cut
+// a3: module_first / module_end are keyed by module id (S12).  Every run start also counts one run of its module:
+// two or more runs make the event NONCONTIGUOUS (S11; offsets_kernel raises the flag).  None of the three atomics
+// returns a value, so nothing waits for them.  key = event_rel << 16 | module, g = global word index.
 __device__ __forceinline__ void run_start(const Chunk& c, uint32_t key, uint32_t g) {
   const uint32_t er = key >> 16, m = key & 0xFFFFu;
   atomicMin(c.module_first + ((size_t)(c.e0 + er) * c.M + m), g - c.segB[er * c.F]);
-  atomicAdd(c.n_clus + ((size_t)er * c.M + m), NCLUS_RUN);
+  atomicAdd(c.n_runs + ((size_t)er * c.M + m), 1u);
 }
 // true when module m of event er (launch-group relative) has more than one run: its range is not a run (S11)
 __device__ __forceinline__ bool module_split(const Chunk& c, uint32_t er, uint32_t m) {
-  return c.n_clus[(size_t)er * c.M + m] >= 2u * NCLUS_RUN;
+  return c.n_runs[(size_t)er * c.M + m] >= 2u;
 }
 __device__ __forceinline__ void run_end(const Chunk& c, uint32_t key, uint32_t g) {
   const uint32_t er = key >> 16, m = key & 0xFFFFu;
