@@ -253,11 +253,12 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
 }
 
 // ------------------------------------------------------------------ kernel
-// Runs of up to SMEM_CAP digis keep all their tables in shared memory; longer ones use the global workspace.
-constexpr int OVF_THREADS = 256;
-constexpr uint32_t SMEM_CAP = 2048;
+// One block per run, taken from a task list by ticket.  Runs of up to CAP digis keep all their tables in shared
+// memory; longer ones go to the next list (a larger size of this kernel) or, in the last size, use the global
+// workspace.  One size is in use: 256 threads / 2048 digis (88 KB).  (Measured: as the kernel for ALL the runs the
+// fused kernel leaves, in a 128-thread / 512-digi size, it took 4.3 ms on 200 PU200-like events where the bucket-hash
+// run kernels of findrun.cu take 1.9 ms.)
 constexpr size_t SMEM_PER_DIGI = 8 + 8 + 2 * 4 + 4 * 5;  // sx, sy, 2 hash slots, pos, chg, label, q, npix
-constexpr size_t OVF_SMEM = SMEM_CAP * SMEM_PER_DIGI;
 
 __device__ __forceinline__ Tables<uint32_t> carve(unsigned char* base, uint32_t cap) {
   Tables<uint32_t> T;
@@ -272,25 +273,36 @@ __device__ __forceinline__ Tables<uint32_t> carve(unsigned char* base, uint32_t 
   return T;
 }
 
-__global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_constant__ Chunk c) {
+template <int THREADS, uint32_t CAP>
+__global__ void __launch_bounds__(THREADS) block_kernel(const __grid_constant__ Chunk c, const uint32_t* __restrict__ in_list,
+                                                        uint32_t ctl_count, uint32_t ctl_ticket, uint32_t* __restrict__ long_list,
+                                                        uint32_t ctl_long) {
   extern __shared__ __align__(16) unsigned char ovf_smem[];
-  __shared__ uint32_t s_scan[OVF_THREADS / 32 + 1];
+  __shared__ uint32_t s_scan[THREADS / 32 + 1];
   __shared__ uint32_t s_task;
-  const BlockGroup<OVF_THREADS> g{s_scan};
-  uint32_t count = c.ctl[CTL_OVF_COUNT];
+  const BlockGroup<THREADS> g{s_scan};
+  uint32_t count = c.ctl[ctl_count];
   count = count < c.list_cap ? count : c.list_cap;
   while (true) {
     __syncthreads();
-    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + CTL_OVF_TICKET, 1u);
+    if (threadIdx.x == 0) s_task = atomicAdd(c.ctl + ctl_ticket, 1u);
     __syncthreads();
     const uint32_t t = s_task;
     if (t >= count) break;
-    const uint32_t task = c.ovf_list[t];
+    const uint32_t task = in_list[t];
     const uint32_t er = task / c.M, m = task - er * c.M;
     if (module_split(c, er, m)) continue;  // S11: the module has several runs; the event is not clustered
     const uint32_t first = c.module_first[(size_t)(c.e0 + er) * c.M + m];
-    if (c.module_end[(size_t)(c.e0 + er) * c.M + m] - first <= SMEM_CAP) {
-      cluster_task<BlockGroup<OVF_THREADS>, uint32_t, true>(c, g, carve(ovf_smem, SMEM_CAP), task);
+    const uint32_t n = c.module_end[(size_t)(c.e0 + er) * c.M + m] - first;
+    if (n <= CAP) {
+      cluster_task<BlockGroup<THREADS>, uint32_t, true>(c, g, carve(ovf_smem, CAP), task);
+      continue;
+    }
+    if (long_list) {  // too long for this size of the kernel: the next one takes it (a task moves down the lists once)
+      if (threadIdx.x == 0) {
+        const uint32_t i = atomicAdd(c.ctl + ctl_long, 1u);
+        if (i < c.list_cap) long_list[i] = task;
+      }
       continue;
     }
     const uint32_t ebase = c.segB[er * c.F];
@@ -300,18 +312,22 @@ __global__ void __launch_bounds__(OVF_THREADS) overflow_kernel(const __grid_cons
     T.pos = c.g_pos + rb; T.chg = nullptr;
     T.label = reinterpret_cast<uint32_t*>(c.d_clus + (size_t)ebase + first);  // clus is written last, per digi
     T.q = c.g_q + rb; T.npix = c.g_npix + rb; T.sx = c.g_sx + rb; T.sy = c.g_sy + rb;
-    cluster_task<BlockGroup<OVF_THREADS>, unsigned long long, false>(c, g, T, task);
+    cluster_task<BlockGroup<THREADS>, unsigned long long, false>(c, g, T, task);
   }
 }
+
+constexpr int T_B = 256;
+constexpr uint32_t CAP_B = 2048;
 
 }  // namespace
 
 cudaError_t configure_overflow_kernel() {
-  return cudaFuncSetAttribute(overflow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OVF_SMEM);
+  return cudaFuncSetAttribute(block_kernel<T_B, CAP_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(CAP_B * SMEM_PER_DIGI));
 }
 
+// the runs the run kernels (findrun.cu) left: longer than 1024 digis, dense, or with 64-bit charge sums
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
-  overflow_kernel<<<n_sm * 2, OVF_THREADS, OVF_SMEM, stream>>>(c);
+  block_kernel<T_B, CAP_B><<<n_sm * 2, T_B, CAP_B * SMEM_PER_DIGI, stream>>>(c, c.ovf_list, CTL_OVF_COUNT, CTL_OVF_TICKET, nullptr, 0u);
 }
 
 }  // namespace pix
