@@ -53,6 +53,8 @@ def _load():
         lib.pixo_calibrate.restype = ctypes.c_int32
         lib.pixo_rechits.argtypes = [ctypes.c_uint32, ctypes.c_uint32] + [vp] * 6 + [ctypes.c_uint32] + [vp] * 10
         lib.pixo_rechits.restype = ctypes.c_int
+        lib.pixo_legacy.argtypes = [ctypes.c_uint32, ctypes.c_uint32] + [vp] * 7 + [ctypes.c_uint32, ctypes.c_uint32] + [vp] * 6
+        lib.pixo_legacy.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -120,3 +122,23 @@ def rechits(det, o: dict) -> dict:
     if rc != 0:
         raise ValueError(f"pixo_rechits returned {rc}")
     return h
+
+
+def legacy(det, words: np.ndarray, fed_offsets, o: dict, module_raw_id: np.ndarray, max_errors: int) -> dict:
+    """Legacy digi format + FED error words (S29-S31) from one event's raw words and process() output."""
+    words = np.ascontiguousarray(words, np.uint32)
+    n = len(words)
+    rid = np.ascontiguousarray(module_raw_id, np.uint32)
+    fo = None if fed_offsets is None else np.ascontiguousarray(fed_offsets, np.uint32)
+    out = dict(pdigi=np.zeros(n, np.uint32), raw_id=np.zeros(n, np.uint32), err_word=np.zeros(max_errors, np.uint32),
+               err_fed=np.zeros(max_errors, np.uint16), err_type=np.zeros(max_errors, np.uint8), n_errors=np.zeros(1, np.uint32))
+    ins = [np.ascontiguousarray(o[k]) for k in ("module", "row", "col", "status")]
+    rc = _load().pixo_legacy(n, det.n_feds, words.ctypes.data, None if fo is None else fo.ctypes.data,
+                             *[a.ctypes.data for a in ins], rid.ctypes.data, det.n_modules, max_errors,
+                             *[out[k].ctypes.data for k in ("pdigi", "raw_id", "err_word", "err_fed", "err_type", "n_errors")])
+    if rc != 0:
+        raise ValueError(f"pixo_legacy returned {rc}")
+    k = min(int(out["n_errors"][0]), max_errors)
+    for name in ("err_word", "err_fed", "err_type"):
+        out[name] = out[name][:k]
+    return out

@@ -21,6 +21,8 @@
 // invariants; metamorphic permutations; the generator's injected-error tallies.
 // RecHits-lite (pixo_rechits, readings S25-S28): closed forms on hand-built clusters and a numpy group-by
 // recomputation (tests/test_oracle_rechits.py).
+// Legacy format (pixo_legacy, readings S29-S31): a hand-computed packed word, an independent numpy unpacking and
+// error-list recomputation, the generator's injected-error tallies, the capacity clamp (tests/test_oracle_legacy.py).
 // PARITY UNPINNED against paper-printed values: the paper prints no worked example, count or
 // intermediate value for this path.
 #include <cstdint>
@@ -280,6 +282,38 @@ int pixo_rechits(uint32_t n_words, uint32_t M, const uint16_t* d_module, const u
     if (c_n_pix[g] == 1) f |= 4;                                                                                   // SINGLE_PIXEL
     h_flags[g] = f;
   }
+  return 0;
+}
+
+// ---- Legacy digi format and FED error words (PAPER.md:31 names "optional modules ... to convert
+// the SoA to legacy data formats" and leaves them out; nothing about the format is in the paper).
+// Readings S29-S31 of DESIGN.md.  Per word i of one event:
+//   pdigi[i]  = row | col << 11 | adc << 22 for a decodable word (adc = the raw word's low byte), 0 otherwise      (S29)
+//   raw_id[i] = module_raw_id[module] for a decodable word, 0 otherwise                                            (S30)
+// Error list (S31): every word whose status is ERR_LINK / ERR_ROC / ERR_DCOL / ERR_PXID (padding words are not
+// errors), in word order: the raw word, the FED block it sits in, the status code.  *n_errors is the true count;
+// the list holds the first max_errors of them.
+int pixo_legacy(uint32_t n_words, uint32_t n_feds, const uint32_t* words, const uint32_t* fed_offsets,
+                const uint16_t* d_module, const uint16_t* d_row, const uint16_t* d_col, const uint8_t* d_status,
+                const uint32_t* module_raw_id, uint32_t n_modules, uint32_t max_errors,
+                uint32_t* pdigi, uint32_t* raw_id, uint32_t* err_word, uint16_t* err_fed, uint8_t* err_type, uint32_t* n_errors) {
+  uint32_t ne = 0, fed = 0;
+  for (uint32_t i = 0; i < n_words; ++i) {
+    if (fed_offsets) while (fed + 1 < n_feds && i >= fed_offsets[fed + 1]) ++fed;
+    const uint8_t st = d_status[i];
+    if (st <= ST_DUP) {  // decodable: OK, CUT, BELOW_THRESHOLD, DUPLICATE
+      if (d_module[i] >= n_modules) return 1;
+      pdigi[i] = (uint32_t)d_row[i] | ((uint32_t)d_col[i] << 11) | ((words[i] & 255u) << 22);
+      raw_id[i] = module_raw_id[d_module[i]];
+    } else {
+      pdigi[i] = 0; raw_id[i] = 0;
+      if (st >= ST_ERR_LINK) {
+        if (ne < max_errors) { err_word[ne] = words[i]; err_fed[ne] = (uint16_t)fed; err_type[ne] = st; }
+        ++ne;
+      }
+    }
+  }
+  *n_errors = ne;
   return 0;
 }
 
