@@ -184,6 +184,26 @@ typedef struct {
 int pix_rechits(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* event_word_offsets,
                 const pix_digis* digis, const pix_clusters* clusters, const pix_hits* out_hits);
 
+/* Legacy digi format and FED error words ("optional modules ... to convert the SoA to
+ * legacy data formats", which the paper leaves out; the format is this build's own, readings S29-S31 of DESIGN.md).
+ * Per word i (batch: global word index):
+ *   pdigi[i]  = row | col << 11 | adc << 22 for a decodable word (status OK / CUT / BELOW_THRESHOLD / DUPLICATE; adc = the
+ *               raw word's low byte), 0 otherwise                                                              (S29)
+ *   raw_id[i] = module_raw_id[module] for a decodable word, 0 otherwise                                        (S30)
+ * Error list of event e, at stride max_errors_per_event: every word with status ERR_LINK / ERR_ROC / ERR_DCOL / ERR_PXID
+ * (padding words are not errors), in word order: the raw word, the FED block it sits in, the status code; n_errors[e]
+ * is the true count, the list holds the first max_errors_per_event of them (S31).
+ * All pointers DEVICE; raw_words, event_word_offsets and fed_offsets as given to pix_process_batch, digis its output;
+ * module_raw_id [M].  Never allocates or synchronises; list elements beyond n_errors[e] are left untouched. */
+typedef struct {
+  uint32_t* pdigi; uint32_t* raw_id;                         /* [n_words_total] */
+  uint32_t* err_word; uint16_t* err_fed; uint8_t* err_type;  /* [n_events * max_errors_per_event] */
+  uint32_t* n_errors;                                        /* [n_events] */
+} pix_legacy;
+int pix_legacy_format(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* raw_words, uint32_t n_words_total,
+                      const uint32_t* event_word_offsets, const uint32_t* fed_offsets, const pix_digis* digis,
+                      const uint32_t* module_raw_id, uint32_t max_errors_per_event, const pix_legacy* out);
+
 /* Number of CUDA kernels this handle has launched so far (for launch accounting). */
 uint64_t pix_kernel_launches(const pix_handle* h);
 

@@ -25,7 +25,7 @@ SUMMARY = ("n_words", "n_decoded", "n_empty", "n_err_link", "n_err_roc", "n_err_
 FLAG_NONCONTIGUOUS, FLAG_CLUSTER_CAPACITY_OVERFLOW, FLAG_EVENT_TOO_LARGE = 1, 2, 4
 EXPORTS = ("pix_create", "pix_clone", "pix_destroy", "pix_process", "pix_process_batch", "pix_process_batch_host",
            "pix_rechits", "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile",
-           "pix_overflow_runs", "pix_host_bytes_out")
+           "pix_overflow_runs", "pix_host_bytes_out", "pix_legacy_format")
 
 _vp, _u32 = ctypes.c_void_p, ctypes.c_uint32
 
@@ -52,6 +52,10 @@ class Digis(ctypes.Structure):
 class Clusters(ctypes.Structure):
     _fields_ = [(n, _vp) for n in ("module", "first_digi", "n_pix", "charge", "x_col", "y_row", "module_first",
                                    "module_end", "clus_module_start", "summary")]
+
+
+class Legacy(ctypes.Structure):
+    _fields_ = [(n, _vp) for n in ("pdigi", "raw_id", "err_word", "err_fed", "err_type", "n_errors")]
 
 
 class Hits(ctypes.Structure):
@@ -255,6 +259,33 @@ def pix_rechits(h: Handle, stream, n_events: int, event_word_offsets, digis: dic
     rc = lib.pix_rechits(h.ptr, _stream_ptr(stream), n_events, _ptr(event_word_offsets), ctypes.byref(d), ctypes.byref(c),
                          ctypes.byref(hh))
     return _check(h, rc, raise_on_error)
+
+
+def pix_legacy_format(h: Handle, stream, n_events: int, raw_words, n_words_total: int, event_word_offsets, fed_offsets,
+                      digis: dict, module_raw_id, max_errors_per_event: int, out: dict, raise_on_error: bool = True) -> int:
+    """Legacy digi format + FED error words over the outputs of pix_process_batch (device pointers, asynchronous)."""
+    d = Digis(*[_ptr(digis.get(n)) for n, _ in Digis._fields_])
+    o = Legacy(*[_ptr(out.get(n)) for n, _ in Legacy._fields_])
+    lib = load()
+    lib.pix_legacy_format.argtypes = [_vp, _vp, _u32, _vp, _u32, _vp, _vp, ctypes.POINTER(Digis), _vp, _u32, ctypes.POINTER(Legacy)]
+    lib.pix_legacy_format.restype = ctypes.c_int
+    rc = lib.pix_legacy_format(h.ptr, _stream_ptr(stream), n_events, _ptr(raw_words), n_words_total, _ptr(event_word_offsets),
+                               _ptr(fed_offsets), ctypes.byref(d), _ptr(module_raw_id), max_errors_per_event, ctypes.byref(o))
+    return _check(h, rc, raise_on_error)
+
+
+def alloc_legacy(n_words: int, n_events: int, max_errors_per_event: int, device="cuda", fill: int | None = None):
+    import torch
+    shapes = dict(pdigi=(n_words + 16, "uint32"), raw_id=(n_words + 16, "uint32"),
+                  err_word=(n_events * max_errors_per_event, "uint32"), err_fed=(n_events * max_errors_per_event, "uint16"),
+                  err_type=(n_events * max_errors_per_event, "uint8"), n_errors=(n_events, "uint32"))
+    out = {}
+    for k, (n, dt) in shapes.items():
+        t = torch.empty(max(int(n), 1), dtype=getattr(torch, dt), device=device)
+        if fill is not None:
+            t.view(torch.uint8).fill_(fill)
+        out[k] = t
+    return out
 
 
 HIT_DTYPES = dict(x_local="float32", y_local="float32", min_row="uint16", max_row="uint16", min_col="uint16",

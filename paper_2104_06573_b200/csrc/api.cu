@@ -13,6 +13,9 @@
 namespace pix {
 void launch_rechits(uint32_t n_events, uint32_t M, uint32_t cap_ev, const uint32_t* ev_off, const pix_digis& d,
                     const pix_clusters& k, const pix_hits& h, cudaStream_t stream);
+void launch_legacy(uint32_t n_events, uint32_t F, uint32_t M, uint32_t n_total, const uint32_t* words, const uint32_t* ev_off,
+                   const uint32_t* fed_off, const pix_digis& d, const uint32_t* raw_id_of, uint32_t cap, const pix_legacy& o,
+                   int n_sm, cudaStream_t stream);
 }
 
 namespace {
@@ -449,6 +452,27 @@ int pix_rechits(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint3
   pix::launch_rechits(n_events, h->M, h->p.max_clusters_per_event, event_word_offsets, *digis, *clusters, *out_hits,
                       (cudaStream_t)cuda_stream);
   h->launches += (n_events + 65534u) / 65535u;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
+  return PIX_OK;
+}
+
+int pix_legacy_format(pix_handle* h, void* cuda_stream, uint32_t n_events, const uint32_t* raw_words, uint32_t n_words_total,
+                      const uint32_t* event_word_offsets, const uint32_t* fed_offsets, const pix_digis* digis,
+                      const uint32_t* module_raw_id, uint32_t max_errors_per_event, const pix_legacy* out) {
+  if (!h) return PIX_ERR_INVALID_ARG;
+  h->err.clear();
+  if (n_events == 0) return PIX_OK;
+  if (!event_word_offsets || !digis || !module_raw_id || !out) return fail(h, PIX_ERR_INVALID_ARG, "NULL argument");
+  if (n_words_total > 0 && !raw_words) return fail(h, PIX_ERR_INVALID_ARG, "raw_words is NULL");
+  if (h->F > 1 && !fed_offsets) return fail(h, PIX_ERR_INVALID_ARG, "fed_offsets is NULL but n_feds > 1");
+  if (!digis->module || !digis->row || !digis->col || !digis->status) return fail(h, PIX_ERR_INVALID_ARG, "a digi input array is NULL");
+  if (!out->pdigi || !out->raw_id || !out->n_errors || (max_errors_per_event && (!out->err_word || !out->err_fed || !out->err_type)))
+    return fail(h, PIX_ERR_INVALID_ARG, "a legacy output array is NULL");
+  if (n_events > h->p.max_events_per_batch) return fail(h, PIX_ERR_CAPACITY, "n_events > max_events_per_batch");
+  pix::launch_legacy(n_events, h->F, h->M, n_words_total, raw_words, event_word_offsets, h->F > 1 ? fed_offsets : nullptr, *digis,
+                     module_raw_id, max_errors_per_event, *out, h->n_sm, (cudaStream_t)cuda_stream);
+  h->launches += 1;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail_cuda(h, e, "kernel launch");
   return PIX_OK;

@@ -264,3 +264,43 @@ def test_cfg4_full_size_sampled(gu, full):
     """BASELINE.json configs[4] at its batch size: 100 edge-case events in one call."""
     _, b = pixgen.config("cfg4")
     _full_size(gu, full, b, 30, 4, "cfg4 full size")
+
+
+def test_legacy_format(gu, full):
+    """pix_legacy_format (S29-S31) against the oracle: packed digi words, raw detector ids, the error list in
+    word order with its FED index and type, the true count beyond the list capacity; everything bit-exact."""
+    import oracle
+    import paper_2104_06573_b200 as pix
+    import torch
+    b = pixgen.events(full, ["pu50", "errors", "allbad", "empty", "dups", "errors", "oneword"], 600 + np.arange(7))
+    sizes = np.diff(b.event_offsets.astype(np.int64))
+    E, M, F, n = b.n_events, full.n_modules, full.n_feds, len(b.words)
+    kmax, cap = int(sizes.max()), 1500  # the "allbad" event has more errors than the list holds
+    rid = (0x12000000 + np.random.default_rng(3).permutation(M).astype(np.uint32) * 4).astype(np.uint32)
+    h = gu.make_handle(full, P, int(sizes.max()), kmax, E, 3)
+    try:
+        words = torch.from_numpy(np.concatenate([b.words, np.zeros(16, np.uint32)]).view(np.int32)).cuda()
+        ev_off = torch.from_numpy(b.event_offsets.view(np.int32).copy()).cuda()
+        fed_off = torch.from_numpy(b.fed_offsets.view(np.int32).reshape(-1).copy()).cuda()
+        digis, cl = pix.alloc_outputs(n, E, M, kmax, "cuda", fill=0xCD)
+        leg = pix.alloc_legacy(n, E, cap, "cuda", fill=0xCD)
+        rid_d = torch.from_numpy(rid.view(np.int32)).cuda()
+        pix.pix_process_batch(h, None, E, words, n, ev_off, fed_off, digis, cl)
+        pix.pix_legacy_format(h, None, E, words, n, ev_off, fed_off, digis, rid_d, cap, leg)
+        got = gu.to_numpy(leg)
+    finally:
+        torch.cuda.synchronize()
+        pix.pix_destroy(h)
+    clipped = 0
+    for e in range(E):
+        w, fo = b.event(e)
+        o = oracle.process(full, w, fo, P, max_clusters_per_event=kmax)
+        lo = oracle.legacy(full, w, fo, o, rid, cap)
+        a, z = int(b.event_offsets[e]), int(b.event_offsets[e + 1])
+        assert np.array_equal(got["pdigi"][a:z], lo["pdigi"]) and np.array_equal(got["raw_id"][a:z], lo["raw_id"]), e
+        ne = int(lo["n_errors"][0]); k = min(ne, cap); clipped += ne > cap
+        assert int(got["n_errors"][e]) == ne, e
+        for name in ("err_word", "err_fed", "err_type"):
+            assert np.array_equal(got[name][e * cap:e * cap + k], lo[name]), (e, name)
+        assert np.all(got["err_type"][e * cap + k:(e + 1) * cap] == 0xCD)  # untouched beyond the count
+    assert clipped >= 1
