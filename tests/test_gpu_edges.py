@@ -304,3 +304,57 @@ def test_legacy_format(gu, full):
             assert np.array_equal(got[name][e * cap:e * cap + k], lo[name]), (e, name)
         assert np.all(got["err_type"][e * cap + k:(e + 1) * cap] == 0xCD)  # untouched beyond the count
     assert clipped >= 1
+
+
+def test_guard_bands_and_repeatability(gu, full):
+    """compute-sanitizer is closed on this pool, so bounds and races are checked by hand: every output array sits
+    between two poisoned guard bands that must stay untouched, and twelve runs of a batch that exercises every kernel
+    (PU200 runs for the block kernels, dense modules, duplicates, invalid words, a flagged event) on alternating
+    streams and launch-group sizes must be bit-identical -- a lost update or a read of an unfinished neighbour
+    shows up as a run that differs."""
+    import paper_2104_06573_b200 as pix
+    import torch
+    b = pixgen.events(full, ["pu50", "dense", "dups", "errors", "pu200", "edges", "empty", "pu50"], 800 + np.arange(8),
+                      cap_words_per_event=1 << 19)
+    sizes = np.diff(b.event_offsets.astype(np.int64))
+    E, M, F, n = b.n_events, full.n_modules, full.n_feds, len(b.words)
+    kmax, G = int(sizes.max()), 4096
+    words = torch.from_numpy(np.concatenate([b.words, np.zeros(16, np.uint32)]).view(np.int32)).cuda()
+    ev_off = torch.from_numpy(b.event_offsets.view(np.int32).copy()).cuda()
+    fed_off = torch.from_numpy(b.fed_offsets.view(np.int32).reshape(-1).copy()).cuda()
+    sizes_of = dict(module=n, row=n, col=n, charge=n, clus=n, status=n)
+    csz = {k: E * kmax for k in pix.CLUSTER_DTYPES}
+    csz.update(module_first=E * M, module_end=E * M, clus_module_start=E * (M + 1), summary=E * 16)
+    dts = dict(pix.DIGI_DTYPES); cdt = dict(pix.CLUSTER_DTYPES); cdt.update(pix.PER_EVENT)
+
+    def guarded(size, dt):
+        t = torch.empty(size + 2 * G, dtype=getattr(torch, dt), device="cuda")
+        t.view(torch.uint8).fill_(0xCD)
+        return t
+
+    ref = None
+    streams = [None, torch.cuda.Stream(), torch.cuda.Stream()]
+    for it in range(12):
+        h = gu.make_handle(full, P, int(sizes.max()), kmax, E, (0, 3, 5)[it % 3])
+        try:
+            raw_d = {k: guarded(v, dts[k]) for k, v in sizes_of.items()}
+            raw_c = {k: guarded(v, cdt[k]) for k, v in csz.items()}
+            d = {k: v[G:G + sizes_of[k]] for k, v in raw_d.items()}
+            c = {k: v[G:G + csz[k]] for k, v in raw_c.items()}
+            pix.pix_process_batch(h, streams[it % 3], E, words, n, ev_off, fed_off, d, c)
+            torch.cuda.synchronize()
+            for k, v, size in [(k, v, sizes_of[k]) for k, v in raw_d.items()] + [(k, v, csz[k]) for k, v in raw_c.items()]:
+                u = v.view(torch.uint8); es = v.element_size()
+                assert bool((u[:G * es] == 0xCD).all()) and bool((u[(G + size) * es:] == 0xCD).all()), f"guard band of {k} touched"
+            out = gu.split_events(full, b, {k: v.cpu().numpy() for k, v in d.items()}, {k: v.cpu().numpy() for k, v in c.items()}, kmax)
+        finally:
+            torch.cuda.synchronize()
+            pix.pix_destroy(h)
+        if ref is None:
+            ref = out
+            for e, (g, o) in enumerate(zip(out, gu.oracle_events(full, b, P, kmax=kmax))):
+                gu.assert_event_equal(g, o, tag=f"guarded run, event {e}")
+        else:
+            for e, (x, y) in enumerate(zip(ref, out)):
+                for k in x:
+                    assert np.array_equal(x[k], y[k]), (it, e, k)
