@@ -90,8 +90,9 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
   c.n_clus = (uint32_t*)take(Ec * M * 4);
   c.n_runs = (uint32_t*)take(Ec * M * 4);
-  c.t_a = (uint4*)take(W * sizeof(uint4));
-  c.t_y = (float*)take(W * sizeof(float));
+  c.t_a = (uint4*)take(2 * W * sizeof(uint4));
+  c.t_y = (float*)take(2 * W * sizeof(float));
+  c.t_base = (uint32_t*)take(Ec * M * 4);
   c.g_hash = (unsigned long long*)take(W * 16);
   c.g_pos = (uint32_t*)take(W * 4); c.g_q = (uint32_t*)take(W * 4); c.g_npix = (uint32_t*)take(W * 4);
   c.g_sx = (unsigned long long*)take(W * 8); c.g_sy = (unsigned long long*)take(W * 8);

@@ -199,7 +199,10 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     atomicAdd(T.sy + r, (unsigned long long)e * row);
   }
   g.sync();
-  // 5: roots in digi order -> local ids (S14), temp records (S18)
+  // 5: roots in digi order -> local ids (S14), temp records (S18) in a stretch of n slots of the temp area
+  if (rk == 0) g.s_scan[0] = alloc_temp(c, n);
+  g.sync();
+  const uint32_t tbase = g.s_scan[0];
   uint32_t n_pre = 0, n_post = 0;
   for (uint32_t k0 = 0; k0 < n; k0 += gs) {
     const uint32_t k = k0 + rk;
@@ -215,8 +218,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     const uint32_t id = n_post + g.scan_flag(surv, tot_post);
     if (root) {
       if (surv) {
-        const uint32_t o = rb + id;
-        put_temp(c, o, first + k, T.npix[k], Q, (float)((double)T.sx[k] / (double)Q),
+        put_temp(c, tbase + id, first + k, T.npix[k], Q, (float)((double)T.sx[k] / (double)Q),
                  (float)((double)T.sy[k] / (double)Q));
       }
       T.q[k] = surv ? id : NO_INDEX;
@@ -245,7 +247,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
   }
   n_dup = g.sum(n_dup); n_below = g.sum(n_below); n_ok = g.sum(n_ok); n_cut = g.sum(n_cut);
   if (rk == 0) {
-    c.n_clus[task] = n_post;
+    c.n_clus[task] = n_post; c.t_base[task] = tbase;
     uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
     atomicAdd(ec + EC_PRECUT, n_pre); atomicAdd(ec + EC_DUP, n_dup); atomicAdd(ec + EC_BELOW, n_below);
     atomicAdd(ec + EC_OK, n_ok); atomicAdd(ec + EC_CUT, n_cut);

@@ -128,8 +128,7 @@ __global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_const
     __syncthreads();
     const uint32_t total = s_start[M];
     const uint32_t n_emit = total < c.cap_ev ? total : c.cap_ev;
-    const uint32_t rel = c.segB[er * c.F] - c.segB[0];
-    const uint32_t* mfirst = c.module_first + (size_t)e * M;
+    const uint32_t* tbase = c.t_base + (size_t)er * M;
 #pragma unroll
     for (uint32_t j = 0; j < SLICE / FIN_THREADS; ++j) {
       const uint32_t g = g0 + j * FIN_THREADS + tid;
@@ -139,7 +138,7 @@ __global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_const
         const uint32_t mid = (lo + hi + 1u) >> 1;
         if (s_start[mid] <= g) lo = mid; else hi = mid - 1u;
       }
-      const uint32_t src = rel + mfirst[lo] + (g - s_start[lo]);
+      const uint32_t src = tbase[lo] + (g - s_start[lo]);
       const size_t o = (size_t)e * c.cap_ev + g;
       c.c_module[o] = (uint16_t)lo;
       const uint4 a = c.t_a[src];

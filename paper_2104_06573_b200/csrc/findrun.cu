@@ -42,6 +42,7 @@ struct __align__(16) RunSmem {
   uint32_t wpre[RM / 32]; // survivors before each word of bits
   uint32_t ne[2];         // edges listed in this round / the next one
   uint32_t task, flags, n_surv, n_roots;
+  uint32_t tbase, pad2[3];  // the run's stretch of the temp record area
   uint32_t cnt[4];        // dup, below, ok, cut
   uint32_t pad[2];
 };
@@ -231,6 +232,8 @@ __global__ void __launch_bounds__(RK<RM>::NT) findrun_kernel(const __grid_consta
       if (tid == 0) { const uint32_t i = atomicAdd(c.ctl + CTL_OVF_COUNT, 1u); if (i < c.list_cap) c.ovf_list[i] = task; }
       continue;
     }
+    if (tid == 0) s.tbase = alloc_temp(c, s.n_surv);  // after the check above: a run is allotted by the kernel that finishes it
+    __syncthreads();
     // ---- renumber (S14: local id = rank among the surviving roots, in digi order), temp records (S18)
 #pragma unroll 1
     for (uint32_t k = 0; k < nk; ++k) {
@@ -242,7 +245,7 @@ __global__ void __launch_bounds__(RK<RM>::NT) findrun_kernel(const __grid_consta
           id = s.wpre[t >> 5] + __popc(w & ((1u << (t & 31u)) - 1u));
           const uint32_t Q = q[t];
           const float fq = (float)Q;
-          put_temp(c, (gb - gBeg) + id, first + t, np[t], Q, __fdividef((float)sx[t], fq), __fdividef((float)sy[t], fq));
+          put_temp(c, s.tbase + id, first + t, np[t], Q, __fdividef((float)sx[t], fq), __fdividef((float)sy[t], fq));
         }
         lid[t] = (uint16_t)id;
       }
@@ -273,7 +276,7 @@ __global__ void __launch_bounds__(RK<RM>::NT) findrun_kernel(const __grid_consta
     }
     __syncthreads();
     if (tid == 0) {
-      c.n_clus[task] = s.n_surv;
+      c.n_clus[task] = s.n_surv; c.t_base[task] = s.tbase;
       uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
       if (s.cnt[0]) atomicAdd(ec + EC_DUP, s.cnt[0]);
       if (s.cnt[1]) atomicAdd(ec + EC_BELOW, s.cnt[1]);

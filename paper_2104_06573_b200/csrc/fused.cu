@@ -89,9 +89,8 @@ struct __align__(16) WarpSmem {
   uint32_t skey[MAXT];     // ring of two chunks: staged words (lane-private while staged: slot t belongs to lane t & 31)
   uint16_t chg[MAXT];      // ring: charges
   uint16_t edge[ECAP];     // a | b << 8; after the unions: local id of a root, or NO_ID
-  uint32_t run_ifirst[RC + 2];  // event-relative index of the run's first digi
   uint32_t run_key[RC + 2];     // event_rel << 16 | module
-  uint16_t run_first[RC + 2];   // window slot of the run's first digi
+  uint16_t run_base[RC + 2];    // clusters of the window that survive the cut before the run's first
   uint16_t run_cnt[RC + 2];     // clusters of the run that survive the cut
   uint8_t run_bad[RC + 2];      // the run is left to the warp-per-run kernel
 };
@@ -376,6 +375,9 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           // window slot t <-> chunk slot f_t + t <-> ring entry (hb + f_t + t) & 255 <-> word wb + t
           const uint32_t len = e_t - f_t, nk = (len + 31u) >> 5, pb = hb + f_t, wb = b + f_t;
           const uint32_t nhome = HC - f_t;  // window slots of the home chunk; the rest is the head of the next chunk
+          // the window's stretch of the temp record area, one slot per digi: asked for now, needed in phase F
+          uint32_t wbase_l = 0u;
+          if (lane == 0) wbase_l = alloc_temp(c, len);
           // ============================================================== B: clear; run tables; insert
           {
             uint4* t4 = reinterpret_cast<uint4*>(s.tab);
@@ -400,8 +402,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
               const uint32_t er = cur.one_event ? cur.er0 : event_of(c, S, sgc, wb + t);
               const uint32_t m = c.d_module[wb + t];  // written by this warp when it decoded the chunk
               if (r <= RC) {
-                s.run_first[r] = (uint16_t)t; s.run_key[r] = (er << 16) | m;
-                s.run_ifirst[r] = wb + t - (cur.one_event ? cur.ebase0 : segB[er * F]);
+                s.run_key[r] = (er << 16) | m;
               } else {
                 push_run(c, c.mid_list, CTL_MID_COUNT, er, m);  // too many runs: left to findrun
               }
@@ -513,10 +514,12 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           __syncwarp();
 
           // ============================================================== F: cut, renumber, temp records (one root per lane)
+          uint32_t wbase_w = 0u;
           {
             uint32_t cnt = 0u;                   // surviving roots before this iteration
             uint32_t run_c = 0u, base_c = 0u;    // the run of the last root so far and the survivors before that run
-            const uint32_t relb = wb - gBeg;     // launch-group index of window slot 0
+            const uint32_t wbase = __shfl_sync(FULL, wbase_l, 0);
+            wbase_w = wbase;
 #pragma unroll 1
             for (uint32_t i0 = 0u; i0 < nr; i0 += 32u) {
               const bool valid = i0 + lane < nr;
@@ -542,16 +545,15 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
                 uint32_t id = NO_ID;
                 if (surv) {
                   id = rank - base;
-                  const uint32_t rf = s.run_first[r];
                   // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
                   const float fq = (float)Q;
-                  put_temp(c, relb + rf + id, s.run_ifirst[r] + (t - rf), np, Q, __fdividef((float)sx[t], fq),
-                           __fdividef((float)sy[t], fq));
+                  const uint32_t ifirst = wb + t - (cur.one_event ? cur.ebase0 : segB[(s.run_key[r] >> 16) * F]);  // event-relative index
+                  put_temp(c, wbase + rank, ifirst, np, Q, __fdividef((float)sx[t], fq), __fdividef((float)sy[t], fq));
                 }
                 lid[t] = (uint16_t)id;
                 // the last root of the run in this iteration leaves the run's count so far
                 const bool lastofrun = lane == 31u || i0 + lane + 1u == nr || ((bnd >> (lane + 1u)) & 1u);
-                if (lastofrun) s.run_cnt[r] = (uint16_t)(rank + (surv ? 1u : 0u) - base);
+                if (lastofrun) { s.run_cnt[r] = (uint16_t)(rank + (surv ? 1u : 0u) - base); s.run_base[r] = (uint16_t)base; }
               }
               const uint32_t lastl = 31u - (uint32_t)__clz(__ballot_sync(FULL, valid));
               run_c = __shfl_sync(FULL, r, lastl); base_c = __shfl_sync(FULL, base, lastl);
@@ -562,7 +564,10 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           for (uint32_t r = 1u + lane; r <= Rw; r += 32u) {
             const uint32_t key = s.run_key[r];
             if (s.run_bad[r]) push_run(c, c.mid_list, CTL_MID_COUNT, key >> 16, key & 0xFFFFu);
-            else c.n_clus[(key >> 16) * c.M + (key & 0xFFFFu)] = s.run_cnt[r];
+            else {
+              const uint32_t mo = (key >> 16) * c.M + (key & 0xFFFFu);
+              c.n_clus[mo] = s.run_cnt[r]; c.t_base[mo] = wbase_w + s.run_base[r];
+            }
           }
 
           // ============================================================== G: final status and clus, counters

@@ -37,7 +37,7 @@ constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus;
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
        EC_PRECUT, EC_PUSHED /* runs the event has put on the task lists (at most M) */, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_TEMP_COUNT = 8, CTL_WORDS = 16 };
 
 // Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
 //   x = module | bad << 16 | scol << 24     bad: 0, ST_ERR_LINK or ST_ERR_ROC; scol = +1 / -1 (int8)
@@ -82,9 +82,13 @@ struct Chunk {
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
   uint32_t* n_runs;         // [(e1-e0)*M] runs of the module (more than one: the event is NONCONTIGUOUS, S11)
-  // temp cluster records, indexed by chunk-relative word index (run first + local id): dense 16 + 4 bytes
-  uint4* t_a;               // first_digi, n_pix, charge, x_col bits
-  float* t_y;
+  // temp cluster records: every window / run takes a stretch of the area (alloc_temp) and leaves its start in t_base,
+  // so the records are dense in memory whatever the words-per-cluster ratio; 16 + 4 bytes per record.
+  // Capacity 2 x cap_words: a window allots one slot per root (<= its digis), a run that is redone by a later
+  // kernel (32-bit sums at risk) is allotted once more, by the kernel that finishes it.
+  uint4* t_a;               // [2*cap_words] first_digi, n_pix, charge, x_col bits
+  float* t_y;               // [2*cap_words]
+  uint32_t* t_base;         // [(e1-e0)*M] index of the module's first temp record (local id 0)
   // overflow-kernel scratch, indexed by chunk-relative word index
   unsigned long long* g_hash;  // [2*cap_words]
   uint32_t* g_pos; uint32_t* g_q; uint32_t* g_npix; unsigned long long* g_sx; unsigned long long* g_sy;
@@ -93,6 +97,7 @@ struct Chunk {
 __device__ __forceinline__ uint32_t ev_offset(const Chunk& c, uint32_t e) {
   return c.ev_off ? c.ev_off[e] : (e ? c.n_single : 0u);
 }
+__device__ __forceinline__ uint32_t alloc_temp(const Chunk& c, uint32_t count) { return atomicAdd(c.ctl + CTL_TEMP_COUNT, count); }
 __device__ __forceinline__ void put_temp(const Chunk& c, uint32_t i, uint32_t first, uint32_t npix, uint32_t charge, float x, float y) {
   c.t_a[i] = make_uint4(first, npix, charge, __float_as_uint(x)); c.t_y[i] = y;
 }
