@@ -3,24 +3,31 @@
 // a3 module boundaries (S11, S12), a4 findClus (S10, S13) and a5 sums / charge cut / renumber / temp records
 // (S9, S14, S18) in one pass over the raw words.  SURVEY 8f NEXT-3.
 //
-// The word stream is cut into chunks of 128 words.  A warp takes a range of consecutive chunks (a ticket) and walks
-// it with a two-chunk ring in shared memory: while chunk i is clustered, chunk i+1 is already decoded (one word per
-// lane and round, four rounds), so
+// The word stream is cut into chunks of 128 words.  A warp takes a ticket of consecutive chunks and walks it with a
+// two-chunk ring in shared memory: while the window of chunk i is clustered, chunk i+1 is already decoded (four
+// consecutive words per lane: one 128-bit load, 128-bit / 64-bit stores), so
 //   - the "previous decodable word" that decides whether a word starts a module run is carried in registers from
-//     chunk to chunk (a look-back into memory happens once per range, bounded by the start of the event),
+//     chunk to chunk (a look-back into memory happens once per ticket, bounded by the start of the event; every
+//     event's last run is closed by segfill_kernel),
 //   - the look-ahead a window needs (a run belongs to the warp whose chunk holds its first word; the last run of a
 //     chunk may end in the next chunk) is the next chunk's own decode, done once,
-//   - per-event counters live in registers and are flushed when the range ends or the event changes.
-// Per window (the runs that start in chunk i, up to the first run start of chunk i+1; at most 256 slots):
-//   B  clear the position hash; give every digi its run, insert it keyed by (run, row, col); equal keys keep the
-//      lowest digi (S10)
-//   D  forward-neighbour lookups -> dense edge list -> unions (lock-free hook-and-descend, pix_device.cuh)
-//   E  every live digi adds charge | 1 << 24, charge*col, charge*row into its root's accumulators
-//   F  in slot order: roots with Q >= cut are numbered per run (ballot/popc), temp records written
-//   G  final status and clus of every word of the chunk (undecodable words included), counters
+//   - the raw words of the chunk after that are already in flight (loaded one iteration ahead),
+//   - per-event counters live in registers and are flushed when the ticket ends or the event changes.
+// The decode stages every word in its final form: position | run (counted inside the chunk) | below-threshold |
+// run start.  Per window (the runs that start in chunk i, up to the first run start of chunk i+1; at most 256
+// slots, numbered from the window's first word so that the rounds of 32 are full):
+//   B  clear the position hash; insert every digi keyed by (run, row, col); equal keys keep the lowest digi (S10)
+//   D  forward-neighbour lookups (one branch for the four) -> dense edge list -> unions (lock-free
+//      hook-and-descend, pix_device.cuh), two pointer-jumping rounds
+//   E  every live digi adds charge | 1 << 24, charge*col, charge*row into its root's accumulators; dense root list
+//   F  one root per lane: Q >= cut survives, numbered per run (ballot/popc); temp records into the window's stretch
+//      of the temp area
+//   G  final status and clus of the window's digis, counters (undecodable words are finished by the decode)
 // Warps never wait for each other (no block barrier); all tables are per-warp shared memory.  Runs that do not fit
 // the window, chunks with more than RC runs, hash buckets that overflow and charge sums that could overflow 32 bits go
-// to the warp-per-run kernel (findrun.cu).  Nothing here is shared with oracle/.
+// to the block-per-run kernel (findrun.cu).  Measured: the kernel is bound by instruction issue and, with 50 KB of
+// code walked once per window, by instruction fetch: unrolling any of its loops makes it slower.
+// Nothing here is shared with oracle/.
 #include "pix_common.cuh"
 #include "pix_device.cuh"
 
@@ -28,42 +35,14 @@ namespace pix {
 
 namespace {
 
-#ifndef PIX_WPB
-#define PIX_WPB 4
-#endif
-#ifndef PIX_BPS
-#define PIX_BPS 7
-#endif
-#ifndef PIX_JUMPS
-#define PIX_JUMPS 2
-#endif
-#ifndef PIX_UB
-#define PIX_UB 1
-#endif
-#ifndef PIX_UD
-#define PIX_UD 1
-#endif
-#ifndef PIX_UE
-#define PIX_UE 1
-#endif
-#ifndef PIX_UF
-#define PIX_UF 1
-#endif
-#ifndef PIX_UG
-#define PIX_UG 1
-#endif
-#ifndef PIX_GMAX
-#define PIX_GMAX 32
-#endif
-constexpr int U_UB = PIX_UB, U_UD = PIX_UD, U_UE = PIX_UE, U_UG = PIX_UG;
-constexpr int WPB = PIX_WPB;              // warps per block (they share nothing but the block)
+constexpr int WPB = 4;                    // warps per block (they share nothing but the block)
 constexpr int FT = WPB * 32;
-constexpr int BLOCKS_PER_SM = PIX_BPS;
+constexpr int BLOCKS_PER_SM = 7;          // 8000 B of shared memory per warp, 72 registers per thread
 constexpr uint32_t HC = CHUNK_WORDS;      // words of a chunk (rounds 0-3 of a window)
 constexpr uint32_t MAXT = 256;            // window: home chunk + up to 4 rounds of the next chunk
 constexpr uint32_t RC = 62;               // runs a window can own
 constexpr uint32_t ECAP = 256;            // edge list; flushed (united) when a round might not fit
-constexpr uint32_t GMAX = PIX_GMAX;             // chunks per ticket, at most
+constexpr uint32_t GMAX = 32;             // chunks per ticket, at most
 constexpr uint32_t NOKEY = 0xFFFFFFFFu, FULL = 0xFFFFFFFFu;
 constexpr uint32_t MARK_DUP = 0xFFFFFFFEu, MARK_BELOW = 0xFFFFFFFDu;  // label of a digi that is not live
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;  // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
@@ -391,7 +370,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           if (Rown > RC && lane == 0) s.run_bad[RC + 1u] = 1;  // the runs beyond RC are all "run RC + 1"
           bool dup_seen = false;
           const uint32_t Rr = R <= RC ? R : RC + 1u;             // run of the slots of the next chunk
-#pragma unroll U_UB
+#pragma unroll 1
           for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane, ph = (pb + t) & (MAXT - 1u);
             uint32_t sk = s.skey[ph];
@@ -430,7 +409,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1).  When S is live, SW and SE
           // are joined to it by their own E edges, so d-S alone is enough; when E is live, SE is E's S neighbour.
           uint32_t ne = 0u;
-#pragma unroll U_UD
+#pragma unroll 1
           for (uint32_t k = 0; k <= nk; ++k) {
             if (k == nk || ne + 96u > ECAP) {  // the last round is done, or the next round's edges might not fit: unite what is listed
               __syncwarp();
@@ -473,7 +452,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
             ne += __popc(m2);
           }
 #pragma unroll 1
-          for (int pass = 0; pass < PIX_JUMPS; ++pass) {  // pointer jumping: the chains shrink before the sums
+          for (int pass = 0; pass < 2; ++pass) {  // two pointer-jumping rounds: the chains shrink 4x before the sums (measured: 0 -> 1 -> 2 rounds = 2.91 -> 2.78 -> 2.73 ms)
             for (uint32_t k = 0; k < nk; ++k) {
               const uint32_t t = 32u * k + lane;
               const uint32_t l = s.label[t];
@@ -491,7 +470,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
           }
           __syncwarp();
           uint32_t nr = 0u;  // roots so far
-#pragma unroll U_UE
+#pragma unroll 1
           for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane;
             volatile uint32_t* L = s.label;
@@ -572,7 +551,7 @@ __global__ void __launch_bounds__(FT, BLOCKS_PER_SM) fused_kernel(const __grid_c
 
           // ============================================================== G: final status and clus, counters
           uint32_t cntA = 0u, cntB = 0u, n_pre = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
-#pragma unroll U_UG
+#pragma unroll 1
           for (uint32_t k = 0; k < nk; ++k) {
             const uint32_t t = 32u * k + lane, sk = s.skey[(pb + t) & (MAXT - 1u)];
             if (t < len && sk < SK_BAD && !s.run_bad[(sk >> SK_RUN_SHIFT) & 63u]) {
