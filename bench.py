@@ -2,9 +2,9 @@
 
     python bench.py --gpus 1 --steps 10 --warmup 3            # this repo's CUDA path
     python bench.py --impl reference --steps 3 --warmup 1     # the oracle on the host cores (the reference arm)
-
-A step = one pass of the whole hot path (init; the fused kernel = unpack + calibrate + boundaries + cluster + cut + renumber;
-the warp-per-run and block-per-run kernels for the runs it leaves; finalize = offsets + scatter) over one batch of synthetic events: BASELINE.json configs[2], 1000 PU50-like events (config[1]'s
+A step = one pass of the whole hot path (init; runs = module boundaries + work items; the tile kernel = unpack +
+calibrate + cluster + cut + renumber; the block-per-run kernel for the runs it leaves; finalize = offsets + scatter)
+over one batch of synthetic events: BASELINE.json configs[2], 1000 PU50-like events (config[1]'s
 generator, seeds 0..999), through pix_process_batch.  `value` is timed with the inputs resident in HBM; `e2e`
 goes through pix_process_batch_host with pinned HOST buffers, host<->device copies inside the timed region.
 Under torchrun (N > 1) every rank runs its own 1000 events (seeds rank*1000 ..): weak scaling, no collective
@@ -342,10 +342,10 @@ def run_ours(args):
     torch.cuda.synchronize()
     summ = clusters["summary"].cpu().numpy().reshape(E, 16).astype(np.int64)
     K = int(summ[:, 14].sum())
-    # algorithmic bytes per kernel: the fused kernel reads the raw word and writes the six digi
-    # arrays (19 B per word) and the 20 B temp records; finalize moves the records (20 B in, 22 B out) and writes the
-    # per-event arrays
-    kernel_bytes = {"init": 12 * M * E, "fused": 19 * W + 20 * K, "findrun": 0, "overflow": 0,
+    # algorithmic bytes per kernel: the runs pre-pass reads the raw word and writes one bit; the
+    # tile kernel reads the raw word and writes the six digi arrays (19 B per word) and the 20 B temp records;
+    # finalize moves the records (20 B in, 22 B out) and writes the per-event arrays
+    kernel_bytes = {"init": 12 * M * E, "runs": 4 * W + W // 8, "tile": 19 * W + 20 * K, "overflow": 0,
                     "finalize": 42 * K + (4 * (M + 1) + 64 + 4 * M) * E}
     top = max(prof, key=prof.get)
     peak, peak_src = peak_hbm()
@@ -471,7 +471,7 @@ def run_ours(args):
                        "l2": "inputs+outputs per step (~1.5 GB) exceed the 126 MB L2; no flush"},
             "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e,
             # the chain's algorithmic bytes per step over the step time, against the measured copy bandwidth
-            "roofline": {"bound": "hbm", "kernel": "chain (init, fused, findrun x2, overflow, offsets, scatter)", "achieved": chain_gbs,
+            "roofline": {"bound": "hbm", "kernel": "chain (init, segfill, runs, pack, tile, overflow, offsets, scatter)", "achieved": chain_gbs,
                          "peak": peak, "unit": "GB/s", "frac": chain_gbs / peak, "traffic": chain_traffic, "traffic_note": traffic_note,
                          "peak_source": peak_src, "algorithmic_bytes_per_step": chain_bytes, "formula": "19 W + 22 K + (12 M + 68) E"},
             # the dominant kernel by device time: its own algorithmic bytes over its own launch duration

@@ -190,7 +190,7 @@ def pix_overflow_runs(h: Handle) -> int:
     return int(n.value)
 
 
-KERNEL_FAMILIES = ("init", "fused", "findrun", "overflow", "finalize")
+KERNEL_FAMILIES = ("init", "runs", "tile", "overflow", "finalize")
 
 
 def pix_set_profiling(h: Handle, enable: bool) -> None:

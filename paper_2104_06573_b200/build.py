@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpixclus.so")
-SOURCES = ("decode.cu", "fused.cu", "findrun.cu", "cluster.cu", "finalize.cu", "rechits.cu", "legacy.cu", "api.cu")
+SOURCES = ("decode.cu", "runs.cu", "tile.cu", "cluster.cu", "finalize.cu", "rechits.cu", "legacy.cu", "api.cu")
 HEADERS = (os.path.join(CSRC, "pix_common.cuh"), os.path.join(CSRC, "pix_device.cuh"), os.path.join(HERE, "..", "include", "pixclus.h"))
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",

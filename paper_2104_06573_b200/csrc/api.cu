@@ -88,6 +88,9 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.list_cap = (uint32_t)(Ec * M);
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
+  c.sbits = (uint32_t*)take((W / 32 + 16) * 4);
+  c.item_cap = (uint32_t)(W / 64 + 4 * Ec + 64);
+  c.items = (uint4*)take((size_t)c.item_cap * sizeof(uint4));
   c.n_clus = (uint32_t*)take(Ec * M * 4);
   c.n_runs = (uint32_t*)take(Ec * M * 4);
   c.t_a = (uint4*)take(2 * W * sizeof(uint4));
@@ -136,7 +139,7 @@ void bind_outputs(pix::Chunk& c, const pix_digis* d, const pix_clusters* k) {
 }
 
 // the launch sequence of one chunk
-constexpr int PROF_EVENTS = 6;  // families: init, fused, findrun, overflow, finalize (offsets + scatter)
+constexpr int PROF_EVENTS = 6;  // families: init, runs (runs + pack), tile, overflow, finalize (offsets + scatter)
 int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t words_bound, cudaStream_t s) {
   cudaEvent_t* ev = nullptr;
   if (h->profiling) {
@@ -151,9 +154,9 @@ int run_chunk(pix_handle* h, const pix::Chunk& c, uint32_t n_total, uint32_t wor
   }
   pix::launch_init(c, n_total, h->n_sm, s);
   if (ev) cudaEventRecord(ev[1], s);
-  pix::launch_fused(c, words_bound, h->n_sm, s);
+  pix::launch_runs(c, words_bound, h->n_sm, s);
   if (ev) cudaEventRecord(ev[2], s);
-  pix::launch_findrun(c, h->n_sm, s);
+  pix::launch_tile(c, h->n_sm, s);
   if (ev) cudaEventRecord(ev[3], s);
   pix::launch_overflow(c, h->n_sm, s);
   if (ev) cudaEventRecord(ev[4], s);
@@ -185,8 +188,7 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   h->F = F; h->M = M; h->p = *params;
   cudaError_t e = cudaGetDevice(&h->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
-  if (e == cudaSuccess) e = pix::configure_fused_kernel();
-  if (e == cudaSuccess) e = pix::configure_findrun_kernel();
+  if (e == cudaSuccess) e = pix::configure_tile_kernel();
   if (e == cudaSuccess) e = pix::configure_finalize_kernel();
   if (e == cudaSuccess) e = pix::configure_overflow_kernel();
   if (e != cudaSuccess) { delete h; cudaGetLastError(); return PIX_ERR_CUDA; }

@@ -37,7 +37,11 @@ constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus;
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
        EC_PRECUT, EC_PUSHED /* runs the event has put on the task lists (at most M) */, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_TEMP_COUNT = 8, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_TEMP_COUNT = 8, CTL_ITEM_COUNT = 9, CTL_WORDS = 16 };
+// work items of the tile kernel (runs.cu packs them, tile.cu takes them): x = global index of the first word,
+// y = words | flags << 16, z = event (launch-group relative) | FED of the first word << 16
+constexpr uint32_t TILE_WORDS = 1024, ITEM_WIN = 992, ITEM_WIN2 = 224, ITEM_RUNS = 255;
+constexpr uint32_t ITEM_DECODE_ONLY = 1u, ITEM_LONG_HEAD = 2u;
 
 // Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
 //   x = module | bad << 16 | scol << 24     bad: 0, ST_ERR_LINK or ST_ERR_ROC; scol = +1 / -1 (int8)
@@ -80,6 +84,9 @@ struct Chunk {
   uint32_t list_cap;        // (e1-e0)*M: every event lists at most M runs (push_run)
   uint32_t* chunk_seg;      // [cap_words/128 + 2] segment (event_rel*F + fed) of the chunk's first word
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
+  uint32_t* sbits;          // [cap_words/32 + 16] run-start bits, bit (g - T0) (runs.cu)
+  uint4* items;             // [item_cap] work items of the tile kernel
+  uint32_t item_cap;
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module
   uint32_t* n_runs;         // [(e1-e0)*M] runs of the module (more than one: the event is NONCONTIGUOUS, S11)
   // temp cluster records: every window / run takes a stretch of the area (alloc_temp) and leaves its start in t_base,
@@ -106,6 +113,9 @@ __device__ __forceinline__ void put_temp(const Chunk& c, uint32_t i, uint32_t fi
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream);
 void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
 void launch_findrun(const Chunk& c, int n_sm, cudaStream_t stream);
+void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
+void launch_tile(const Chunk& c, int n_sm, cudaStream_t stream);
+cudaError_t configure_tile_kernel();
 
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);

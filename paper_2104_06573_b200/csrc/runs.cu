@@ -1,0 +1,239 @@
+// runs.cu -- a3 of the Clusters path ("clusters the pixels on each detector module": the module
+// boundaries come first) as a streaming pre-pass, and the packing of module runs into work items for the tile
+// kernel (tile.cu).  DESIGN.md S11, S12.
+//
+// runs_kernel: one warp per 128 raw words, four consecutive words per lane (one 128-bit load).  A word is decoded as
+// far as its status and module (cabling gather only); a decodable word starts a run when its (event, module) differs
+// from the previous decodable word's.  Output: one start bit per word (bit g - T0 of sbits, T0 = first word of the
+// launch group rounded down to 128), module_first / module_end / the per-module run count (run_start, run_end).
+// The previous decodable word before a chunk is searched backwards, 32 words at a time, never beyond the start of the
+// event (an earlier event's word never continues a run; segfill_kernel closes every event's last run).
+//
+// pack_kernel: one warp per event walks the event's start bits and cuts it into items: maximal stretches of whole
+// runs of at most ITEM_WIN words (greedy: the next item starts at the last run start inside the window), at most
+// ITEM_RUNS runs each.  A run longer than TILE_WORDS words is cut into equal pieces that the tile kernel only decodes;
+// the first piece carries ITEM_LONG_HEAD and the tile kernel hands the run to the block-per-run kernel (cluster.cu).
+// Any two consecutive items of an event cover more than ITEM_WIN2 words, which bounds the item list.
+// Nothing here is shared with oracle/.
+#include "pix_common.cuh"
+#include "pix_device.cuh"
+
+namespace pix {
+
+namespace {
+
+constexpr uint32_t HC = CHUNK_WORDS, FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
+
+__global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk c) {
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
+  const uint32_t* __restrict__ segB = c.segB;
+  const uint32_t gBeg = segB[0], gEnd = segB[S];
+  if (gBeg >= gEnd) return;
+  const uint32_t T0 = gBeg & ~(HC - 1u);
+  const uint32_t n_chunks = (gEnd - T0 + HC - 1u) / HC;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  const uint32_t nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t ci = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; ci < n_chunks; ci += nwarp) {
+    const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
+    const uint32_t sg0 = c.chunk_seg[ci];
+    const uint32_t er0 = div_F(c, sg0), fed0 = sg0 - er0 * F;
+    const uint32_t nextB0 = segB[sg0 + 1u];
+    const bool all_in = b >= gBeg && b + HC <= gEnd;
+    const bool one_seg = all_in && b + HC <= nextB0;
+    uint4 wv = make_uint4(0u, 0u, 0u, 0u);
+    if (all_in) wv = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
+    else {
+      if (g0 >= gBeg && g0 < gEnd) wv.x = __ldg(c.words + g0);
+      if (g0 + 1u >= gBeg && g0 + 1u < gEnd) wv.y = __ldg(c.words + g0 + 1u);
+      if (g0 + 2u >= gBeg && g0 + 2u < gEnd) wv.z = __ldg(c.words + g0 + 2u);
+      if (g0 + 3u >= gBeg && g0 + 3u < gEnd) wv.w = __ldg(c.words + g0 + 3u);
+    }
+    // ---- the last decodable word before the chunk, inside the event of the chunk's first word
+    uint32_t carry_key = NOKEY, carry_g = 0u;
+    {
+      const uint32_t gw = b < gBeg ? gBeg : b, evb = segB[er0 * F];
+      uint32_t g = gw;  // words [evb, g) are still to be searched, backwards
+      while (g > evb) {
+        const bool in = lane < g - evb;
+        const uint32_t gi = g - 1u - lane;
+        uint32_t key = NOKEY;
+        if (in) {
+          uint32_t sg = sg0;
+          while (segB[sg] > gi) --sg;
+          uint32_t m, r, cc;
+          if (decode_word(c.cab, __ldg(c.words + gi), (sg - er0 * F) << 11, m, r, cc) == ST_OK) key = (er0 << 16) | m;
+        }
+        const uint32_t bal = __ballot_sync(FULL, key != NOKEY);
+        if (bal) {
+          const int src = __ffs(bal) - 1;
+          carry_key = __shfl_sync(FULL, key, src);
+          carry_g = g - 1u - (uint32_t)src;
+          break;
+        }
+        g = (g - evb > 32u) ? g - 32u : evb;
+      }
+    }
+    const uint32_t w[4] = {wv.x, wv.y, wv.z, wv.w};
+    uint32_t key[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t g = g0 + j;
+      const bool exists = all_in || (g >= gBeg && g < gEnd);
+      uint32_t er = er0, fed = fed0;
+      if (!one_seg && exists) {  // rare: a FED / event boundary inside the chunk
+        uint32_t sg = sg0;
+        while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
+        er = div_F(c, sg); fed = sg - er * F;
+      }
+      uint32_t m, r, cc;
+      const uint32_t st = decode_word(c.cab, w[j], fed << 11, m, r, cc);
+      key[j] = (exists && st == ST_OK) ? ((er << 16) | m) : NOKEY;
+    }
+    // a word starts a run when its (event, module) differs from the previous decodable word's
+    uint32_t tkey = NOKEY, tj = 0u;  // the lane's last decodable word
+#pragma unroll
+    for (int j = 0; j < 4; ++j) if (key[j] != NOKEY) { tkey = key[j]; tj = j; }
+    const uint32_t has = __ballot_sync(FULL, tkey != NOKEY);
+    const uint32_t below_l = has & lt_mask;
+    const int src = below_l ? 31 - __clz(below_l) : 0;
+    uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = b + 4u * (uint32_t)src + __shfl_sync(FULL, tj, src);
+    if (!below_l) { pkey = carry_key; pg = carry_g; }
+    uint32_t startmask = 0u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (key[j] == NOKEY) continue;
+      if (key[j] != pkey) {
+        startmask |= 1u << j;
+        run_start(c, key[j], g0 + j);
+        if (pkey != NOKEY) run_end(c, pkey, pg);
+      }
+      pkey = key[j]; pg = g0 + j;
+    }
+    // start bits of the chunk: lane l's nibble sits at bit 4 l of the 128-bit row
+    const uint32_t nib = startmask << (4u * (lane & 7u));
+#pragma unroll
+    for (uint32_t k = 0; k < 4u; ++k) {
+      const uint32_t v = __reduce_or_sync(FULL, (lane >> 3) == k ? nib : 0u);
+      if (lane == k) c.sbits[ci * 4u + k] = v;
+    }
+  }
+}
+
+// highest start bit in (lo, hi] (bit indices relative to T0; hi - lo <= 992 so the range spans at most 32 words), or NO_INDEX
+__device__ __forceinline__ uint32_t last_start(const uint32_t* __restrict__ sbits, uint32_t lo, uint32_t hi, uint32_t lane) {
+  const int w_hi = (int)(hi >> 5), w_lo = (int)(lo >> 5), wi = w_hi - (int)lane;
+  uint32_t v = 0u;
+  if (wi >= w_lo) {
+    v = sbits[wi];
+    if (wi == w_hi) v &= (2u << (hi & 31u)) - 1u;
+    if (wi == w_lo) v &= ~((2u << (lo & 31u)) - 1u);
+  }
+  const uint32_t bal = __ballot_sync(FULL, v != 0u);
+  if (!bal) return NO_INDEX;
+  const int src = __ffs(bal) - 1;
+  const uint32_t vv = __shfl_sync(FULL, v, src);
+  return (uint32_t)(w_hi - src) * 32u + 31u - (uint32_t)__clz(vv);
+}
+// lowest start bit in (lo, hi], same limits
+__device__ __forceinline__ uint32_t first_start(const uint32_t* __restrict__ sbits, uint32_t lo, uint32_t hi, uint32_t lane) {
+  const int w_hi = (int)(hi >> 5), w_lo = (int)(lo >> 5), wi = w_lo + (int)lane;
+  uint32_t v = 0u;
+  if (wi <= w_hi) {
+    v = sbits[wi];
+    if (wi == w_hi) v &= (2u << (hi & 31u)) - 1u;
+    if (wi == w_lo) v &= ~((2u << (lo & 31u)) - 1u);
+  }
+  const uint32_t bal = __ballot_sync(FULL, v != 0u);
+  if (!bal) return NO_INDEX;
+  const int src = __ffs(bal) - 1;
+  const uint32_t vv = __shfl_sync(FULL, v, src);
+  return (uint32_t)(w_lo + src) * 32u + (uint32_t)__ffs(vv) - 1u;
+}
+// start bits in [lo, hi), hi - lo <= 1024
+__device__ __forceinline__ uint32_t count_starts(const uint32_t* __restrict__ sbits, uint32_t lo, uint32_t hi, uint32_t lane) {
+  if (hi <= lo) return 0u;
+  const uint32_t last = hi - 1u;
+  const int w_hi = (int)(last >> 5), w_lo = (int)(lo >> 5);
+  uint32_t n = 0u;
+  for (int wi = w_lo + (int)lane; wi <= w_hi; wi += 32) {
+    uint32_t v = sbits[wi];
+    if (wi == w_hi) v &= (2u << (last & 31u)) - 1u;
+    if (wi == w_lo) v &= ~((1u << (lo & 31u)) - 1u);
+    n += __popc(v);
+  }
+  return __reduce_add_sync(FULL, n);
+}
+
+__global__ void __launch_bounds__(128) pack_kernel(const __grid_constant__ Chunk c) {
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t F = c.F, Ec = c.e1 - c.e0, S = Ec * F;
+  const uint32_t* __restrict__ segB = c.segB;
+  const uint32_t gBeg = segB[0], gEnd = segB[S];
+  if (gBeg >= gEnd) return;
+  const uint32_t T0 = gBeg & ~(HC - 1u);
+  const uint32_t* __restrict__ sbits = c.sbits;
+  const uint32_t nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t er = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; er < Ec; er += nwarp) {
+    const uint32_t evb = segB[er * F], eve = segB[(er + 1u) * F];
+    uint32_t sg = er * F;
+    uint32_t s = evb;
+    auto emit = [&](uint32_t g, uint32_t len, uint32_t flags) {
+      while (sg + 1u < (er + 1u) * F && segB[sg + 1u] <= g) ++sg;
+      if (lane == 0) {
+        const uint32_t i = atomicAdd(c.ctl + CTL_ITEM_COUNT, 1u);
+        if (i < c.item_cap) c.items[i] = make_uint4(g, len | (flags << 16), er | ((sg - er * F) << 16), 0u);
+      }
+    };
+    while (s < eve) {
+      const uint32_t rs = s - T0, rlast = eve - 1u - T0;  // bit indices of the item's first word and of the event's last word
+      uint32_t win = ITEM_WIN;
+      uint32_t nxt;  // bit index of the next item's first word
+      while (true) {
+        if (rlast - rs < win) { nxt = rlast + 1u; }  // the rest of the event fits
+        else {
+          nxt = last_start(sbits, rs, rs + win, lane);
+        }
+        if (nxt == NO_INDEX || win == ITEM_WIN2) break;
+        if (count_starts(sbits, rs, nxt, lane) <= ITEM_RUNS) break;
+        win = ITEM_WIN2;  // too many runs: a shorter item (at most ITEM_WIN2 + 1 <= ITEM_RUNS runs)
+      }
+      if (nxt != NO_INDEX) {
+        emit(s, nxt - rs, 0u);
+        s = T0 + nxt;
+        continue;
+      }
+      // no run starts in (s, s + ITEM_WIN]: one run (or a stretch of undecodable words) longer than that
+      uint32_t p = rs + win;
+      nxt = NO_INDEX;
+      while (nxt == NO_INDEX && p < rlast) {
+        const uint32_t q = (rlast - p > 992u) ? p + 992u : rlast;
+        nxt = first_start(sbits, p, q, lane);
+        p = q;
+      }
+      if (nxt == NO_INDEX) nxt = rlast + 1u;
+      const uint32_t L = nxt - rs;
+      if (L <= TILE_WORDS) emit(s, L, 0u);
+      else {
+        const bool head = (sbits[rs >> 5] >> (rs & 31u)) & 1u;
+        const uint32_t pieces = (L + TILE_WORDS - 1u) / TILE_WORDS, plen = (L + pieces - 1u) / pieces;
+        for (uint32_t k = 0, o = 0; o < L; ++k, o += plen)
+          emit(s + o, (L - o < plen) ? L - o : plen, ITEM_DECODE_ONLY | ((k == 0 && head) ? ITEM_LONG_HEAD : 0u));
+      }
+      s = T0 + nxt;
+    }
+  }
+}
+
+}  // namespace
+
+void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
+  uint64_t nb = ((uint64_t)words_bound + 2 * HC + 8 * HC - 1) / (8 * HC);
+  if (nb < 1) nb = 1;
+  if (nb > (uint64_t)n_sm * 16) nb = (uint64_t)n_sm * 16;
+  runs_kernel<<<(int)nb, 256, 0, stream>>>(c);
+  const uint32_t Ec = c.e1 - c.e0;
+  pack_kernel<<<(int)((Ec + 3u) / 4u), 128, 0, stream>>>(c);
+}
+
+}  // namespace pix

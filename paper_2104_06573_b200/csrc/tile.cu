@@ -1,0 +1,407 @@
+// tile.cu -- the tile kernel of the Clusters path ("unpacks them, calibrates the individual pixels, and
+// clusters the pixels on each detector module"): a1 decode (S1-S6), a2 calibrate (S7-S9), a4 findClus (S10,
+// S13) and a5 sums / charge cut / renumber / temp records (S9, S14, S18) for one work item per block.
+//
+// A work item (runs.cu) is a stretch of at most 1024 raw words holding whole module runs.  A block of 256 threads
+// takes it with four words per thread (word p = tid + 256 j, so every access is coalesced); the word's key, charge
+// and root stay in registers through all phases, only the tables live in shared memory:
+//   P1  decode, calibrate, store module / row / col / charge; run index from the start bits; insert into the
+//       position hash: key = run | row | col -> bucket (10 bits) + tag (15 bits), exact; a bucket holds four 16-bit
+//       tags (one 64-bit load per lookup) plus four more in a second level that is only read when the first is full;
+//       slots are handed out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
+//   P2  duplicates (S10: the lowest word owns the pixel; rare path), then four forward-neighbour lookups per live
+//       pixel and lock-free hook-and-descend unions on the labels (pix_device.cuh)
+//   P3  root of every live pixel; charge | pixel count, charge*col, charge*row added into the root's accumulators
+//   P4  roots: Q >= cut survives (ballot bitmap, block scan), numbered per run in word order; temp records
+//   P5  final status and clus, per-run cluster count and temp base, per-event counters
+// Runs are separated by block barriers only (about ten per 1024 words); all warps of a block walk the same code at
+// the same time, and the whole kernel fits the instruction cache.
+// What the kernel cannot take goes to the block-per-run kernel (cluster.cu): runs longer than 1024 words (decoded
+// here, ITEM_DECODE_ONLY), items whose hash overflows a bucket (8 keys), runs with a cluster charge beyond Q_SAFE.
+// Nothing here is shared with oracle/.
+#include "pix_common.cuh"
+#include "pix_device.cuh"
+
+namespace pix {
+
+namespace {
+
+constexpr int NT = 256, NJ = 4, BLOCKS_PER_SM = 4;
+constexpr uint32_t FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
+constexpr uint32_t NBK = 1024;                       // buckets
+constexpr uint32_t HMASK = (1u << 25) - 1u;          // key: run (8) | row (8) | col (9)
+constexpr uint32_t HMUL = 0x9E3779B1u;
+constexpr uint32_t D_E = (1u * HMUL) & HMASK, D_SW = (511u * HMUL) & HMASK, D_S = (512u * HMUL) & HMASK, D_SE = (513u * HMUL) & HMASK;
+constexpr uint32_t MARK = 0xFFFFFFFDu;               // label of a word that is not a live pixel
+constexpr uint32_t NONE = 0xFFFFu, NO_ID = 0xFFFFu;
+constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;      // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
+constexpr uint32_t BIG_RUN = 256u;                   // runs this long count their pixels in a word of their own
+
+struct __align__(16) TileSmem {
+  uint2 tagsA[NBK];          // first level: 4 x (0x8000 | tag), 0 = free
+  uint16_t idsA[4 * NBK];    // word of the entry | below_threshold << 15; after P2: lid (local id of a root, or NO_ID)
+  uint32_t tagsB[NBK];       // second level, 4 entries per 4 buckets: tag | (bucket & 3) << 16 | word << 18 | below << 28
+  uint32_t cnt[NBK / 4];     // entries per bucket, one byte each
+  uint32_t cntB[NBK / 16];   // entries per second-level bucket, one byte each (tagsB is never cleared)
+  uint32_t edge[NT / 32][3 * 128];  // per warp: the edges its words found, a | b << 16
+  uint32_t label[TILE_WORDS];
+  uint32_t qn[TILE_WORDS], sx[TILE_WORDS], sy[TILE_WORDS], npx[TILE_WORDS];
+  uint32_t bits[32], pre[32];        // run-start bits of the item, run starts before each word of bits
+  uint32_t survb[36], spre[36];      // roots that survive the cut, survivors before each word of survb
+  uint16_t run_pos[256], run_mod[256];
+  uint8_t run_big[256], run_bad[256];
+  uint32_t n_runs, wbase, pad[2];
+};
+static_assert(sizeof(TileSmem) <= 57344 - 64, "four blocks per SM");
+
+__device__ __forceinline__ uint32_t zero_half(uint32_t x, uint32_t ww) {
+  const uint32_t y = x ^ ww;
+  return (y - 0x00010001u) & ~y & 0x80008000u;  // bit 15 / 31 set where a half of x equals the half of ww (the lower set bit is exact)
+}
+
+__device__ __forceinline__ uint32_t countB(const TileSmem& s, uint32_t bB) {
+  const uint32_t n = (s.cntB[bB >> 2] >> ((bB & 3u) * 8u)) & 0xFFu;
+  return n > 4u ? 4u : n;
+}
+__device__ __noinline__ uint32_t lookup_B(const TileSmem& s, uint32_t b, uint32_t want) {
+  const uint32_t bB = b >> 2, n = countB(s, bB), w18 = want | ((b & 3u) << 16);
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t e = s.tagsB[bB * 4u + i];
+    if ((e & 0x3FFFFu) == w18) return (e >> 28) ? NONE : ((e >> 18) & 0x3FFu);
+  }
+  return NONE;
+}
+
+// the live pixel with hash h, or NONE
+__device__ __forceinline__ uint32_t lookup(const TileSmem& s, uint32_t h) {
+  const uint32_t b = h >> 15, want = (h & 0x7FFFu) | 0x8000u, ww = want * 0x00010001u;
+  const uint2 x = s.tagsA[b];
+  const uint32_t z0 = zero_half(x.x, ww), z1 = zero_half(x.y, ww);
+  const bool hit = (z0 | z1) != 0u;
+  const uint32_t k = z0 ? ((z0 & 0x8000u) ? 0u : 1u) : ((z1 & 0x8000u) ? 2u : 3u);
+  uint32_t idv = 0x8000u;
+  if (hit) idv = s.idsA[b * 4u + k];
+  uint32_t res = (idv >> 15) ? NONE : (idv & 0x3FFu);
+  if (!hit && (x.y >> 31)) res = lookup_B(s, b, want);  // rare: the first level is full
+  return res;
+}
+
+// rare: the pixel of word p appears more than once in its bucket.  The lowest word owns it (S10); every entry of the
+// pixel is made to name the owner, so a lookup may take any of them.  Returns true when p is not the owner.
+__device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want, uint32_t p, uint32_t k_own) {
+  const uint16_t* tA = reinterpret_cast<const uint16_t*>(s.tagsA) + b * 4u;
+  const uint32_t bB = b >> 2, nB = tA[3] ? countB(s, bB) : 0u, w18 = want | ((b & 3u) << 16);
+  uint32_t best = 0xFFFFFFFFu;  // word << 1 | below
+  for (uint32_t i = 0; i < 4u; ++i) {
+    if (tA[i] != want) continue;
+    const uint32_t idv = s.idsA[b * 4u + i], v = ((idv & 0x3FFu) << 1) | (idv >> 15);
+    best = v < best ? v : best;
+  }
+  for (uint32_t i = 0; i < nB; ++i) {
+    const uint32_t e = s.tagsB[bB * 4u + i];
+    if ((e & 0x3FFFFu) != w18) continue;
+    const uint32_t v = (((e >> 18) & 0x3FFu) << 1) | (e >> 28);
+    best = v < best ? v : best;
+  }
+  if ((best >> 1) == p) return false;
+  if (k_own < 4u) s.idsA[b * 4u + k_own] = (uint16_t)((best >> 1) | ((best & 1u) << 15));
+  else s.tagsB[bB * 4u + k_own - 4u] = w18 | ((best >> 1) << 18) | ((best & 1u) << 28);
+  return true;
+}
+
+__global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_constant__ Chunk c) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  TileSmem& s = *reinterpret_cast<TileSmem*>(smem_raw);
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
+  const uint32_t* __restrict__ segB = c.segB;
+  const uint32_t gBeg = segB[0], gEnd = segB[S];
+  if (gBeg >= gEnd) return;
+  const uint32_t T0 = gBeg & ~(CHUNK_WORDS - 1u);
+  uint32_t n_items = c.ctl[CTL_ITEM_COUNT];
+  n_items = n_items < c.item_cap ? n_items : c.item_cap;
+  const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
+  uint16_t* const tagA16 = reinterpret_cast<uint16_t*>(s.tagsA);
+  uint16_t* const lid = s.idsA;
+
+  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const uint4 item = c.items[it];
+    const uint32_t g0 = item.x, len = item.y & 0xFFFFu, iflags = item.y >> 16, er = item.z & 0xFFFFu, fed0 = item.z >> 16;
+    uint32_t w[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j;
+      w[j] = p < len ? __ldg(c.words + g0 + p) : 0u;
+    }
+    __syncthreads();  // the previous item is done with the shared tables
+    // ================================================================== P0: clear; start bits of the item
+    {
+      const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+      uint4* tA = reinterpret_cast<uint4*>(s.tagsA);
+      tA[tid] = z4; tA[tid + NT] = z4;
+      uint4* sm = reinterpret_cast<uint4*>(s.qn);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) sm[tid + NT * k] = z4;
+      if (tid < NBK / 16 + NBK / 64) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
+      if (tid < 128) reinterpret_cast<uint32_t*>(s.run_big)[tid] = 0u;  // run_big and run_bad
+      if (warp == 0) {
+        const uint32_t rel = g0 - T0, wq = rel >> 5;
+        uint32_t v = __funnelshift_r(c.sbits[wq + lane], c.sbits[wq + lane + 1u], rel & 31u);
+        const uint32_t nb = len > 32u * lane ? len - 32u * lane : 0u;
+        v &= nb >= 32u ? FULL : ((1u << nb) - 1u);
+        s.bits[lane] = v;
+        uint32_t pc = __popc(v), inc = pc;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const uint32_t o = __shfl_up_sync(FULL, inc, d);
+          if (lane >= (uint32_t)d) inc += o;
+        }
+        s.pre[lane] = inc - pc;
+        if (lane == 31) s.n_runs = inc;
+      }
+    }
+    __syncthreads();
+    // ================================================================== P1: decode, calibrate, insert
+    const uint32_t ebase = segB[er * F];
+    const bool one_seg = g0 + len <= segB[er * F + fed0 + 1u];
+    const bool cluster_it = !(iflags & ITEM_DECODE_ONLY);
+    uint32_t key[NJ], chg[NJ];
+    uint32_t fl = 0u;    // per word j: bit j below threshold, bit 4 + j duplicate
+    uint32_t kpack = 0u; // per word j: its slot in the bucket (4 bits)
+    bool fail = false;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j, g = g0 + p;
+      const bool valid = p < len;
+      uint32_t fed = fed0;
+      if (!one_seg && valid) {  // a FED boundary inside the item
+        uint32_t sg = er * F + fed0;
+        while (sg + 1u < (er + 1u) * F && segB[sg + 1u] <= g) ++sg;
+        fed = sg - er * F;
+      }
+      uint32_t m, row, col;
+      const uint32_t st = decode_word(c.cab, w[j], fed << 11, m, row, col);
+      const bool ok = valid && st == ST_OK;
+      int32_t e = 0;
+      if (ok) e = calibrate(c, w[j] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
+      else { m = row = col = 0xFFFFu; }
+      if (valid) {
+        c.d_module[g] = (uint16_t)m; c.d_row[g] = (uint16_t)row; c.d_col[g] = (uint16_t)col; c.d_charge[g] = e;
+        if (!ok) {  // undecodable words are finished here
+          c.d_status[g] = (uint8_t)st; c.d_clus[g] = -1;
+          atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
+        }
+      }
+      const uint32_t bw = s.bits[j * 8 + warp];
+      const uint32_t r = s.pre[j * 8 + warp] + __popc(bw & le_mask) - 1u;  // a decodable word lies in a run: r >= 0
+      const bool below = e < c.thr;  // S9
+      key[j] = NOKEY; chg[j] = (uint32_t)e;
+      if (ok) {
+        key[j] = (r << 17) | (row << 9) | col;
+        if ((bw >> lane) & 1u) { s.run_pos[r] = (uint16_t)p; s.run_mod[r] = (uint16_t)m; }
+        if (below) fl |= 1u << j;
+        if (cluster_it) {
+          const uint32_t h = (key[j] * HMUL) & HMASK, b = h >> 15, sh8 = (b & 3u) * 8u;
+          const uint32_t k = (atomicAdd(&s.cnt[b >> 2], 1u << sh8) >> sh8) & 0xFFu;
+          const uint16_t tag = (uint16_t)((h & 0x7FFFu) | 0x8000u), idv = (uint16_t)(p | (below ? 0x8000u : 0u));
+          uint32_t kk = k;
+          if (k < 4u) { tagA16[b * 4u + k] = tag; s.idsA[b * 4u + k] = idv; }
+          else {  // rare: the bucket's first level is full
+            const uint32_t bB = b >> 2, shB = (bB & 3u) * 8u;
+            const uint32_t kb = (atomicAdd(&s.cntB[bB >> 2], 1u << shB) >> shB) & 0xFFu;
+            if (kb < 4u) s.tagsB[bB * 4u + kb] = tag | ((b & 3u) << 16) | (p << 18) | (below ? 1u << 28 : 0u);
+            else fail = true;
+            kk = 4u + (kb < 4u ? kb : 0u);
+          }
+          kpack |= kk << (4 * j);
+        }
+      }
+      s.label[p] = (ok && !below) ? p : MARK;
+    }
+    if (!cluster_it) {  // a piece of a run longer than the tile: the block-per-run kernel clusters it
+      if ((iflags & ITEM_LONG_HEAD) && tid == 0 && key[0] != NOKEY) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[0]);
+      continue;
+    }
+    const uint32_t R = s.n_runs;
+    if (__syncthreads_or(fail)) {  // a bucket with more than 8 keys: the block-per-run kernel takes the runs of the item
+      if (tid < R) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[tid]);
+      continue;
+    }
+    // ================================================================== P2: duplicates; neighbours -> unions
+    {
+      uint32_t cand = 0u;  // bit j: the pixel of word j may sit in its bucket more than once
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+        const uint32_t h = (key[j] * HMUL) & HMASK, b = h >> 15, ww = ((h & 0x7FFFu) | 0x8000u) * 0x00010001u;
+        const uint2 x = s.tagsA[b];
+        const bool cj = key[j] != NOKEY && (__popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww)) >= 2 || (x.y >> 31));
+        cand |= cj ? 1u << j : 0u;
+      }
+      if (__syncthreads_or(cand != 0u)) {
+        if (cand) {
+#pragma unroll 1
+          for (int j = 0; j < NJ; ++j) {
+            if (!((cand >> j) & 1u)) continue;
+            const uint32_t p = tid + NT * j;
+            const uint32_t h = (key[j] * HMUL) & HMASK, b = h >> 15;
+            if (resolve_dup(s, b, (h & 0x7FFFu) | 0x8000u, p, (kpack >> (4 * j)) & 15u)) { fl |= 16u << j; s.label[p] = MARK; }
+          }
+        }
+        __syncthreads();
+      }
+    }
+    if (tid < R) {
+      const uint32_t e1 = tid + 1u < R ? s.run_pos[tid + 1u] : len;
+      s.run_big[tid] = (e1 - s.run_pos[tid] >= BIG_RUN) ? 1 : 0;
+    }
+    __syncwarp();
+    {
+      // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1); col 416..511 and row 160..255
+      // never occur, so no bounds checks.  When S is live, SW and SE are joined to it by their own E edges; when E is
+      // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the
+      // edges go to the warp's list, and the list is united with all lanes busy.
+      uint32_t* const el = s.edge[warp];
+      uint32_t ne = 0u;
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+        const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
+        const uint32_t p = tid + NT * j;
+        const uint32_t h = (key[j] * HMUL) & HMASK;
+        const uint32_t nE = lookup(s, (h + D_E) & HMASK), nS = lookup(s, (h + D_S) & HMASK);
+        const uint32_t nSW = lookup(s, (h + D_SW) & HMASK), nSE = lookup(s, (h + D_SE) & HMASK);
+        const uint32_t t1 = nS != NONE ? nS : nSW;
+        const bool f0 = live && nE != NONE, f1 = live && t1 != NONE, f2 = live && nS == NONE && nE == NONE && nSE != NONE;
+        const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
+        if (f0) el[ne + __popc(m0 & lt_mask)] = p | (nE << 16);
+        ne += __popc(m0);
+        if (f1) el[ne + __popc(m1 & lt_mask)] = p | (t1 << 16);
+        ne += __popc(m1);
+        if (f2) el[ne + __popc(m2 & lt_mask)] = p | (nSE << 16);
+        ne += __popc(m2);
+      }
+      __syncwarp();
+      for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
+        if (i0 + lane < ne) {
+          const uint32_t e = el[i0 + lane];
+          hook(s.label, e & 0xFFFFu, e >> 16);
+        }
+        __syncwarp();
+      }
+    }
+    __syncthreads();
+    // ================================================================== P3: roots; sums
+    uint32_t root[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      root[j] = NONE;
+      if (key[j] == NOKEY || ((fl >> j) & 0x11u)) continue;
+      const uint32_t p = tid + NT * j;
+      uint32_t r = s.label[p];
+      while (true) { const uint32_t n = s.label[r]; if (n == r) break; r = n; }
+      root[j] = r;
+      const uint32_t big = s.run_big[key[j] >> 17];
+      atomicAdd(&s.qn[r], big ? chg[j] : (chg[j] | (1u << 24)));  // below BIG_RUN words a cluster has at most 255 pixels and Q < 2^24
+      atomicAdd(&s.sx[r], chg[j] * (key[j] & 511u));
+      atomicAdd(&s.sy[r], chg[j] * ((key[j] >> 9) & 255u));
+      if (big) atomicAdd(&s.npx[r], 1u);
+    }
+    __syncthreads();
+    // ================================================================== P4: cut, renumber, temp records
+    uint32_t surv = 0u;  // bit j: word j is a root that survives the cut
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j;
+      bool sv = false;
+      if (root[j] == p) {
+        const uint32_t run = key[j] >> 17;
+        const uint32_t a = s.qn[p], Q = s.run_big[run] ? a : (a & 0xFFFFFFu);
+        sv = (int32_t)Q >= c.cut;  // S9: equality keeps (Q < 2^31)
+        if (Q > Q_SAFE) s.run_bad[run] = 1;  // 32-bit weighted sums may have wrapped
+      }
+      const uint32_t bal = __ballot_sync(FULL, sv);
+      if (lane == 0) s.survb[j * 8 + warp] = bal;
+      surv |= sv ? 1u << j : 0u;
+    }
+    __syncthreads();
+    if (warp == 0) {
+      const uint32_t pc = __popc(s.survb[lane]);
+      uint32_t inc = pc;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(FULL, inc, d);
+        if (lane >= (uint32_t)d) inc += o;
+      }
+      s.spre[lane] = inc - pc;
+      if (lane == 31) { s.spre[32] = inc; s.survb[32] = 0u; s.wbase = alloc_temp(c, inc); }
+    }
+    __syncthreads();
+    const uint32_t wbase = s.wbase;
+    auto rank_before = [&](uint32_t pos) { return s.spre[pos >> 5] + __popc(s.survb[pos >> 5] & ((1u << (pos & 31u)) - 1u)); };
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j;
+      if (root[j] != p) continue;
+      uint32_t id = NO_ID;
+      if ((surv >> j) & 1u) {
+        const uint32_t run = key[j] >> 17, big = s.run_big[run];
+        const uint32_t a = s.qn[p], Q = big ? a : (a & 0xFFFFFFu), np = big ? s.npx[p] : (a >> 24);
+        const uint32_t rank = rank_before(p);
+        id = rank - rank_before(s.run_pos[run]);
+        const float fq = (float)Q;  // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
+        put_temp(c, wbase + rank, g0 + p - ebase, np, Q, __fdividef((float)s.sx[p], fq), __fdividef((float)s.sy[p], fq));
+      }
+      lid[p] = (uint16_t)id;
+    }
+    __syncthreads();
+    // ================================================================== P5: final status and clus, run outputs, counters
+    uint32_t cntA = 0u, cntB = 0u, cntP = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      if (key[j] == NOKEY) continue;
+      if (s.run_bad[key[j] >> 17]) continue;
+      const uint32_t p = tid + NT * j, g = g0 + p;
+      uint32_t so; int32_t cl = -1;
+      if ((fl >> j) & 16u) { so = ST_DUP; cntA += 1u; }
+      else if ((fl >> j) & 1u) { so = ST_BELOW; cntA += 0x10000u; }
+      else {
+        const uint32_t id = lid[root[j]];
+        if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
+        cntP += root[j] == p ? 1u : 0u;
+      }
+      c.d_status[g] = (uint8_t)so; c.d_clus[g] = cl;
+    }
+    if (tid < R) {
+      const uint32_t m = s.run_mod[tid];
+      if (s.run_bad[tid]) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, m);
+      else {
+        const uint32_t p0 = s.run_pos[tid], p1 = tid + 1u < R ? s.run_pos[tid + 1u] : len;
+        const uint32_t b0 = rank_before(p0);
+        const size_t mo = (size_t)er * c.M + m;
+        c.n_clus[mo] = rank_before(p1) - b0; c.t_base[mo] = wbase + b0;
+      }
+    }
+    {
+      const uint32_t a = __reduce_add_sync(FULL, cntA), bb = __reduce_add_sync(FULL, cntB), pp = __reduce_add_sync(FULL, cntP);
+      if (lane == 0) {
+        uint32_t* ec = c.ev_cnt + (size_t)er * EC_STRIDE;
+        if (a & 0xFFFFu) atomicAdd(ec + EC_DUP, a & 0xFFFFu);
+        if (a >> 16) atomicAdd(ec + EC_BELOW, a >> 16);
+        if (bb & 0xFFFFu) atomicAdd(ec + EC_OK, bb & 0xFFFFu);
+        if (bb >> 16) atomicAdd(ec + EC_CUT, bb >> 16);
+        if (pp) atomicAdd(ec + EC_PRECUT, pp);
+      }
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t configure_tile_kernel() {
+  return cudaFuncSetAttribute(tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
+}
+
+void launch_tile(const Chunk& c, int n_sm, cudaStream_t stream) {
+  tile_kernel<<<n_sm * BLOCKS_PER_SM, NT, sizeof(TileSmem), stream>>>(c);
+}
+
+}  // namespace pix
