@@ -28,53 +28,69 @@ namespace {
 
 constexpr int NT = 256, NJ = 4, BLOCKS_PER_SM = 4;
 constexpr uint32_t FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
-constexpr uint32_t NBK = 1024;                       // buckets
-constexpr uint32_t HMASK = (1u << 25) - 1u;          // key: run (8) | row (8) | col (9)
+constexpr uint32_t NBK = 2048, NBK_LOG2 = 11;        // buckets of 4 entries (load 0.5: a bucket is full for 0.2% of the lookups)
+// key: run (8) | row (8) | col (9) = 25 bits.  h = (key << 7) * HMUL mod 2^32: the top 25 bits are key * HMUL mod 2^25,
+// a bijection of the key; bucket = top 11 bits, tag = the next 14, so (bucket, tag) names the key exactly, and the hash
+// of a neighbour is h + a constant.
 constexpr uint32_t HMUL = 0x9E3779B1u;
-constexpr uint32_t D_E = (1u * HMUL) & HMASK, D_SW = (511u * HMUL) & HMASK, D_S = (512u * HMUL) & HMASK, D_SE = (513u * HMUL) & HMASK;
+constexpr uint32_t D_E = (1u << 7) * HMUL, D_SW = (511u << 7) * HMUL, D_S = (512u << 7) * HMUL, D_SE = (513u << 7) * HMUL;
 constexpr uint32_t MARK = 0xFFFFFFFDu;               // label of a word that is not a live pixel
 constexpr uint32_t NONE = 0xFFFFu, NO_ID = 0xFFFFu;
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;      // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
 constexpr uint32_t BIG_RUN = 256u;                   // runs this long count their pixels in a word of their own
+constexpr uint32_t ECAP = 3 * 64;                    // edges a warp lists before it unites them (two words per lane)
 
 struct __align__(16) TileSmem {
-  uint2 tagsA[NBK];          // first level: 4 x (0x8000 | tag), 0 = free
+  union {
+    uint2 tagsA[NBK];        // first level: 4 x (0x8000 | tag), 0 = free
+    struct { uint32_t qn[TILE_WORDS], sx[TILE_WORDS], sy[TILE_WORDS], npx[TILE_WORDS]; } sum;  // after P2: the roots' accumulators
+  };
   uint16_t idsA[4 * NBK];    // word of the entry | below_threshold << 15; after P2: lid (local id of a root, or NO_ID)
-  uint32_t tagsB[NBK];       // second level, 4 entries per 4 buckets: tag | (bucket & 3) << 16 | word << 18 | below << 28
+  uint32_t tagsB[1024];      // second level, 4 entries per 8 buckets: tag | (bucket & 7) << 16 | word << 19 | below << 29
   uint32_t cnt[NBK / 4];     // entries per bucket, one byte each
-  uint32_t cntB[NBK / 16];   // entries per second-level bucket, one byte each (tagsB is never cleared)
-  uint32_t edge[NT / 32][3 * 128];  // per warp: the edges its words found, a | b << 16
+  uint32_t cntB[64];         // entries per second-level bucket, one byte each (tagsB is never cleared)
+  uint32_t edge[NT / 32][ECAP];  // per warp: the edges its words found, a | b << 16
   uint32_t label[TILE_WORDS];
-  uint32_t qn[TILE_WORDS], sx[TILE_WORDS], sy[TILE_WORDS], npx[TILE_WORDS];
   uint32_t bits[32], pre[32];        // run-start bits of the item, run starts before each word of bits
-  uint32_t survb[36], spre[36];      // roots that survive the cut, survivors before each word of survb
+  uint32_t survb[32];                // roots that survive the cut
   uint16_t run_pos[256], run_mod[256];
   uint8_t run_big[256], run_bad[256];
   uint32_t n_runs, wbase, pad[2];
 };
 static_assert(sizeof(TileSmem) <= 57344 - 64, "four blocks per SM");
+static_assert(sizeof(uint2) * NBK == 4 * 4 * TILE_WORDS, "the accumulators take the place of the first-level tags");
 
+__device__ __forceinline__ uint32_t hash_of(uint32_t key) { return (key << 7) * HMUL; }
+__device__ __forceinline__ uint32_t bucket_of(uint32_t h) { return h >> (32 - NBK_LOG2); }
+__device__ __forceinline__ uint32_t want_of(uint32_t h) { return ((h >> 7) & 0x3FFFu) | 0x8000u; }
 __device__ __forceinline__ uint32_t zero_half(uint32_t x, uint32_t ww) {
   const uint32_t y = x ^ ww;
   return (y - 0x00010001u) & ~y & 0x80008000u;  // bit 15 / 31 set where a half of x equals the half of ww (the lower set bit is exact)
 }
-
 __device__ __forceinline__ uint32_t countB(const TileSmem& s, uint32_t bB) {
   const uint32_t n = (s.cntB[bB >> 2] >> ((bB & 3u) * 8u)) & 0xFFu;
   return n > 4u ? 4u : n;
 }
+// second level (rare): the live pixel, or NONE
 __device__ __noinline__ uint32_t lookup_B(const TileSmem& s, uint32_t b, uint32_t want) {
-  const uint32_t bB = b >> 2, n = countB(s, bB), w18 = want | ((b & 3u) << 16);
+  const uint32_t bB = b >> 3, n = countB(s, bB), w19 = want | ((b & 7u) << 16);
   for (uint32_t i = 0; i < n; ++i) {
     const uint32_t e = s.tagsB[bB * 4u + i];
-    if ((e & 0x3FFFFu) == w18) return (e >> 28) ? NONE : ((e >> 18) & 0x3FFu);
+    if ((e & 0x7FFFFu) == w19) return (e >> 29) ? NONE : ((e >> 19) & 0x3FFu);
   }
   return NONE;
+}
+// second level (rare): entries of the pixel
+__device__ __noinline__ uint32_t matches_B(const TileSmem& s, uint32_t b, uint32_t want) {
+  const uint32_t bB = b >> 3, n = countB(s, bB), w19 = want | ((b & 7u) << 16);
+  uint32_t k = 0u;
+  for (uint32_t i = 0; i < n; ++i) k += (s.tagsB[bB * 4u + i] & 0x7FFFFu) == w19 ? 1u : 0u;
+  return k;
 }
 
 // the live pixel with hash h, or NONE
 __device__ __forceinline__ uint32_t lookup(const TileSmem& s, uint32_t h) {
-  const uint32_t b = h >> 15, want = (h & 0x7FFFu) | 0x8000u, ww = want * 0x00010001u;
+  const uint32_t b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
   const uint2 x = s.tagsA[b];
   const uint32_t z0 = zero_half(x.x, ww), z1 = zero_half(x.y, ww);
   const bool hit = (z0 | z1) != 0u;
@@ -90,7 +106,7 @@ __device__ __forceinline__ uint32_t lookup(const TileSmem& s, uint32_t h) {
 // pixel is made to name the owner, so a lookup may take any of them.  Returns true when p is not the owner.
 __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want, uint32_t p, uint32_t k_own) {
   const uint16_t* tA = reinterpret_cast<const uint16_t*>(s.tagsA) + b * 4u;
-  const uint32_t bB = b >> 2, nB = tA[3] ? countB(s, bB) : 0u, w18 = want | ((b & 3u) << 16);
+  const uint32_t bB = b >> 3, nB = tA[3] ? countB(s, bB) : 0u, w19 = want | ((b & 7u) << 16);
   uint32_t best = 0xFFFFFFFFu;  // word << 1 | below
   for (uint32_t i = 0; i < 4u; ++i) {
     if (tA[i] != want) continue;
@@ -99,13 +115,13 @@ __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want,
   }
   for (uint32_t i = 0; i < nB; ++i) {
     const uint32_t e = s.tagsB[bB * 4u + i];
-    if ((e & 0x3FFFFu) != w18) continue;
-    const uint32_t v = (((e >> 18) & 0x3FFu) << 1) | (e >> 28);
+    if ((e & 0x7FFFFu) != w19) continue;
+    const uint32_t v = (((e >> 19) & 0x3FFu) << 1) | (e >> 29);
     best = v < best ? v : best;
   }
   if ((best >> 1) == p) return false;
   if (k_own < 4u) s.idsA[b * 4u + k_own] = (uint16_t)((best >> 1) | ((best & 1u) << 15));
-  else s.tagsB[bB * 4u + k_own - 4u] = w18 | ((best >> 1) << 18) | ((best & 1u) << 28);
+  else s.tagsB[bB * 4u + k_own - 4u] = w19 | ((best >> 1) << 19) | ((best & 1u) << 29);
   return true;
 }
 
@@ -127,22 +143,24 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
     const uint4 item = c.items[it];
     const uint32_t g0 = item.x, len = item.y & 0xFFFFu, iflags = item.y >> 16, er = item.z & 0xFFFFu, fed0 = item.z >> 16;
+    const bool cluster_it = !(iflags & ITEM_DECODE_ONLY);
     uint32_t w[NJ];
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j;
       w[j] = p < len ? __ldg(c.words + g0 + p) : 0u;
     }
+    // the item's stretch of the temp record area, one slot per word: asked for now, needed in P4
+    uint32_t wbase_t0 = 0u;
+    if (tid == 0 && cluster_it) wbase_t0 = alloc_temp(c, len);
     __syncthreads();  // the previous item is done with the shared tables
     // ================================================================== P0: clear; start bits of the item
     {
       const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
       uint4* tA = reinterpret_cast<uint4*>(s.tagsA);
-      tA[tid] = z4; tA[tid + NT] = z4;
-      uint4* sm = reinterpret_cast<uint4*>(s.qn);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) sm[tid + NT * k] = z4;
-      if (tid < NBK / 16 + NBK / 64) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
+      for (int k = 0; k < 4; ++k) tA[tid + NT * k] = z4;
+      if (tid < NBK / 16 + 16) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
       if (tid < 128) reinterpret_cast<uint32_t*>(s.run_big)[tid] = 0u;  // run_big and run_bad
       if (warp == 0) {
         const uint32_t rel = g0 - T0, wq = rel >> 5;
@@ -163,8 +181,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     __syncthreads();
     // ================================================================== P1: decode, calibrate, insert
     const uint32_t ebase = segB[er * F];
-    const bool one_seg = g0 + len <= segB[er * F + fed0 + 1u];
-    const bool cluster_it = !(iflags & ITEM_DECODE_ONLY);
+    const uint32_t nextB = segB[er * F + fed0 + 1u];        // first word of the next FED
+    const bool one_seg = g0 + len <= nextB;
     uint32_t key[NJ], chg[NJ];
     uint32_t fl = 0u;    // per word j: bit j below threshold, bit 4 + j duplicate
     uint32_t kpack = 0u; // per word j: its slot in the bucket (4 bits)
@@ -174,8 +192,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t p = tid + NT * j, g = g0 + p;
       const bool valid = p < len;
       uint32_t fed = fed0;
-      if (!one_seg && valid) {  // a FED boundary inside the item
-        uint32_t sg = er * F + fed0;
+      if (!one_seg && valid && g >= nextB) {  // a FED boundary inside the item
+        uint32_t sg = er * F + fed0 + 1u;
         while (sg + 1u < (er + 1u) * F && segB[sg + 1u] <= g) ++sg;
         fed = sg - er * F;
       }
@@ -201,15 +219,16 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         if ((bw >> lane) & 1u) { s.run_pos[r] = (uint16_t)p; s.run_mod[r] = (uint16_t)m; }
         if (below) fl |= 1u << j;
         if (cluster_it) {
-          const uint32_t h = (key[j] * HMUL) & HMASK, b = h >> 15, sh8 = (b & 3u) * 8u;
+          const uint32_t h = hash_of(key[j]), b = bucket_of(h), sh8 = (b & 3u) * 8u;
           const uint32_t k = (atomicAdd(&s.cnt[b >> 2], 1u << sh8) >> sh8) & 0xFFu;
-          const uint16_t tag = (uint16_t)((h & 0x7FFFu) | 0x8000u), idv = (uint16_t)(p | (below ? 0x8000u : 0u));
+          const uint32_t tag = want_of(h);
+          const uint16_t idv = (uint16_t)(p | (below ? 0x8000u : 0u));
           uint32_t kk = k;
-          if (k < 4u) { tagA16[b * 4u + k] = tag; s.idsA[b * 4u + k] = idv; }
+          if (k < 4u) { tagA16[b * 4u + k] = (uint16_t)tag; s.idsA[b * 4u + k] = idv; }
           else {  // rare: the bucket's first level is full
-            const uint32_t bB = b >> 2, shB = (bB & 3u) * 8u;
+            const uint32_t bB = b >> 3, shB = (bB & 3u) * 8u;
             const uint32_t kb = (atomicAdd(&s.cntB[bB >> 2], 1u << shB) >> shB) & 0xFFu;
-            if (kb < 4u) s.tagsB[bB * 4u + kb] = tag | ((b & 3u) << 16) | (p << 18) | (below ? 1u << 28 : 0u);
+            if (kb < 4u) s.tagsB[bB * 4u + kb] = tag | ((b & 7u) << 16) | (p << 19) | (below ? 1u << 29 : 0u);
             else fail = true;
             kk = 4u + (kb < 4u ? kb : 0u);
           }
@@ -222,88 +241,114 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       if ((iflags & ITEM_LONG_HEAD) && tid == 0 && key[0] != NOKEY) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[0]);
       continue;
     }
+    if (tid == 0) s.wbase = wbase_t0;
     const uint32_t R = s.n_runs;
     if (__syncthreads_or(fail)) {  // a bucket with more than 8 keys: the block-per-run kernel takes the runs of the item
       if (tid < R) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[tid]);
       continue;
     }
-    // ================================================================== P2: duplicates; neighbours -> unions
-    {
-      uint32_t cand = 0u;  // bit j: the pixel of word j may sit in its bucket more than once
-#pragma unroll
-      for (int j = 0; j < NJ; ++j) {
-        const uint32_t h = (key[j] * HMUL) & HMASK, b = h >> 15, ww = ((h & 0x7FFFu) | 0x8000u) * 0x00010001u;
-        const uint2 x = s.tagsA[b];
-        const bool cj = key[j] != NOKEY && (__popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww)) >= 2 || (x.y >> 31));
-        cand |= cj ? 1u << j : 0u;
-      }
-      if (__syncthreads_or(cand != 0u)) {
-        if (cand) {
-#pragma unroll 1
-          for (int j = 0; j < NJ; ++j) {
-            if (!((cand >> j) & 1u)) continue;
-            const uint32_t p = tid + NT * j;
-            const uint32_t h = (key[j] * HMUL) & HMASK, b = h >> 15;
-            if (resolve_dup(s, b, (h & 0x7FFFu) | 0x8000u, p, (kpack >> (4 * j)) & 15u)) { fl |= 16u << j; s.label[p] = MARK; }
-          }
-        }
-        __syncthreads();
-      }
-    }
+    // ================================================================== P2: neighbours -> edges -> unions; duplicates
     if (tid < R) {
       const uint32_t e1 = tid + 1u < R ? s.run_pos[tid + 1u] : len;
       s.run_big[tid] = (e1 - s.run_pos[tid] >= BIG_RUN) ? 1 : 0;
     }
     __syncwarp();
-    {
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
       // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1); col 416..511 and row 160..255
       // never occur, so no bounds checks.  When S is live, SW and SE are joined to it by their own E edges; when E is
       // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the
       // edges go to the warp's list, and the list is united with all lanes busy.
       uint32_t* const el = s.edge[warp];
-      uint32_t ne = 0u;
+      uint32_t cand = 0u;  // bit j: the pixel of word j sits in its bucket more than once (S10)
 #pragma unroll
-      for (int j = 0; j < NJ; ++j) {
-        const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
-        const uint32_t p = tid + NT * j;
-        const uint32_t h = (key[j] * HMUL) & HMASK;
-        const uint32_t nE = lookup(s, (h + D_E) & HMASK), nS = lookup(s, (h + D_S) & HMASK);
-        const uint32_t nSW = lookup(s, (h + D_SW) & HMASK), nSE = lookup(s, (h + D_SE) & HMASK);
-        const uint32_t t1 = nS != NONE ? nS : nSW;
-        const bool f0 = live && nE != NONE, f1 = live && t1 != NONE, f2 = live && nS == NONE && nE == NONE && nSE != NONE;
-        const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
-        if (f0) el[ne + __popc(m0 & lt_mask)] = p | (nE << 16);
-        ne += __popc(m0);
-        if (f1) el[ne + __popc(m1 & lt_mask)] = p | (t1 << 16);
-        ne += __popc(m1);
-        if (f2) el[ne + __popc(m2 & lt_mask)] = p | (nSE << 16);
-        ne += __popc(m2);
-      }
-      __syncwarp();
-      for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
-        if (i0 + lane < ne) {
-          const uint32_t e = el[i0 + lane];
-          hook(s.label, e & 0xFFFFu, e >> 16);
+      for (int half = 0; half < 2; ++half) {
+        uint32_t ne = 0u;
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) {
+          const int j = 2 * half + jj;
+          const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
+          const uint32_t p = tid + NT * j;
+          const uint32_t h = hash_of(key[j]);
+          if (pass == 0) {  // the word's own bucket: more than one entry with its tag
+            const uint32_t b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
+            const uint2 x = s.tagsA[b];
+            uint32_t nm = __popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww));
+            if ((x.y >> 31) && key[j] != NOKEY) nm += matches_B(s, b, want);  // rare: the first level is full
+            cand |= (nm >= 2u && key[j] != NOKEY) ? 1u << j : 0u;
+          }
+          const uint32_t nE = lookup(s, h + D_E), nS = lookup(s, h + D_S), nSW = lookup(s, h + D_SW), nSE = lookup(s, h + D_SE);
+          const uint32_t t1 = nS != NONE ? nS : nSW;
+          const bool f0 = live && nE != NONE, f1 = live && t1 != NONE, f2 = live && nS == NONE && nE == NONE && nSE != NONE;
+          const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
+          if (f0) el[ne + __popc(m0 & lt_mask)] = p | (nE << 16);
+          ne += __popc(m0);
+          if (f1) el[ne + __popc(m1 & lt_mask)] = p | (t1 << 16);
+          ne += __popc(m1);
+          if (f2) el[ne + __popc(m2 & lt_mask)] = p | (nSE << 16);
+          ne += __popc(m2);
         }
         __syncwarp();
+        for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
+          if (i0 + lane < ne) {
+            const uint32_t e = el[i0 + lane];
+            hook(s.label, e & 0xFFFFu, e >> 16);
+          }
+          __syncwarp();
+        }
       }
+      if (!__syncthreads_or(pass == 0 && cand != 0u)) break;
+      // rare: some pixel appears twice.  Name the owner in every entry of the pixel, mark the other words DUPLICATE,
+      // start the labels again and look up once more.
+      if (cand) {
+#pragma unroll 1
+        for (int j = 0; j < NJ; ++j) {
+          if (!((cand >> j) & 1u)) continue;
+          const uint32_t h = hash_of(key[j]);
+          if (resolve_dup(s, bucket_of(h), want_of(h), tid + NT * j, (kpack >> (4 * j)) & 15u)) fl |= 16u << j;
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) s.label[tid + NT * j] = (key[j] != NOKEY && !((fl >> j) & 0x11u)) ? tid + NT * j : MARK;
+      __syncthreads();
     }
-    __syncthreads();
     // ================================================================== P3: roots; sums
+    // One pointer-jumping step first (a label only ever moves to an ancestor, so concurrent walkers stay correct).
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j;
+      const uint32_t l = s.label[p];
+      if (l < TILE_WORDS) { const uint32_t ll = s.label[l]; if (ll != l) s.label[p] = ll; }
+    }
+    __syncwarp();
     uint32_t root[NJ];
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
-      root[j] = NONE;
-      if (key[j] == NOKEY || ((fl >> j) & 0x11u)) continue;
       const uint32_t p = tid + NT * j;
-      uint32_t r = s.label[p];
-      while (true) { const uint32_t n = s.label[r]; if (n == r) break; r = n; }
-      root[j] = r;
-      const uint32_t big = s.run_big[key[j] >> 17];
-      atomicAdd(&s.qn[r], big ? chg[j] : (chg[j] | (1u << 24)));  // below BIG_RUN words a cluster has at most 255 pixels and Q < 2^24
-      atomicAdd(&s.sx[r], chg[j] * (key[j] & 511u));
-      atomicAdd(&s.sy[r], chg[j] * ((key[j] >> 9) & 255u));
-      if (big) atomicAdd(&s.npx[r], 1u);
+      const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
+      uint32_t r = live ? s.label[p] : 0u;
+      bool done = !live;
+      while (!done) { const uint32_t n = s.label[r]; done = n == r; r = n; }  // single exit: the warp reconverges
+      root[j] = live ? r : NONE;
+      if (live && r == p) {  // a root starts its accumulators with its own pixel (the hash is dead: nobody looks up any more)
+        const uint32_t big = s.run_big[key[j] >> 17];
+        s.sum.qn[p] = big ? chg[j] : (chg[j] | (1u << 24));  // below BIG_RUN words a cluster has at most 255 pixels and Q < 2^24
+        s.sum.sx[p] = chg[j] * (key[j] & 511u);
+        s.sum.sy[p] = chg[j] * ((key[j] >> 9) & 255u);
+        s.sum.npx[p] = 1u;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j, r = root[j];
+      if (r != NONE && r != p) {
+        const uint32_t big = s.run_big[key[j] >> 17];
+        atomicAdd(&s.sum.qn[r], big ? chg[j] : (chg[j] | (1u << 24)));
+        atomicAdd(&s.sum.sx[r], chg[j] * (key[j] & 511u));
+        atomicAdd(&s.sum.sy[r], chg[j] * ((key[j] >> 9) & 255u));
+        if (big) atomicAdd(&s.sum.npx[r], 1u);
+      }
     }
     __syncthreads();
     // ================================================================== P4: cut, renumber, temp records
@@ -314,7 +359,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       bool sv = false;
       if (root[j] == p) {
         const uint32_t run = key[j] >> 17;
-        const uint32_t a = s.qn[p], Q = s.run_big[run] ? a : (a & 0xFFFFFFu);
+        const uint32_t a = s.sum.qn[p], Q = s.run_big[run] ? a : (a & 0xFFFFFFu);
         sv = (int32_t)Q >= c.cut;  // S9: equality keeps (Q < 2^31)
         if (Q > Q_SAFE) s.run_bad[run] = 1;  // 32-bit weighted sums may have wrapped
       }
@@ -323,34 +368,39 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       surv |= sv ? 1u << j : 0u;
     }
     __syncthreads();
-    if (warp == 0) {
-      const uint32_t pc = __popc(s.survb[lane]);
-      uint32_t inc = pc;
+    // every warp scans the 32 words of the survivor bitmap for itself: lane l holds word l and the survivors before it
+    const uint32_t sv_bits = s.survb[lane];
+    uint32_t sv_pre = __popc(sv_bits);
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t o = __shfl_up_sync(FULL, inc, d);
-        if (lane >= (uint32_t)d) inc += o;
-      }
-      s.spre[lane] = inc - pc;
-      if (lane == 31) { s.spre[32] = inc; s.survb[32] = 0u; s.wbase = alloc_temp(c, inc); }
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(FULL, sv_pre, d);
+      if (lane >= (uint32_t)d) sv_pre += o;
     }
-    __syncthreads();
+    const uint32_t sv_total = __shfl_sync(FULL, sv_pre, 31);
+    sv_pre -= __popc(sv_bits);
+    auto rank_before = [&](uint32_t pos) {  // survivors among the words before pos (all lanes call it together)
+      const uint32_t wi = pos >> 5;
+      const uint32_t r = __shfl_sync(FULL, sv_pre, wi) + __popc(__shfl_sync(FULL, sv_bits, wi) & ((1u << (pos & 31u)) - 1u));
+      return pos >= TILE_WORDS ? sv_total : r;
+    };
     const uint32_t wbase = s.wbase;
-    auto rank_before = [&](uint32_t pos) { return s.spre[pos >> 5] + __popc(s.survb[pos >> 5] & ((1u << (pos & 31u)) - 1u)); };
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j;
-      if (root[j] != p) continue;
-      uint32_t id = NO_ID;
-      if ((surv >> j) & 1u) {
-        const uint32_t run = key[j] >> 17, big = s.run_big[run];
-        const uint32_t a = s.qn[p], Q = big ? a : (a & 0xFFFFFFu), np = big ? s.npx[p] : (a >> 24);
-        const uint32_t rank = rank_before(p);
-        id = rank - rank_before(s.run_pos[run]);
-        const float fq = (float)Q;  // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
-        put_temp(c, wbase + rank, g0 + p - ebase, np, Q, __fdividef((float)s.sx[p], fq), __fdividef((float)s.sy[p], fq));
+      const bool is_root = root[j] == p;
+      const uint32_t run = is_root ? key[j] >> 17 : 0u;
+      const uint32_t rank = rank_before(p), base = rank_before(is_root ? (uint32_t)s.run_pos[run] : 0u);
+      if (is_root) {
+        uint32_t id = NO_ID;
+        if ((surv >> j) & 1u) {
+          const uint32_t big = s.run_big[run];
+          const uint32_t a = s.sum.qn[p], Q = big ? a : (a & 0xFFFFFFu), np = big ? s.sum.npx[p] : (a >> 24);
+          id = rank - base;
+          const float fq = (float)Q;  // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
+          put_temp(c, wbase + rank, g0 + p - ebase, np, Q, __fdividef((float)s.sum.sx[p], fq), __fdividef((float)s.sum.sy[p], fq));
+        }
+        lid[p] = (uint16_t)id;
       }
-      lid[p] = (uint16_t)id;
     }
     __syncthreads();
     // ================================================================== P5: final status and clus, run outputs, counters
@@ -370,14 +420,18 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       }
       c.d_status[g] = (uint8_t)so; c.d_clus[g] = cl;
     }
-    if (tid < R) {
-      const uint32_t m = s.run_mod[tid];
-      if (s.run_bad[tid]) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, m);
-      else {
-        const uint32_t p0 = s.run_pos[tid], p1 = tid + 1u < R ? s.run_pos[tid + 1u] : len;
-        const uint32_t b0 = rank_before(p0);
-        const size_t mo = (size_t)er * c.M + m;
-        c.n_clus[mo] = rank_before(p1) - b0; c.t_base[mo] = wbase + b0;
+    __syncwarp();
+    if (warp * 32u < R) {  // the warps that hold a run each in some lane
+      const bool has = tid < R;
+      const uint32_t p0 = has ? (uint32_t)s.run_pos[tid] : 0u, p1 = (has && tid + 1u < R) ? (uint32_t)s.run_pos[tid + 1u] : len;
+      const uint32_t b0 = rank_before(p0), b1 = rank_before(p1);  // all lanes shuffle together
+      if (has) {
+        const uint32_t m = s.run_mod[tid];
+        if (s.run_bad[tid]) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, m);
+        else {
+          const size_t mo = (size_t)er * c.M + m;
+          c.n_clus[mo] = b1 - b0; c.t_base[mo] = wbase + b0;
+        }
       }
     }
     {
