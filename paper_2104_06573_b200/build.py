@@ -16,7 +16,7 @@ SOURCES = ("decode.cu", "runs.cu", "tile.cu", "cluster.cu", "finalize.cu", "rech
 HEADERS = (os.path.join(CSRC, "pix_common.cuh"), os.path.join(CSRC, "pix_device.cuh"), os.path.join(HERE, "..", "include", "pixclus.h"))
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-         "-Xptxas", "-v"]
+         "-Xptxas", "-v"] + os.environ.get("PIXCLUS_NVCC_FLAGS", "").split()  # extra flags, e.g. -DTILE_NT=256 (tuning experiments)
 
 
 def _stale(target: str, deps) -> bool:

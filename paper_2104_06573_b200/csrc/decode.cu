@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk
   for (uint32_t t = tid; t < nmod; t += nth) { mf[t] = NO_INDEX; me[t] = 0u; c.n_clus[t] = 0u; c.n_runs[t] = 0u; }
 }
 
-// chunk_seg[ci] = segment (event, FED) of the first word of 128-word chunk ci (its first word inside the launch
+// chunk_seg[ci] = event << 16 | FED of the first word of 128-word chunk ci (its first word inside the launch
 // group).  One thread per segment writes the chunks that start inside it.  One warp per event closes the event's
 // last run: module_end of the module of the event's last decodable word (the fused kernel closes a run when it
 // sees the next run start of the same event, and never looks back beyond the start of an event).
@@ -69,7 +69,8 @@ __global__ void __launch_bounds__(256) segfill_kernel(const __grid_constant__ Ch
     if (lo >= hi) continue;
     const uint32_t c_lo = lo == gBeg ? 0u : (lo - T0 + CHUNK_WORDS - 1u) / CHUNK_WORDS;
     const uint32_t c_hi = (hi - T0 + CHUNK_WORDS - 1u) / CHUNK_WORDS;  // exclusive
-    for (uint32_t ci = c_lo; ci < c_hi; ++ci) c.chunk_seg[ci] = sgi;
+    const uint32_t er = div_F(c, sgi), packed = (er << 16) | (sgi - er * F);  // F, Ec <= 65535 (pix_create)
+    for (uint32_t ci = c_lo; ci < c_hi; ++ci) c.chunk_seg[ci] = packed;
   }
   const uint32_t lane = threadIdx.x & 31u;
   for (uint32_t er = tid >> 5; er < Ec; er += nth >> 5) {

@@ -40,7 +40,10 @@ enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS
 enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_TEMP_COUNT = 8, CTL_ITEM_COUNT = 9, CTL_WORDS = 16 };
 // work items of the tile kernel (runs.cu packs them, tile.cu takes them): x = global index of the first word,
 // y = words | flags << 16, z = event (launch-group relative) | FED of the first word << 16
-constexpr uint32_t TILE_WORDS = 1024, ITEM_WIN = 992, ITEM_WIN2 = 224, ITEM_RUNS = 255;
+#ifndef PIX_TILE_WORDS
+#define PIX_TILE_WORDS 1024
+#endif
+constexpr uint32_t TILE_WORDS = PIX_TILE_WORDS, ITEM_WIN = TILE_WORDS - 32, ITEM_WIN2 = 224, ITEM_RUNS = 255;
 constexpr uint32_t ITEM_DECODE_ONLY = 1u, ITEM_LONG_HEAD = 2u;
 
 // Cabling table as the kernels read it (built once in pix_create from pix_cabling_map.entry, reading S3):
@@ -82,7 +85,7 @@ struct Chunk {
   uint32_t* big_list;       // [(e1-e0)*M] runs of 513..1024 words, left by findrun<512> to findrun<1024>
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
   uint32_t list_cap;        // (e1-e0)*M: every event lists at most M runs (push_run)
-  uint32_t* chunk_seg;      // [cap_words/128 + 2] segment (event_rel*F + fed) of the chunk's first word
+  uint32_t* chunk_seg;      // [cap_words/128 + 2] event_rel << 16 | fed of the chunk's first word
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* sbits;          // [cap_words/32 + 16] run-start bits, bit (g - T0) (runs.cu)
   uint4* items;             // [item_cap] work items of the tile kernel

@@ -23,6 +23,14 @@ namespace pix {
 namespace {
 
 constexpr uint32_t HC = CHUNK_WORDS, FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
+constexpr uint32_t RANGE = 8;  // chunks a warp walks in one go (the look-back is done once per range)
+
+// (event, module) of a decodable word, NOKEY otherwise (S4-S6: the same checks as decode_word, without the position)
+__device__ __forceinline__ uint32_t run_key(const CabEntry* __restrict__ cab, uint32_t w, uint32_t fedbase, uint32_t er) {
+  const uint32_t ex = __ldg(reinterpret_cast<const uint32_t*>(cab + fedbase + (w >> 21)));  // .x: module | bad << 16 | ...
+  const bool ok = !(ex & 0xFF0000u) && ((w >> 16) & 31u) < 26u && ((w >> 8) & 255u) < 160u && w != 0u;
+  return ok ? ((er << 16) | (ex & 0xFFFFu)) : NOKEY;
+}
 
 __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk c) {
   const uint32_t lane = threadIdx.x & 31u;
@@ -34,24 +42,12 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
   const uint32_t n_chunks = (gEnd - T0 + HC - 1u) / HC;
   const uint32_t lt_mask = (1u << lane) - 1u;
   const uint32_t nwarp = (gridDim.x * blockDim.x) >> 5;
-  for (uint32_t ci = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; ci < n_chunks; ci += nwarp) {
-    const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
-    const uint32_t sg0 = c.chunk_seg[ci];
-    const uint32_t er0 = div_F(c, sg0), fed0 = sg0 - er0 * F;
-    const uint32_t nextB0 = segB[sg0 + 1u];
-    const bool all_in = b >= gBeg && b + HC <= gEnd;
-    const bool one_seg = all_in && b + HC <= nextB0;
-    uint4 wv = make_uint4(0u, 0u, 0u, 0u);
-    if (all_in) wv = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
-    else {
-      if (g0 >= gBeg && g0 < gEnd) wv.x = __ldg(c.words + g0);
-      if (g0 + 1u >= gBeg && g0 + 1u < gEnd) wv.y = __ldg(c.words + g0 + 1u);
-      if (g0 + 2u >= gBeg && g0 + 2u < gEnd) wv.z = __ldg(c.words + g0 + 2u);
-      if (g0 + 3u >= gBeg && g0 + 3u < gEnd) wv.w = __ldg(c.words + g0 + 3u);
-    }
-    // ---- the last decodable word before the chunk, inside the event of the chunk's first word
+  for (uint32_t c0 = ((blockIdx.x * blockDim.x + threadIdx.x) >> 5) * RANGE; c0 < n_chunks; c0 += nwarp * RANGE) {
+    const uint32_t c1 = c0 + RANGE < n_chunks ? c0 + RANGE : n_chunks;
+    // ---- the last decodable word before the range, inside the event of the range's first word
     uint32_t carry_key = NOKEY, carry_g = 0u;
     {
+      const uint32_t b = T0 + c0 * HC, cs = c.chunk_seg[c0], er0 = cs >> 16, sg0 = er0 * F + (cs & 0xFFFFu);
       const uint32_t gw = b < gBeg ? gBeg : b, evb = segB[er0 * F];
       uint32_t g = gw;  // words [evb, g) are still to be searched, backwards
       while (g > evb) {
@@ -61,8 +57,7 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
         if (in) {
           uint32_t sg = sg0;
           while (segB[sg] > gi) --sg;
-          uint32_t m, r, cc;
-          if (decode_word(c.cab, __ldg(c.words + gi), (sg - er0 * F) << 11, m, r, cc) == ST_OK) key = (er0 << 16) | m;
+          key = run_key(c.cab, __ldg(c.words + gi), (sg - er0 * F) << 11, er0);
         }
         const uint32_t bal = __ballot_sync(FULL, key != NOKEY);
         if (bal) {
@@ -74,58 +69,123 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
         g = (g - evb > 32u) ? g - 32u : evb;
       }
     }
-    const uint32_t w[4] = {wv.x, wv.y, wv.z, wv.w};
-    uint32_t key[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const uint32_t g = g0 + j;
-      const bool exists = all_in || (g >= gBeg && g < gEnd);
-      uint32_t er = er0, fed = fed0;
-      if (!one_seg && exists) {  // rare: a FED / event boundary inside the chunk
-        uint32_t sg = sg0;
-        while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
-        er = div_F(c, sg); fed = sg - er * F;
+    for (uint32_t ci = c0; ci < c1; ++ci) {
+      const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
+      const uint32_t cs = c.chunk_seg[ci];
+      const uint32_t er0 = cs >> 16, fed0 = cs & 0xFFFFu, sg0 = er0 * F + fed0;
+      const bool all_in = b >= gBeg && b + HC <= gEnd;
+      const bool one_seg = all_in && b + HC <= segB[sg0 + 1u];
+      uint4 wv = make_uint4(0u, 0u, 0u, 0u);
+      if (all_in) wv = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
+      else {
+        if (g0 >= gBeg && g0 < gEnd) wv.x = __ldg(c.words + g0);
+        if (g0 + 1u >= gBeg && g0 + 1u < gEnd) wv.y = __ldg(c.words + g0 + 1u);
+        if (g0 + 2u >= gBeg && g0 + 2u < gEnd) wv.z = __ldg(c.words + g0 + 2u);
+        if (g0 + 3u >= gBeg && g0 + 3u < gEnd) wv.w = __ldg(c.words + g0 + 3u);
       }
-      uint32_t m, r, cc;
-      const uint32_t st = decode_word(c.cab, w[j], fed << 11, m, r, cc);
-      key[j] = (exists && st == ST_OK) ? ((er << 16) | m) : NOKEY;
-    }
-    // a word starts a run when its (event, module) differs from the previous decodable word's
-    uint32_t tkey = NOKEY, tj = 0u;  // the lane's last decodable word
+      const uint32_t w[4] = {wv.x, wv.y, wv.z, wv.w};
+      uint32_t key[4];
+      if (one_seg) {
 #pragma unroll
-    for (int j = 0; j < 4; ++j) if (key[j] != NOKEY) { tkey = key[j]; tj = j; }
-    const uint32_t has = __ballot_sync(FULL, tkey != NOKEY);
-    const uint32_t below_l = has & lt_mask;
-    const int src = below_l ? 31 - __clz(below_l) : 0;
-    uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = b + 4u * (uint32_t)src + __shfl_sync(FULL, tj, src);
-    if (!below_l) { pkey = carry_key; pg = carry_g; }
-    uint32_t startmask = 0u;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      if (key[j] == NOKEY) continue;
-      if (key[j] != pkey) {
-        startmask |= 1u << j;
-        run_start(c, key[j], g0 + j);
-        if (pkey != NOKEY) run_end(c, pkey, pg);
+        for (int j = 0; j < 4; ++j) key[j] = run_key(c.cab, w[j], fed0 << 11, er0);
+      } else {  // a FED / event boundary inside the chunk, or a chunk at the edge of the launch group
+#pragma unroll 1
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t g = g0 + j;
+          uint32_t k = NOKEY;
+          if (g >= gBeg && g < gEnd) {
+            uint32_t sg = sg0;
+            while (sg + 1u < S && segB[sg + 1u] <= g) ++sg;
+            const uint32_t er = div_F(c, sg);
+            k = run_key(c.cab, w[j], (sg - er * F) << 11, er);
+          }
+          key[0] = key[1]; key[1] = key[2]; key[2] = key[3]; key[3] = k;  // after four turns key[j] is word j's
+        }
       }
-      pkey = key[j]; pg = g0 + j;
-    }
-    // start bits of the chunk: lane l's nibble sits at bit 4 l of the 128-bit row
-    const uint32_t nib = startmask << (4u * (lane & 7u));
+      // a word starts a run when its (event, module) differs from the previous decodable word's
+      uint32_t tkey = NOKEY, tj = 0u;  // the lane's last decodable word
 #pragma unroll
-    for (uint32_t k = 0; k < 4u; ++k) {
-      const uint32_t v = __reduce_or_sync(FULL, (lane >> 3) == k ? nib : 0u);
-      if (lane == k) c.sbits[ci * 4u + k] = v;
+      for (int j = 0; j < 4; ++j) if (key[j] != NOKEY) { tkey = key[j]; tj = j; }
+      const uint32_t has = __ballot_sync(FULL, tkey != NOKEY);
+      const uint32_t below_l = has & lt_mask;
+      const int src = below_l ? 31 - __clz(below_l) : 0;
+      uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = b + 4u * (uint32_t)src + __shfl_sync(FULL, tj, src);
+      if (!below_l) { pkey = carry_key; pg = carry_g; }
+      uint32_t startmask = 0u;
+      uint32_t s_key = NOKEY, s_g = 0u, s_pkey = NOKEY, s_pg = 0u;  // the lane's first run start and its predecessor
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        if (key[j] == NOKEY) continue;
+        if (key[j] != pkey) {
+          if (!startmask) { s_key = key[j]; s_g = g0 + j; s_pkey = pkey; s_pg = pg; }
+          startmask |= 1u << j;
+        }
+        pkey = key[j]; pg = g0 + j;
+      }
+      if (s_key != NOKEY) {  // one copy of the atomics for the usual case of at most one start per lane
+        run_start(c, s_key, s_g);
+        if (s_pkey != NOKEY) run_end(c, s_pkey, s_pg);
+      }
+      if (startmask & (startmask - 1u)) {  // rare: several runs start inside the lane's four words
+        uint32_t pk = NOKEY, pgg = 0u;
+        bool first = true;
+#pragma unroll 1
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t kj = key[0];
+          key[0] = key[1]; key[1] = key[2]; key[2] = key[3]; key[3] = kj;  // rotate: kj is word j's key
+          if (kj == NOKEY) continue;
+          if ((startmask >> j) & 1u) {
+            if (!first) { run_start(c, kj, g0 + j); run_end(c, pk, pgg); }
+            first = false;
+          }
+          pk = kj; pgg = g0 + j;
+        }
+      }
+      if (has) {
+        const int top = 31 - __clz(has);
+        carry_key = __shfl_sync(FULL, tkey, top); carry_g = b + 4u * (uint32_t)top + __shfl_sync(FULL, tj, top);
+      }
+      // start bits of the chunk: lane l's nibble sits at bit 4 l of the 128-bit row
+      const uint32_t nib = startmask << (4u * (lane & 7u));
+#pragma unroll
+      for (uint32_t k = 0; k < 4u; ++k) {
+        const uint32_t v = __reduce_or_sync(FULL, (lane >> 3) == k ? nib : 0u);
+        if (lane == k) c.sbits[ci * 4u + k] = v;
+      }
     }
   }
 }
 
+// ---- pack_kernel: one warp per event.  The event's start bits are staged in shared memory, BUFW words at a time.
+constexpr uint32_t BUFW = 288, NEED = 34;  // a step looks at the words [s >> 5, (s >> 5) + NEED)
+constexpr int PACK_WARPS = 4;
+
+struct PackWarp {
+  uint32_t buf[BUFW];
+  uint4 items[32];
+};
+
+struct Stage {  // a warp's window on the start bits
+  const uint32_t* __restrict__ sbits;
+  uint32_t* buf;
+  uint32_t w0, w_end;  // first staged word; one past the last word of the launch group's bits that may be read
+  uint32_t lane;
+  __device__ __forceinline__ void ensure(uint32_t w_lo) {  // words [w_lo, w_lo + NEED) readable
+    if (w_lo >= w0 && w_lo + NEED <= w0 + BUFW) return;
+    __syncwarp();
+    w0 = w_lo;
+    for (uint32_t i = lane; i < BUFW; i += 32u) buf[i] = (w0 + i < w_end) ? sbits[w0 + i] : 0u;
+    __syncwarp();
+  }
+  __device__ __forceinline__ uint32_t rd(uint32_t wi) const { return buf[wi - w0]; }
+};
+
 // highest start bit in (lo, hi] (bit indices relative to T0; hi - lo <= 992 so the range spans at most 32 words), or NO_INDEX
-__device__ __forceinline__ uint32_t last_start(const uint32_t* __restrict__ sbits, uint32_t lo, uint32_t hi, uint32_t lane) {
-  const int w_hi = (int)(hi >> 5), w_lo = (int)(lo >> 5), wi = w_hi - (int)lane;
+__device__ __forceinline__ uint32_t last_start(const Stage& st, uint32_t lo, uint32_t hi) {
+  const int w_hi = (int)(hi >> 5), w_lo = (int)(lo >> 5), wi = w_hi - (int)st.lane;
   uint32_t v = 0u;
   if (wi >= w_lo) {
-    v = sbits[wi];
+    v = st.rd((uint32_t)wi);
     if (wi == w_hi) v &= (2u << (hi & 31u)) - 1u;
     if (wi == w_lo) v &= ~((2u << (lo & 31u)) - 1u);
   }
@@ -136,11 +196,11 @@ __device__ __forceinline__ uint32_t last_start(const uint32_t* __restrict__ sbit
   return (uint32_t)(w_hi - src) * 32u + 31u - (uint32_t)__clz(vv);
 }
 // lowest start bit in (lo, hi], same limits
-__device__ __forceinline__ uint32_t first_start(const uint32_t* __restrict__ sbits, uint32_t lo, uint32_t hi, uint32_t lane) {
-  const int w_hi = (int)(hi >> 5), w_lo = (int)(lo >> 5), wi = w_lo + (int)lane;
+__device__ __forceinline__ uint32_t first_start(const Stage& st, uint32_t lo, uint32_t hi) {
+  const int w_hi = (int)(hi >> 5), w_lo = (int)(lo >> 5), wi = w_lo + (int)st.lane;
   uint32_t v = 0u;
   if (wi <= w_hi) {
-    v = sbits[wi];
+    v = st.rd((uint32_t)wi);
     if (wi == w_hi) v &= (2u << (hi & 31u)) - 1u;
     if (wi == w_lo) v &= ~((2u << (lo & 31u)) - 1u);
   }
@@ -151,13 +211,13 @@ __device__ __forceinline__ uint32_t first_start(const uint32_t* __restrict__ sbi
   return (uint32_t)(w_lo + src) * 32u + (uint32_t)__ffs(vv) - 1u;
 }
 // start bits in [lo, hi), hi - lo <= 1024
-__device__ __forceinline__ uint32_t count_starts(const uint32_t* __restrict__ sbits, uint32_t lo, uint32_t hi, uint32_t lane) {
+__device__ __forceinline__ uint32_t count_starts(const Stage& st, uint32_t lo, uint32_t hi) {
   if (hi <= lo) return 0u;
   const uint32_t last = hi - 1u;
   const int w_hi = (int)(last >> 5), w_lo = (int)(lo >> 5);
   uint32_t n = 0u;
-  for (int wi = w_lo + (int)lane; wi <= w_hi; wi += 32) {
-    uint32_t v = sbits[wi];
+  for (int wi = w_lo + (int)st.lane; wi <= w_hi; wi += 32) {
+    uint32_t v = st.rd((uint32_t)wi);
     if (wi == w_hi) v &= (2u << (last & 31u)) - 1u;
     if (wi == w_lo) v &= ~((1u << (lo & 31u)) - 1u);
     n += __popc(v);
@@ -165,37 +225,48 @@ __device__ __forceinline__ uint32_t count_starts(const uint32_t* __restrict__ sb
   return __reduce_add_sync(FULL, n);
 }
 
-__global__ void __launch_bounds__(128) pack_kernel(const __grid_constant__ Chunk c) {
+__global__ void __launch_bounds__(PACK_WARPS * 32) pack_kernel(const __grid_constant__ Chunk c) {
+  __shared__ PackWarp sm[PACK_WARPS];
   const uint32_t lane = threadIdx.x & 31u;
+  PackWarp& pw = sm[threadIdx.x >> 5];
   const uint32_t F = c.F, Ec = c.e1 - c.e0, S = Ec * F;
   const uint32_t* __restrict__ segB = c.segB;
   const uint32_t gBeg = segB[0], gEnd = segB[S];
   if (gBeg >= gEnd) return;
   const uint32_t T0 = gBeg & ~(HC - 1u);
-  const uint32_t* __restrict__ sbits = c.sbits;
   const uint32_t nwarp = (gridDim.x * blockDim.x) >> 5;
+  Stage st;
+  st.sbits = c.sbits; st.buf = pw.buf; st.lane = lane; st.w_end = ((gEnd - T0 + HC - 1u) / HC) * 4u;
   for (uint32_t er = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; er < Ec; er += nwarp) {
     const uint32_t evb = segB[er * F], eve = segB[(er + 1u) * F];
     uint32_t sg = er * F;
     uint32_t s = evb;
+    uint32_t n_buf = 0u;  // items waiting in pw.items
+    st.w0 = 0xFFFFFFFFu - BUFW;  // nothing staged
+    auto flush = [&]() {
+      __syncwarp();
+      uint32_t base = 0u;
+      if (lane == 0 && n_buf) base = atomicAdd(c.ctl + CTL_ITEM_COUNT, n_buf);
+      base = __shfl_sync(FULL, base, 0);
+      if (lane < n_buf && base + lane < c.item_cap) c.items[base + lane] = pw.items[lane];
+      n_buf = 0u;
+      __syncwarp();
+    };
     auto emit = [&](uint32_t g, uint32_t len, uint32_t flags) {
       while (sg + 1u < (er + 1u) * F && segB[sg + 1u] <= g) ++sg;
-      if (lane == 0) {
-        const uint32_t i = atomicAdd(c.ctl + CTL_ITEM_COUNT, 1u);
-        if (i < c.item_cap) c.items[i] = make_uint4(g, len | (flags << 16), er | ((sg - er * F) << 16), 0u);
-      }
+      if (lane == 0) pw.items[n_buf] = make_uint4(g, len | (flags << 16), er | ((sg - er * F) << 16), 0u);
+      if (++n_buf == 32u) flush();
     };
     while (s < eve) {
       const uint32_t rs = s - T0, rlast = eve - 1u - T0;  // bit indices of the item's first word and of the event's last word
+      st.ensure(rs >> 5);
       uint32_t win = ITEM_WIN;
       uint32_t nxt;  // bit index of the next item's first word
       while (true) {
-        if (rlast - rs < win) { nxt = rlast + 1u; }  // the rest of the event fits
-        else {
-          nxt = last_start(sbits, rs, rs + win, lane);
-        }
+        if (rlast - rs < win) nxt = rlast + 1u;  // the rest of the event fits
+        else nxt = last_start(st, rs, rs + win);
         if (nxt == NO_INDEX || win == ITEM_WIN2) break;
-        if (count_starts(sbits, rs, nxt, lane) <= ITEM_RUNS) break;
+        if (count_starts(st, rs, nxt) <= ITEM_RUNS) break;
         win = ITEM_WIN2;  // too many runs: a shorter item (at most ITEM_WIN2 + 1 <= ITEM_RUNS runs)
       }
       if (nxt != NO_INDEX) {
@@ -203,37 +274,38 @@ __global__ void __launch_bounds__(128) pack_kernel(const __grid_constant__ Chunk
         s = T0 + nxt;
         continue;
       }
-      // no run starts in (s, s + ITEM_WIN]: one run (or a stretch of undecodable words) longer than that
+      // no run starts in (s, s + win]: one run (or a stretch of undecodable words) longer than that
+      const bool head = (st.rd(rs >> 5) >> (rs & 31u)) & 1u;
       uint32_t p = rs + win;
-      nxt = NO_INDEX;
       while (nxt == NO_INDEX && p < rlast) {
         const uint32_t q = (rlast - p > 992u) ? p + 992u : rlast;
-        nxt = first_start(sbits, p, q, lane);
+        st.ensure(p >> 5);
+        nxt = first_start(st, p, q);
         p = q;
       }
       if (nxt == NO_INDEX) nxt = rlast + 1u;
       const uint32_t L = nxt - rs;
       if (L <= TILE_WORDS) emit(s, L, 0u);
       else {
-        const bool head = (sbits[rs >> 5] >> (rs & 31u)) & 1u;
         const uint32_t pieces = (L + TILE_WORDS - 1u) / TILE_WORDS, plen = (L + pieces - 1u) / pieces;
         for (uint32_t k = 0, o = 0; o < L; ++k, o += plen)
           emit(s + o, (L - o < plen) ? L - o : plen, ITEM_DECODE_ONLY | ((k == 0 && head) ? ITEM_LONG_HEAD : 0u));
       }
       s = T0 + nxt;
     }
+    flush();
   }
 }
 
 }  // namespace
 
 void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
-  uint64_t nb = ((uint64_t)words_bound + 2 * HC + 8 * HC - 1) / (8 * HC);
+  uint64_t nb = ((uint64_t)words_bound + 2 * HC + 8 * RANGE * HC - 1) / (8 * RANGE * HC);  // 8 warps of RANGE chunks per block
   if (nb < 1) nb = 1;
   if (nb > (uint64_t)n_sm * 16) nb = (uint64_t)n_sm * 16;
   runs_kernel<<<(int)nb, 256, 0, stream>>>(c);
   const uint32_t Ec = c.e1 - c.e0;
-  pack_kernel<<<(int)((Ec + 3u) / 4u), 128, 0, stream>>>(c);
+  pack_kernel<<<(int)((Ec + PACK_WARPS - 1u) / PACK_WARPS), PACK_WARPS * 32, 0, stream>>>(c);
 }
 
 }  // namespace pix

@@ -19,6 +19,8 @@
 // What the kernel cannot take goes to the block-per-run kernel (cluster.cu): runs longer than 1024 words (decoded
 // here, ITEM_DECODE_ONLY), items whose hash overflows a bucket (8 keys), runs with a cluster charge beyond Q_SAFE.
 // Nothing here is shared with oracle/.
+#include <cstddef>
+
 #include "pix_common.cuh"
 #include "pix_device.cuh"
 
@@ -26,9 +28,15 @@ namespace pix {
 
 namespace {
 
-constexpr int NT = 256, NJ = 4, BLOCKS_PER_SM = 4;
+#ifndef TILE_NT
+#define TILE_NT 256
+#endif
+#ifndef TILE_BLOCKS
+#define TILE_BLOCKS 5
+#endif
+constexpr int NT = TILE_NT, NJ = TILE_WORDS / NT, BLOCKS_PER_SM = TILE_BLOCKS, NWARP = NT / 32;
 constexpr uint32_t FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
-constexpr uint32_t NBK = 2048, NBK_LOG2 = 11;        // buckets of 4 entries (load 0.5: a bucket is full for 0.2% of the lookups)
+constexpr uint32_t NBK = 2 * TILE_WORDS, NBK_LOG2 = TILE_WORDS == 1024 ? 11 : 10, TAG_BITS = 25 - NBK_LOG2, TAG_MASK = (1u << TAG_BITS) - 1u;        // buckets of 4 entries (load 0.5: a bucket is full for 0.2% of the lookups)
 // key: run (8) | row (8) | col (9) = 25 bits.  h = (key << 7) * HMUL mod 2^32: the top 25 bits are key * HMUL mod 2^25,
 // a bijection of the key; bucket = top 11 bits, tag = the next 14, so (bucket, tag) names the key exactly, and the hash
 // of a neighbour is h + a constant.
@@ -38,17 +46,19 @@ constexpr uint32_t MARK = 0xFFFFFFFDu;               // label of a word that is 
 constexpr uint32_t NONE = 0xFFFFu, NO_ID = 0xFFFFu;
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;      // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
 constexpr uint32_t BIG_RUN = 256u;                   // runs this long count their pixels in a word of their own
-constexpr uint32_t ECAP = 3 * 64;                    // edges a warp lists before it unites them (two words per lane)
+constexpr uint32_t ECAP = 3 * 32;                    // edges a warp lists before it unites them (one word per lane)
+constexpr uint32_t BB_SHIFT = 5, BB_MASK = (1u << BB_SHIFT) - 1u;  // first-level buckets per second-level bucket
+constexpr uint32_t B_KEY = (1u << (16 + BB_SHIFT)) - 1u, B_WORD = 16 + BB_SHIFT, B_BELOW = B_WORD + 10;  // fields of a second-level entry
 
 struct __align__(16) TileSmem {
   union {
-    uint2 tagsA[NBK];        // first level: 4 x (0x8000 | tag), 0 = free
+    uint2 tagsA[NBK];        // first level: 4 x (tag + 1), 0 = free
     struct { uint32_t qn[TILE_WORDS], sx[TILE_WORDS], sy[TILE_WORDS], npx[TILE_WORDS]; } sum;  // after P2: the roots' accumulators
   };
   uint16_t idsA[4 * NBK];    // word of the entry | below_threshold << 15; after P2: lid (local id of a root, or NO_ID)
-  uint32_t tagsB[1024];      // second level, 4 entries per 8 buckets: tag | (bucket & 7) << 16 | word << 19 | below << 29
+  uint32_t tagsB[4 * (NBK >> BB_SHIFT)];  // second level, 4 entries per 32 buckets: tag + 1 | (bucket & 31) << 15 | word << 20 | below << 30
   uint32_t cnt[NBK / 4];     // entries per bucket, one byte each
-  uint32_t cntB[64];         // entries per second-level bucket, one byte each (tagsB is never cleared)
+  uint32_t cntB[(NBK >> BB_SHIFT) / 4];  // entries per second-level bucket, one byte each (tagsB is never cleared)
   uint32_t edge[NT / 32][ECAP];  // per warp: the edges its words found, a | b << 16
   uint32_t label[TILE_WORDS];
   uint32_t bits[32], pre[32];        // run-start bits of the item, run starts before each word of bits
@@ -57,12 +67,12 @@ struct __align__(16) TileSmem {
   uint8_t run_big[256], run_bad[256];
   uint32_t n_runs, wbase, pad[2];
 };
-static_assert(sizeof(TileSmem) <= 57344 - 64, "four blocks per SM");
+static_assert(sizeof(TileSmem) <= 233472 / BLOCKS_PER_SM - 1024, "BLOCKS_PER_SM blocks per SM");
 static_assert(sizeof(uint2) * NBK == 4 * 4 * TILE_WORDS, "the accumulators take the place of the first-level tags");
 
 __device__ __forceinline__ uint32_t hash_of(uint32_t key) { return (key << 7) * HMUL; }
 __device__ __forceinline__ uint32_t bucket_of(uint32_t h) { return h >> (32 - NBK_LOG2); }
-__device__ __forceinline__ uint32_t want_of(uint32_t h) { return ((h >> 7) & 0x3FFFu) | 0x8000u; }
+__device__ __forceinline__ uint32_t want_of(uint32_t h) { return ((h >> 7) & TAG_MASK) + 1u; }  // 1 .. 16384: bit 15 stays free for zero_half
 __device__ __forceinline__ uint32_t zero_half(uint32_t x, uint32_t ww) {
   const uint32_t y = x ^ ww;
   return (y - 0x00010001u) & ~y & 0x80008000u;  // bit 15 / 31 set where a half of x equals the half of ww (the lower set bit is exact)
@@ -73,40 +83,53 @@ __device__ __forceinline__ uint32_t countB(const TileSmem& s, uint32_t bB) {
 }
 // second level (rare): the live pixel, or NONE
 __device__ __noinline__ uint32_t lookup_B(const TileSmem& s, uint32_t b, uint32_t want) {
-  const uint32_t bB = b >> 3, n = countB(s, bB), w19 = want | ((b & 7u) << 16);
+  const uint32_t bB = b >> BB_SHIFT, n = countB(s, bB), w19 = want | ((b & BB_MASK) << 16);
   for (uint32_t i = 0; i < n; ++i) {
     const uint32_t e = s.tagsB[bB * 4u + i];
-    if ((e & 0x7FFFFu) == w19) return (e >> 29) ? NONE : ((e >> 19) & 0x3FFu);
+    if ((e & B_KEY) == w19) return (e >> B_BELOW) ? NONE : ((e >> B_WORD) & 0x3FFu);
   }
   return NONE;
 }
 // second level (rare): entries of the pixel
 __device__ __noinline__ uint32_t matches_B(const TileSmem& s, uint32_t b, uint32_t want) {
-  const uint32_t bB = b >> 3, n = countB(s, bB), w19 = want | ((b & 7u) << 16);
+  const uint32_t bB = b >> BB_SHIFT, n = countB(s, bB), w19 = want | ((b & BB_MASK) << 16);
   uint32_t k = 0u;
-  for (uint32_t i = 0; i < n; ++i) k += (s.tagsB[bB * 4u + i] & 0x7FFFFu) == w19 ? 1u : 0u;
+  for (uint32_t i = 0; i < n; ++i) k += (s.tagsB[bB * 4u + i] & B_KEY) == w19 ? 1u : 0u;
   return k;
 }
 
-// the live pixel with hash h, or NONE
-__device__ __forceinline__ uint32_t lookup(const TileSmem& s, uint32_t h) {
-  const uint32_t b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
-  const uint2 x = s.tagsA[b];
-  const uint32_t z0 = zero_half(x.x, ww), z1 = zero_half(x.y, ww);
-  const bool hit = (z0 | z1) != 0u;
-  const uint32_t k = z0 ? ((z0 & 0x8000u) ? 0u : 1u) : ((z1 & 0x8000u) ? 2u : 3u);
-  uint32_t idv = 0x8000u;
-  if (hit) idv = s.idsA[b * 4u + k];
-  uint32_t res = (idv >> 15) ? NONE : (idv & 0x3FFu);
-  if (!hit && (x.y >> 31)) res = lookup_B(s, b, want);  // rare: the first level is full
-  return res;
+// Lookup of four pixels at once (the four loads are in flight together).  sb = shared-memory address of tagsA.  The
+// result is the word of the live pixel with hash h[i], or a value >= 0x8000 (no such pixel, or below threshold).
+__device__ __forceinline__ void lookup4(const TileSmem& s, uint32_t sb, const uint32_t (&h)[4], uint32_t (&res)[4]) {
+  uint32_t ao[4], x0[4], x1[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    ao[i] = sb + ((h[i] >> (32 - NBK_LOG2 - 3)) & ((NBK - 1u) << 3));  // address of the bucket
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x0[i]), "=r"(x1[i]) : "r"(ao[i]));
+  }
+  uint32_t k2[4];
+  bool hit[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const uint32_t ww = ((h[i] >> 7) & TAG_MASK) * 0x00010001u + 0x00010001u;  // tag + 1 in both halves
+    const uint32_t z0 = zero_half(x0[i], ww), z1 = zero_half(x1[i], ww);
+    hit[i] = (z0 | z1) != 0u;
+    k2[i] = z0 ? ((z0 & 0x8000u) ? 0u : 2u) : ((z1 & 0x8000u) ? 4u : 6u);
+    res[i] = 0xFFFFu;
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    if (hit[i]) asm volatile("ld.shared.u16 %0, [%1+%2];" : "=r"(res[i]) : "r"(ao[i] + k2[i]), "n"(sizeof(uint2) * NBK));  // idsA follows tagsA
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    if (!hit[i] && x1[i] >= 0x10000u) res[i] = lookup_B(s, bucket_of(h[i]), want_of(h[i]));  // rare: the first level is full
 }
 
 // rare: the pixel of word p appears more than once in its bucket.  The lowest word owns it (S10); every entry of the
 // pixel is made to name the owner, so a lookup may take any of them.  Returns true when p is not the owner.
 __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want, uint32_t p, uint32_t k_own) {
   const uint16_t* tA = reinterpret_cast<const uint16_t*>(s.tagsA) + b * 4u;
-  const uint32_t bB = b >> 3, nB = tA[3] ? countB(s, bB) : 0u, w19 = want | ((b & 7u) << 16);
+  const uint32_t bB = b >> BB_SHIFT, nB = tA[3] ? countB(s, bB) : 0u, w19 = want | ((b & BB_MASK) << 16);
   uint32_t best = 0xFFFFFFFFu;  // word << 1 | below
   for (uint32_t i = 0; i < 4u; ++i) {
     if (tA[i] != want) continue;
@@ -115,13 +138,13 @@ __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want,
   }
   for (uint32_t i = 0; i < nB; ++i) {
     const uint32_t e = s.tagsB[bB * 4u + i];
-    if ((e & 0x7FFFFu) != w19) continue;
-    const uint32_t v = (((e >> 19) & 0x3FFu) << 1) | (e >> 29);
+    if ((e & B_KEY) != w19) continue;
+    const uint32_t v = (((e >> B_WORD) & 0x3FFu) << 1) | (e >> B_BELOW);
     best = v < best ? v : best;
   }
   if ((best >> 1) == p) return false;
   if (k_own < 4u) s.idsA[b * 4u + k_own] = (uint16_t)((best >> 1) | ((best & 1u) << 15));
-  else s.tagsB[bB * 4u + k_own - 4u] = w19 | ((best >> 1) << 19) | ((best & 1u) << 29);
+  else s.tagsB[bB * 4u + k_own - 4u] = w19 | ((best >> 1) << B_WORD) | ((best & 1u) << B_BELOW);
   return true;
 }
 
@@ -139,6 +162,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
   const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
   uint16_t* const tagA16 = reinterpret_cast<uint16_t*>(s.tagsA);
   uint16_t* const lid = s.idsA;
+  const uint32_t sb_tags = (uint32_t)__cvta_generic_to_shared(s.tagsA);
+  static_assert(offsetof(TileSmem, idsA) == sizeof(uint2) * NBK, "idsA follows tagsA");
 
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
     const uint4 item = c.items[it];
@@ -159,9 +184,10 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
       uint4* tA = reinterpret_cast<uint4*>(s.tagsA);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) tA[tid + NT * k] = z4;
-      if (tid < NBK / 16 + 16) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
+      for (int k = 0; k < (int)(sizeof(uint2) * NBK / 16 / NT); ++k) tA[tid + NT * k] = z4;
+      if (tid < (NBK / 4 + (NBK >> BB_SHIFT) / 4) / 4) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
       if (tid < 128) reinterpret_cast<uint32_t*>(s.run_big)[tid] = 0u;  // run_big and run_bad
+      if (tid < 32) s.survb[tid] = 0u;
       if (warp == 0) {
         const uint32_t rel = g0 - T0, wq = rel >> 5;
         uint32_t v = __funnelshift_r(c.sbits[wq + lane], c.sbits[wq + lane + 1u], rel & 31u);
@@ -183,6 +209,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     const uint32_t ebase = segB[er * F];
     const uint32_t nextB = segB[er * F + fed0 + 1u];        // first word of the next FED
     const bool one_seg = g0 + len <= nextB;
+    uint16_t* const o_module = c.d_module + g0 + tid; uint16_t* const o_row = c.d_row + g0 + tid; uint16_t* const o_col = c.d_col + g0 + tid;
+    int32_t* const o_charge = c.d_charge + g0 + tid; int32_t* const o_clus = c.d_clus + g0 + tid; uint8_t* const o_status = c.d_status + g0 + tid;
     uint32_t key[NJ], chg[NJ];
     uint32_t fl = 0u;    // per word j: bit j below threshold, bit 4 + j duplicate
     uint32_t kpack = 0u; // per word j: its slot in the bucket (4 bits)
@@ -204,14 +232,14 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       if (ok) e = calibrate(c, w[j] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
       else { m = row = col = 0xFFFFu; }
       if (valid) {
-        c.d_module[g] = (uint16_t)m; c.d_row[g] = (uint16_t)row; c.d_col[g] = (uint16_t)col; c.d_charge[g] = e;
+        o_module[NT * j] = (uint16_t)m; o_row[NT * j] = (uint16_t)row; o_col[NT * j] = (uint16_t)col; o_charge[NT * j] = e;
         if (!ok) {  // undecodable words are finished here
-          c.d_status[g] = (uint8_t)st; c.d_clus[g] = -1;
+          o_status[NT * j] = (uint8_t)st; o_clus[NT * j] = -1;
           atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
         }
       }
-      const uint32_t bw = s.bits[j * 8 + warp];
-      const uint32_t r = s.pre[j * 8 + warp] + __popc(bw & le_mask) - 1u;  // a decodable word lies in a run: r >= 0
+      const uint32_t bw = s.bits[j * NWARP + warp];
+      const uint32_t r = s.pre[j * NWARP + warp] + __popc(bw & le_mask) - 1u;  // a decodable word lies in a run: r >= 0
       const bool below = e < c.thr;  // S9
       key[j] = NOKEY; chg[j] = (uint32_t)e;
       if (ok) {
@@ -226,9 +254,9 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           uint32_t kk = k;
           if (k < 4u) { tagA16[b * 4u + k] = (uint16_t)tag; s.idsA[b * 4u + k] = idv; }
           else {  // rare: the bucket's first level is full
-            const uint32_t bB = b >> 3, shB = (bB & 3u) * 8u;
+            const uint32_t bB = b >> BB_SHIFT, shB = (bB & 3u) * 8u;
             const uint32_t kb = (atomicAdd(&s.cntB[bB >> 2], 1u << shB) >> shB) & 0xFFu;
-            if (kb < 4u) s.tagsB[bB * 4u + kb] = tag | ((b & 7u) << 16) | (p << 19) | (below ? 1u << 29 : 0u);
+            if (kb < 4u) s.tagsB[bB * 4u + kb] = tag | ((b & BB_MASK) << 16) | (p << B_WORD) | (below ? 1u << B_BELOW : 0u);
             else fail = true;
             kk = 4u + (kb < 4u ? kb : 0u);
           }
@@ -262,11 +290,9 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       uint32_t* const el = s.edge[warp];
       uint32_t cand = 0u;  // bit j: the pixel of word j sits in its bucket more than once (S10)
 #pragma unroll
-      for (int half = 0; half < 2; ++half) {
+      for (int j = 0; j < NJ; ++j) {
         uint32_t ne = 0u;
-#pragma unroll
-        for (int jj = 0; jj < 2; ++jj) {
-          const int j = 2 * half + jj;
+        {
           const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
           const uint32_t p = tid + NT * j;
           const uint32_t h = hash_of(key[j]);
@@ -274,12 +300,15 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
             const uint32_t b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
             const uint2 x = s.tagsA[b];
             uint32_t nm = __popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww));
-            if ((x.y >> 31) && key[j] != NOKEY) nm += matches_B(s, b, want);  // rare: the first level is full
+            if (x.y >= 0x10000u && key[j] != NOKEY) nm += matches_B(s, b, want);  // rare: the first level is full
             cand |= (nm >= 2u && key[j] != NOKEY) ? 1u << j : 0u;
           }
-          const uint32_t nE = lookup(s, h + D_E), nS = lookup(s, h + D_S), nSW = lookup(s, h + D_SW), nSE = lookup(s, h + D_SE);
-          const uint32_t t1 = nS != NONE ? nS : nSW;
-          const bool f0 = live && nE != NONE, f1 = live && t1 != NONE, f2 = live && nS == NONE && nE == NONE && nSE != NONE;
+          const uint32_t hn[4] = {h + D_E, h + D_S, h + D_SW, h + D_SE};
+          uint32_t nb[4];
+          lookup4(s, sb_tags, hn, nb);
+          const uint32_t nE = nb[0], nS = nb[1], nSW = nb[2], nSE = nb[3];  // >= 0x8000: no live pixel there
+          const uint32_t t1 = nS < 0x8000u ? nS : nSW;
+          const bool f0 = live && nE < 0x8000u, f1 = live && t1 < 0x8000u, f2 = live && nS >= 0x8000u && nE >= 0x8000u && nSE < 0x8000u;
           const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
           if (f0) el[ne + __popc(m0 & lt_mask)] = p | (nE << 16);
           ne += __popc(m0);
@@ -364,7 +393,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         if (Q > Q_SAFE) s.run_bad[run] = 1;  // 32-bit weighted sums may have wrapped
       }
       const uint32_t bal = __ballot_sync(FULL, sv);
-      if (lane == 0) s.survb[j * 8 + warp] = bal;
+      if (lane == 0) s.survb[j * NWARP + warp] = bal;
       surv |= sv ? 1u << j : 0u;
     }
     __syncthreads();
@@ -381,7 +410,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     auto rank_before = [&](uint32_t pos) {  // survivors among the words before pos (all lanes call it together)
       const uint32_t wi = pos >> 5;
       const uint32_t r = __shfl_sync(FULL, sv_pre, wi) + __popc(__shfl_sync(FULL, sv_bits, wi) & ((1u << (pos & 31u)) - 1u));
-      return pos >= TILE_WORDS ? sv_total : r;
+      return pos >= 1024u ? sv_total : r;
     };
     const uint32_t wbase = s.wbase;
 #pragma unroll
@@ -409,7 +438,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     for (int j = 0; j < NJ; ++j) {
       if (key[j] == NOKEY) continue;
       if (s.run_bad[key[j] >> 17]) continue;
-      const uint32_t p = tid + NT * j, g = g0 + p;
+      const uint32_t p = tid + NT * j;
       uint32_t so; int32_t cl = -1;
       if ((fl >> j) & 16u) { so = ST_DUP; cntA += 1u; }
       else if ((fl >> j) & 1u) { so = ST_BELOW; cntA += 0x10000u; }
@@ -418,7 +447,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
         cntP += root[j] == p ? 1u : 0u;
       }
-      c.d_status[g] = (uint8_t)so; c.d_clus[g] = cl;
+      o_status[NT * j] = (uint8_t)so; o_clus[NT * j] = cl;
     }
     __syncwarp();
     if (warp * 32u < R) {  // the warps that hold a run each in some lane
