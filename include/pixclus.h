@@ -216,7 +216,7 @@ int pix_overflow_runs(pix_handle* h, uint32_t* out);
 
 /* Optional per-kernel timing for benchmarks (not legal during stream capture).  While enabled, every chunk
  * records CUDA events between its kernels on the caller's stream.  pix_read_profile waits for them and adds up
- * the device time per kernel since the last read: ms_out[8] = {init, fused, findrun, overflow, finalize, 0, 0, 0};
+ * the device time per kernel since the last read: ms_out[8] = {init, runs, tile, overflow, finalize, 0, 0, 0};
  * *n_chunks_out = chunks covered. */
 int pix_set_profiling(pix_handle* h, int enable);
 int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out);

@@ -83,8 +83,6 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.ev_cnt = (uint32_t*)take(Ec * pix::EC_STRIDE * 4);
   c.ctl = (uint32_t*)take(pix::CTL_WORDS * 4);
   c.ovf_list = (uint32_t*)take(Ec * M * 4);
-  c.mid_list = (uint32_t*)take(Ec * M * 4);
-  c.big_list = (uint32_t*)take(Ec * M * 4);
   c.list_cap = (uint32_t)(Ec * M);
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);

@@ -1,6 +1,6 @@
 // cluster.cu -- the overflow kernel: a4 findClus fused with a5 (cluster sums, charge cut, renumber, temp records)
-// for the module runs the warp kernels (fused.cu, findrun.cu) could not take: runs longer than 512 words, dense
-// runs that overflow a hash bucket neighbourhood, charge sums beyond 32 bits.  One block per run, tables in the global workspace, 64-bit sums.
+// for the module runs the tile kernel (tile.cu) could not take: runs longer than a tile (1024 words), items whose
+// position hash overflowed, charge sums beyond 32 bits.  One block per run, tables in the global workspace, 64-bit sums.
 //
 // "clusters the pixels on each detector module".  The connectivity rule, the duplicate rule,
 // the canonical numbering and the charge cut are DESIGN.md readings S9, S10, S13, S14, S18.
@@ -257,9 +257,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
 // ------------------------------------------------------------------ kernel
 // One block per run, taken from a task list by ticket.  Runs of up to CAP digis keep all their tables in shared
 // memory; longer ones go to the next list (a larger size of this kernel) or, in the last size, use the global
-// workspace.  One size is in use: 256 threads / 2048 digis (88 KB).  (Measured: as the kernel for ALL the runs the
-// fused kernel leaves, in a 128-thread / 512-digi size, it took 4.3 ms on 200 PU200-like events where the bucket-hash
-// run kernels of findrun.cu take 1.9 ms.)
+// workspace.  One size is in use: 256 threads / 2048 digis (88 KB).
 constexpr size_t SMEM_PER_DIGI = 8 + 8 + 2 * 4 + 4 * 5;  // sx, sy, 2 hash slots, pos, chg, label, q, npix
 
 __device__ __forceinline__ Tables<uint32_t> carve(unsigned char* base, uint32_t cap) {
@@ -327,7 +325,7 @@ cudaError_t configure_overflow_kernel() {
   return cudaFuncSetAttribute(block_kernel<T_B, CAP_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(CAP_B * SMEM_PER_DIGI));
 }
 
-// the runs the run kernels (findrun.cu) left: longer than 1024 digis, dense, or with 64-bit charge sums
+// the runs the tile kernel left: longer than 1024 digis, hash overflow, or with 64-bit charge sums
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
   block_kernel<T_B, CAP_B><<<n_sm * 2, T_B, CAP_B * SMEM_PER_DIGI, stream>>>(c, c.ovf_list, CTL_OVF_COUNT, CTL_OVF_TICKET, nullptr, 0u);
 }

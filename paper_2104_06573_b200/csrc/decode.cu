@@ -1,6 +1,6 @@
 // decode.cu -- the two set-up kernels of a launch group: init (segment table, range sentinels, zeroed counters) and
 // segfill (segment of every 128-word chunk; end of every event's last module run, a3 of the path PAPER.md:31
-// describes).  The decode itself (a1, a2) lives in the fused kernel (fused.cu).  Nothing here is shared with oracle/.
+// describes).  The decode itself (a1, a2) lives in the tile kernel (tile.cu).  Nothing here is shared with oracle/.
 #include "pix_common.cuh"
 #include "pix_device.cuh"
 
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk
 
 // chunk_seg[ci] = event << 16 | FED of the first word of 128-word chunk ci (its first word inside the launch
 // group).  One thread per segment writes the chunks that start inside it.  One warp per event closes the event's
-// last run: module_end of the module of the event's last decodable word (the fused kernel closes a run when it
+// last run: module_end of the module of the event's last decodable word (the runs kernel closes a run when it
 // sees the next run start of the same event, and never looks back beyond the start of an event).
 __global__ void __launch_bounds__(256) segfill_kernel(const __grid_constant__ Chunk c) {
   const uint32_t F = c.F, Ec = c.e1 - c.e0, S = Ec * F;

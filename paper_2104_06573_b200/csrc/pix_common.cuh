@@ -7,11 +7,11 @@
 // Kernel chain for one chunk of events:
 //   init      -> segment table, range sentinels, zeroed counters; segfill -> segment of every 128-word chunk,
 //                end of every event's last run
-//   fused     -> a1 decode + a2 calibrate + a3 run boundaries + a4 findClus + a5 sums/cut/renumber for every module
-//                run that fits a warp's 256-word window (home chunk of 128 words + the head of the next chunk)
-//   findrun   -> a4 + a5 for runs that do not fit a window: one warp per run, two sizes (512 / 1024 words)
-//   overflow  -> a4 + a5 for the runs neither could take (longer than the window, pathological
-//                charge sums): generic block-per-run kernel, tables in global workspace
+//   runs      -> a3 run boundaries: one start bit per word, module_first / module_end, run counts (runs.cu)
+//   pack      -> work items: stretches of at most 1024 words holding whole module runs (runs.cu)
+//   tile      -> a1 decode + a2 calibrate + a4 findClus + a5 sums/cut/renumber, one block per item (tile.cu)
+//   overflow  -> a4 + a5 for the runs the tile kernel could not take (longer than a tile, pathological
+//                charge sums, hash overflow): generic block-per-run kernel, tables in global workspace (cluster.cu)
 //   offsets   -> a6 clamp + prefix scan (Fig. 3), summary, scatter work list
 //   scatter   -> cluster records to their final place
 // Nothing here is shared with oracle/.
@@ -37,7 +37,7 @@ constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus;
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
        EC_PRECUT, EC_PUSHED /* runs the event has put on the task lists (at most M) */, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_MID_COUNT = 3, CTL_MID_TICKET = 4, CTL_BIG_COUNT = 5, CTL_BIG_TICKET = 6, CTL_RANGE_TICKET = 7, CTL_TEMP_COUNT = 8, CTL_ITEM_COUNT = 9, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_TEMP_COUNT = 8, CTL_ITEM_COUNT = 9, CTL_WORDS = 16 };
 // work items of the tile kernel (runs.cu packs them, tile.cu takes them): x = global index of the first word,
 // y = words | flags << 16, z = event (launch-group relative) | FED of the first word << 16
 #ifndef PIX_TILE_WORDS
@@ -81,8 +81,6 @@ struct Chunk {
   uint32_t* segB;           // [(e1-e0)*F + 1] global word index where segment (event, fed) starts
   uint32_t* ev_cnt;         // [(e1-e0)*EC_STRIDE]
   uint32_t* ctl;            // [CTL_WORDS]
-  uint32_t* mid_list;       // [(e1-e0)*M] task ids left by the fused kernel to the warp-per-run kernel (findrun)
-  uint32_t* big_list;       // [(e1-e0)*M] runs of 513..1024 words, left by findrun<512> to findrun<1024>
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
   uint32_t list_cap;        // (e1-e0)*M: every event lists at most M runs (push_run)
   uint32_t* chunk_seg;      // [cap_words/128 + 2] event_rel << 16 | fed of the chunk's first word
@@ -114,19 +112,15 @@ __device__ __forceinline__ void put_temp(const Chunk& c, uint32_t i, uint32_t fi
 
 // launchers (host), one per kernel; all asynchronous on `stream`
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream);
-void launch_fused(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
-void launch_findrun(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);
 void launch_tile(const Chunk& c, int n_sm, cudaStream_t stream);
 cudaError_t configure_tile_kernel();
 
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream);
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream);
-cudaError_t configure_fused_kernel();
-cudaError_t configure_findrun_kernel();
 cudaError_t configure_finalize_kernel();
 cudaError_t configure_overflow_kernel();
 constexpr uint32_t MAX_MODULES = 16383;  // finalize keeps the M+1 offsets of an event in shared memory
-constexpr int LAUNCHES_PER_CHUNK = 8;    // init, segfill, fused, findrun x2, overflow, offsets, scatter
+constexpr int LAUNCHES_PER_CHUNK = 8;    // init, segfill, runs, pack, tile, overflow, offsets, scatter
 
 }  // namespace pix

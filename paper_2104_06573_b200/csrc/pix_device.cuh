@@ -1,5 +1,5 @@
-// pix_device.cuh -- device helpers shared by the cluster kernels (fused.cu, findrun.cu, cluster.cu): the word decode
-// and the calibration (a1, a2), the union step, and the bucket position hash.  One definition each.
+// pix_device.cuh -- device helpers shared by the kernels (runs.cu, tile.cu, cluster.cu): the word decode
+// and the calibration (a1, a2), the run bookkeeping (a3) and the union step.  One definition each.
 // PAPER.md:31 names the steps ("unpacks them, calibrates the individual pixels, and clusters the pixels on each
 // detector module"); the arithmetic is fixed by readings S1-S10, S13 of DESIGN.md.  Nothing here is shared with oracle/.
 #pragma once
@@ -84,73 +84,5 @@ __device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
     else { a = p; b = lo; }
   }
 }
-
-// ------------------------------------------------------------------ position hash (S10, S13)
-// 2^NB_LOG2 buckets of 4 slots: one 128-bit shared load per lookup and no probing loop on the common path.
-// h = key * HASH_MUL mod 2^KEY_BITS is a bijection on the KEY_BITS-bit keys; bucket = top NB_LOG2 bits of h, tag =
-// the rest, so (bucket, tag) names the key exactly.  A key whose home bucket is full goes to the next bucket(s)
-// and records the displacement: slot = disp (2) | tag | digi (DIGI_BITS) | below_threshold (1).  Slots of a bucket
-// fill in order and are never emptied; equal keys meet in one slot and keep the lowest digi (S10: first index wins).
-template <uint32_t KEY_BITS, uint32_t NB_LOG2, uint32_t DIGI_BITS>
-struct BucketHash {
-  static constexpr uint32_t EMPTY = 0xFFFFFFFFu, HASH_MUL = 0x9E3779B1u, MAX_DISP = 3;
-  static constexpr uint32_t KEY_MASK = (1u << KEY_BITS) - 1u, TAG_BITS = KEY_BITS - NB_LOG2, TAG_MASK = (1u << TAG_BITS) - 1u;
-  static constexpr uint32_t NBUCKET = 1u << NB_LOG2, SLOTS = 4u * NBUCKET, SH = DIGI_BITS + 1u, DIGI_MASK = (1u << DIGI_BITS) - 1u;
-  static_assert(2u + TAG_BITS + SH <= 32u, "slot: disp | tag | digi | below");
-
-  static __device__ __forceinline__ uint32_t mix(uint32_t key) { return (key * HASH_MUL) & KEY_MASK; }
-  // mixed value of key + d, given the mixed value of key
-  static __device__ __forceinline__ uint32_t step(uint32_t h, uint32_t d) { return (h + d * HASH_MUL) & KEY_MASK; }
-
-  // 0: inserted; 1: the key was already there (a duplicate pixel, S10); 2: no room within MAX_DISP buckets.
-  // (Looking at the bucket first and aiming one atomicCAS at its first free slot was measured slower.)
-  static __device__ __noinline__ uint32_t insert(uint32_t* tab, uint32_t key, uint32_t t, uint32_t below) {
-    const uint32_t h = mix(key), tag = h & TAG_MASK;
-    uint32_t p = (h >> TAG_BITS) * 4u, res = 2u;
-#pragma unroll 1
-    for (uint32_t i = 0; i < 4u * (MAX_DISP + 1u) && res == 2u; ++i, p = (p + 1u) & (SLOTS - 1u)) {
-      const uint32_t want = ((i >> 2) << TAG_BITS) | tag, mine = (want << SH) | (t << 1) | below;
-      const uint32_t old = atomicCAS(&tab[p], EMPTY, mine);
-      if (old == EMPTY) res = 0u;
-      else if ((old >> SH) == want) { atomicMin(&tab[p], mine); res = 1u; }  // same pixel: the lowest digi owns it
-    }
-    return res;
-  }
-  static __device__ __forceinline__ uint32_t match4(const uint4& e, uint32_t want) {
-    uint32_t r = EMPTY;
-    if ((e.w >> SH) == want) r = e.w;
-    if ((e.z >> SH) == want) r = e.z;
-    if ((e.y >> SH) == want) r = e.y;
-    if ((e.x >> SH) == want) r = e.x;
-    return r;
-  }
-  static __device__ __noinline__ uint32_t find_slow(const uint32_t* tab, uint32_t h) {
-    const uint32_t tag = h & TAG_MASK;
-    uint32_t b = h >> TAG_BITS, r = EMPTY;
-    for (uint32_t i = 1; i <= MAX_DISP && r == EMPTY; ++i) {  // the buckets after the (full) home bucket
-      b = (b + 1u) & (NBUCKET - 1u);
-      const uint4 e = *reinterpret_cast<const uint4*>(&tab[b * 4u]);
-      r = match4(e, (i << TAG_BITS) | tag);
-      if (e.w == EMPTY) break;
-    }
-    return r;
-  }
-  // slot contents of the key whose mixed value is h, or EMPTY
-  static __device__ __forceinline__ uint32_t find(const uint32_t* tab, uint32_t h) {
-    const uint4 e = *reinterpret_cast<const uint4*>(&tab[(h >> TAG_BITS) * 4u]);
-    uint32_t r = match4(e, h & TAG_MASK);
-    if (r == EMPTY && e.w != EMPTY) r = find_slow(tab, h);  // home bucket full, no match (rare): displaced keys
-    return r;
-  }
-  // the home bucket only; full = the bucket has no free slot, so a key that is not in it may sit in the next buckets
-  static __device__ __forceinline__ uint32_t find_home(const uint32_t* tab, uint32_t h, bool& full) {
-    const uint4 e = *reinterpret_cast<const uint4*>(&tab[(h >> TAG_BITS) * 4u]);
-    const uint32_t r = match4(e, h & TAG_MASK);
-    full = r == EMPTY && e.w != EMPTY;
-    return r;
-  }
-  static __device__ __forceinline__ uint32_t digi(uint32_t e) { return (e >> 1) & DIGI_MASK; }
-  static __device__ __forceinline__ bool live(uint32_t e) { return e != EMPTY && !(e & 1u); }
-};
 
 }  // namespace pix

@@ -267,3 +267,73 @@ def test_graph_replay_equals_direct_launch(gu, full):
     finally:
         torch.cuda.synchronize()
         pix.pix_destroy(h)
+
+
+def test_many_tiny_runs(gu, full):
+    """Every module holds one to three pixels, so a 1024-word stretch has far more than 255 module runs: the packing
+    of runs into work items has to cut shorter items (runs.cu, ITEM_RUNS).  Valid, contiguous events."""
+    rng = np.random.default_rng(5)
+    events = []
+    for _ in range(3):
+        module, row, col = [], [], []
+        for m in range(full.n_modules):
+            n = int(rng.integers(1, 4))
+            r0, c0 = int(rng.integers(0, 158)), int(rng.integers(0, 414))
+            cells = [(r0, c0), (r0 + 1, c0 + 1), (r0, c0 + 2)][:n]  # diagonal neighbours and a gap
+            for r, c in cells:
+                module.append(m); row.append(r); col.append(c)
+        adc = rng.integers(1, 256, size=len(module))
+        events.append((np.array(module), np.array(row), np.array(col), adc))
+    check(gu, full, _hand_batch(full, events))
+
+
+def _tile_bucket(run, row, col):
+    """The tile kernel's position hash (tile.cu): key = run | row | col, h = (key << 7) * 0x9E3779B1 mod 2^32, bucket = top 11 bits."""
+    key = (np.uint64(run) << np.uint64(17)) | (row.astype(np.uint64) << np.uint64(9)) | col.astype(np.uint64)
+    return (((key << np.uint64(7)) * np.uint64(0x9E3779B1)) & np.uint64(0xFFFFFFFF)) >> np.uint64(21)
+
+
+@pytest.mark.parametrize("n_same", [5, 8, 9, 24])
+def test_hash_bucket_overflow(gu, full, n_same):
+    """n_same pixels of one run that all fall into one bucket of the tile kernel's hash (4 entries per bucket, 4 more in
+    the second level, beyond that the item goes to the block-per-run kernel), among ordinary pixels and next to a
+    second run, with neighbours among the colliding pixels where the bucket has some."""
+    rng = np.random.default_rng(17 + n_same)
+    inv = full.inverse()
+    mods = np.nonzero(inv["fed"] == 0)[0][:2]
+    rr, cc = np.divmod(np.arange(160 * 416), 416)
+    events = []
+    for run in (0, 1):  # the colliding run is the item's first or second run
+        bk = _tile_bucket(run, rr, cc)
+        target = int(rng.integers(0, 2048))
+        same = np.nonzero(bk == target)[0]
+        assert len(same) >= n_same
+        pick = same[:n_same]
+        others = rng.choice(160 * 416, size=150, replace=False)
+        near = np.unique(np.clip(np.concatenate([pick + 1, pick + 416, pick - 415]), 0, 160 * 416 - 1))  # neighbours of the colliding pixels
+        sel = np.unique(np.concatenate([pick, others, near]))
+        rng.shuffle(sel)
+        filler = rng.choice(160 * 416, size=60, replace=False)
+        if run == 0:
+            module = np.concatenate([np.full(len(sel), mods[0]), np.full(len(filler), mods[1])]); pos = np.concatenate([sel, filler])
+        else:
+            module = np.concatenate([np.full(len(filler), mods[0]), np.full(len(sel), mods[1])]); pos = np.concatenate([filler, sel])
+        events.append((module, pos // 416, pos % 416, rng.integers(1, 256, size=len(pos))))
+    check(gu, full, _hand_batch(full, events))
+
+
+def test_cluster_charge_beyond_32_bit_sums(gu, full):
+    """One cluster whose charge makes the 32-bit weighted sums wrap (16 x 22 pixels at ADC 255) in a run short enough
+    for the tile kernel, next to a run of 400 low-charge pixels in one cluster (more than 255 pixels: the packed
+    pixel count does not apply) and an ordinary run: the first goes to the 64-bit block-per-run kernel."""
+    rng = np.random.default_rng(23)
+    inv = full.inverse()
+    a, b, c = np.nonzero(inv["fed"] == 0)[0][:3]
+    r1, c1 = np.divmod(np.arange(16 * 22), 22)
+    r2, c2 = np.divmod(np.arange(400), 20)
+    pos3 = rng.choice(160 * 416, size=100, replace=False)
+    module = np.concatenate([np.full(len(r1), a), np.full(len(r2), b), np.full(len(pos3), c)])
+    row = np.concatenate([r1 + 40, r2 + 10, pos3 // 416]); col = np.concatenate([c1 + 300, c2 + 100, pos3 % 416])
+    adc = np.concatenate([np.full(len(r1), 255), np.full(len(r2), 45), rng.integers(1, 256, size=len(pos3))])
+    got, exp = check(gu, full, _hand_batch(full, [(module, row, col, adc)]))
+    assert int(exp[0]["c_n_pix"].max()) == 400 and int(exp[0]["c_charge"].max()) > 0xFFFFFFFF // 415
