@@ -62,7 +62,8 @@ struct __align__(16) TileSmem {
   uint32_t edge[NT / 32][ECAP];  // per warp: the edges its words found, a | b << 16
   uint32_t label[TILE_WORDS];
   uint32_t bits[32], pre[32];        // run-start bits of the item, run starts before each word of bits
-  uint32_t survb[32];                // roots that survive the cut
+  uint32_t survb[32];                // roots that survive the cut, in root order
+  uint32_t rootb[32];                // words that are roots
   uint16_t run_pos[256], run_mod[256];
   uint8_t run_big[256], run_bad[256];
   uint32_t n_runs, wbase, pad[2];
@@ -175,6 +176,13 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t p = tid + NT * j;
       w[j] = p < len ? __ldg(c.words + g0 + p) : 0u;
     }
+    const uint32_t ebase = segB[er * F];
+    const uint32_t nextB = segB[er * F + fed0 + 1u];        // first word of the next FED
+    if (it + gridDim.x < n_items) {  // the next item of this block: its words on their way into L2 / L1 while this one is clustered
+      const uint4 nx = c.items[it + gridDim.x];
+      const uint32_t* q = c.words + nx.x + 32u * tid;  // one 128-byte line per thread covers up to 8192 words
+      if (32u * tid < (nx.y & 0xFFFFu)) asm volatile("prefetch.global.L2 [%0];" :: "l"(q));
+    }
     // the item's stretch of the temp record area, one slot per word: asked for now, needed in P4
     uint32_t wbase_t0 = 0u;
     if (tid == 0 && cluster_it) wbase_t0 = alloc_temp(c, len);
@@ -206,8 +214,6 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     __syncthreads();
     // ================================================================== P1: decode, calibrate, insert
-    const uint32_t ebase = segB[er * F];
-    const uint32_t nextB = segB[er * F + fed0 + 1u];        // first word of the next FED
     const bool one_seg = g0 + len <= nextB;
     uint16_t* const o_module = c.d_module + g0 + tid; uint16_t* const o_row = c.d_row + g0 + tid; uint16_t* const o_col = c.d_col + g0 + tid;
     int32_t* const o_charge = c.d_charge + g0 + tid; int32_t* const o_clus = c.d_clus + g0 + tid; uint8_t* const o_status = c.d_status + g0 + tid;
@@ -330,7 +336,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       // rare: some pixel appears twice.  Name the owner in every entry of the pixel, mark the other words DUPLICATE,
       // start the labels again and look up once more.
       if (cand) {
-#pragma unroll 1
+#pragma unroll  // (a rolled loop would index key[] at run time and put it into local memory)
         for (int j = 0; j < NJ; ++j) {
           if (!((cand >> j) & 1u)) continue;
           const uint32_t h = hash_of(key[j]);
@@ -359,18 +365,39 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       bool done = !live;
       while (!done) { const uint32_t n = s.label[r]; done = n == r; r = n; }  // single exit: the warp reconverges
       root[j] = live ? r : NONE;
-      if (live && r == p) {  // a root starts its accumulators with its own pixel (the hash is dead: nobody looks up any more)
+      const bool is_root = live && r == p;
+      if (is_root) {  // a root starts its accumulators with its own pixel (the hash is dead: nobody looks up any more)
         const uint32_t big = s.run_big[key[j] >> 17];
         s.sum.qn[p] = big ? chg[j] : (chg[j] | (1u << 24));  // below BIG_RUN words a cluster has at most 255 pixels and Q < 2^24
         s.sum.sx[p] = chg[j] * (key[j] & 511u);
         s.sum.sy[p] = chg[j] * ((key[j] >> 9) & 255u);
         s.sum.npx[p] = 1u;
       }
+      const uint32_t bal = __ballot_sync(FULL, is_root);
+      if (lane == 0) s.rootb[j * NWARP + warp] = bal;
     }
     __syncthreads();
+    // every warp scans the 32 words of the root bitmap for itself: lane l holds word l and the roots before it
+    const uint32_t rt_bits = s.rootb[lane];
+    uint32_t rt_pre = __popc(rt_bits);
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(FULL, rt_pre, d);
+      if (lane >= (uint32_t)d) rt_pre += o;
+    }
+    const uint32_t n_roots = __shfl_sync(FULL, rt_pre, 31);
+    rt_pre -= __popc(rt_bits);
+    auto roots_before = [&](uint32_t pos) {  // roots among the words before pos (all lanes call it together)
+      const uint32_t wi = pos >> 5;
+      const uint32_t r = __shfl_sync(FULL, rt_pre, wi) + __popc(__shfl_sync(FULL, rt_bits, wi) & ((1u << (pos & 31u)) - 1u));
+      return pos >= 1024u ? n_roots : r;
+    };
+    uint16_t* const rlist = reinterpret_cast<uint16_t*>(s.edge);  // the roots in word order (the edge lists are dead)
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, r = root[j];
+      const uint32_t di = __shfl_sync(FULL, rt_pre, j * NWARP + warp) + __popc(__shfl_sync(FULL, rt_bits, j * NWARP + warp) & lt_mask);
+      if (r == p) rlist[di] = (uint16_t)p;
       if (r != NONE && r != p) {
         const uint32_t big = s.run_big[key[j] >> 17];
         atomicAdd(&s.sum.qn[r], big ? chg[j] : (chg[j] | (1u << 24)));
@@ -380,24 +407,28 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       }
     }
     __syncthreads();
-    // ================================================================== P4: cut, renumber, temp records
-    uint32_t surv = 0u;  // bit j: word j is a root that survives the cut
-#pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-      const uint32_t p = tid + NT * j;
+    // ================================================================== P4: cut, renumber, temp records -- one root per thread
+    // root i of the list: word, run, charge, pixels
+    auto load_root = [&](uint32_t i, uint32_t& p, uint32_t& run, uint32_t& Q, uint32_t& np) {
+      p = rlist[i];
+      run = s.pre[p >> 5] + __popc(s.bits[p >> 5] & ((2u << (p & 31u)) - 1u)) - 1u;
+      const uint32_t big = s.run_big[run], a = s.sum.qn[p];
+      Q = big ? a : (a & 0xFFFFFFu); np = big ? s.sum.npx[p] : (a >> 24);
+    };
+    for (uint32_t i0 = 0u; i0 < n_roots; i0 += NT) {  // block-uniform trip count (one round unless the item is all single pixels)
+      const uint32_t i = i0 + tid;
       bool sv = false;
-      if (root[j] == p) {
-        const uint32_t run = key[j] >> 17;
-        const uint32_t a = s.sum.qn[p], Q = s.run_big[run] ? a : (a & 0xFFFFFFu);
+      if (i < n_roots) {
+        uint32_t p, run, Q, np;
+        load_root(i, p, run, Q, np);
         sv = (int32_t)Q >= c.cut;  // S9: equality keeps (Q < 2^31)
         if (Q > Q_SAFE) s.run_bad[run] = 1;  // 32-bit weighted sums may have wrapped
       }
       const uint32_t bal = __ballot_sync(FULL, sv);
-      if (lane == 0) s.survb[j * NWARP + warp] = bal;
-      surv |= sv ? 1u << j : 0u;
+      if (lane == 0) s.survb[i >> 5] = bal;  // the words beyond the roots stay 0 (P0)
     }
     __syncthreads();
-    // every warp scans the 32 words of the survivor bitmap for itself: lane l holds word l and the survivors before it
+    // survivors in root order: lane l holds word l of the bitmap and the survivors before it
     const uint32_t sv_bits = s.survb[lane];
     uint32_t sv_pre = __popc(sv_bits);
 #pragma unroll
@@ -407,23 +438,22 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     const uint32_t sv_total = __shfl_sync(FULL, sv_pre, 31);
     sv_pre -= __popc(sv_bits);
-    auto rank_before = [&](uint32_t pos) {  // survivors among the words before pos (all lanes call it together)
-      const uint32_t wi = pos >> 5;
-      const uint32_t r = __shfl_sync(FULL, sv_pre, wi) + __popc(__shfl_sync(FULL, sv_bits, wi) & ((1u << (pos & 31u)) - 1u));
-      return pos >= 1024u ? sv_total : r;
+    auto surv_before_root = [&](uint32_t d) {  // survivors among the roots before root d (all lanes call it together)
+      const uint32_t wi = d >> 5;
+      const uint32_t r = __shfl_sync(FULL, sv_pre, wi) + __popc(__shfl_sync(FULL, sv_bits, wi) & ((1u << (d & 31u)) - 1u));
+      return d >= 1024u ? sv_total : r;
     };
+    auto rank_before = [&](uint32_t pos) { return surv_before_root(roots_before(pos)); };  // survivors among the words before pos
     const uint32_t wbase = s.wbase;
-#pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-      const uint32_t p = tid + NT * j;
-      const bool is_root = root[j] == p;
-      const uint32_t run = is_root ? key[j] >> 17 : 0u;
-      const uint32_t rank = rank_before(p), base = rank_before(is_root ? (uint32_t)s.run_pos[run] : 0u);
-      if (is_root) {
+    for (uint32_t i0 = 0u; i0 < n_roots; i0 += NT) {
+      const uint32_t i = i0 + tid;
+      const bool valid = i < n_roots;
+      uint32_t p = 0u, run = 0u, Q = 0u, np = 0u;
+      if (valid) load_root(i, p, run, Q, np);
+      const uint32_t rank = surv_before_root(i), base = rank_before(valid ? (uint32_t)s.run_pos[run] : 0u);
+      if (valid) {
         uint32_t id = NO_ID;
-        if ((surv >> j) & 1u) {
-          const uint32_t big = s.run_big[run];
-          const uint32_t a = s.sum.qn[p], Q = big ? a : (a & 0xFFFFFFu), np = big ? s.sum.npx[p] : (a >> 24);
+        if ((int32_t)Q >= c.cut) {
           id = rank - base;
           const float fq = (float)Q;  // S18: exact integer sums, one rounding each + a 2-ulp division (within 1e-5)
           put_temp(c, wbase + rank, g0 + p - ebase, np, Q, __fdividef((float)s.sum.sx[p], fq), __fdividef((float)s.sum.sy[p], fq));
