@@ -43,6 +43,9 @@ constexpr uint32_t NBK = 2 * TILE_WORDS, NBK_LOG2 = TILE_WORDS == 1024 ? 11 : 10
 constexpr uint32_t HMUL = 0x9E3779B1u;
 constexpr uint32_t D_E = (1u << 7) * HMUL, D_SW = (511u << 7) * HMUL, D_S = (512u << 7) * HMUL, D_SE = (513u << 7) * HMUL;
 constexpr uint32_t MARK = 0xFFFFFFFDu;               // label of a word that is not a live pixel
+// A word's state word: key (25 bits: run | row | col) and flags.  The hash shifts the flags out (key << 7).
+constexpr uint32_t K_BELOW = 1u << 25, K_DUP = 1u << 26, K_SLOT = 27, K_CAND = 1u << 31;  // K_SLOT: 4 bits, the word's slot in its bucket
+#define ROT4(a) do { const uint32_t t_ = a[0]; a[0] = a[1]; a[1] = a[2]; a[2] = a[3]; a[3] = t_; } while (0)
 constexpr uint32_t NONE = 0xFFFFu, NO_ID = 0xFFFFu;
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;      // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
 constexpr uint32_t BIG_RUN = 256u;                   // runs this long count their pixels in a word of their own
@@ -72,6 +75,8 @@ static_assert(sizeof(TileSmem) <= 233472 / BLOCKS_PER_SM - 1024, "BLOCKS_PER_SM 
 static_assert(sizeof(uint2) * NBK == 4 * 4 * TILE_WORDS, "the accumulators take the place of the first-level tags");
 
 __device__ __forceinline__ uint32_t hash_of(uint32_t key) { return (key << 7) * HMUL; }
+__device__ __forceinline__ bool k_live(uint32_t k) { return (k & (K_BELOW | K_DUP)) == 0u; }  // NOKEY has every bit set
+__device__ __forceinline__ uint32_t k_run(uint32_t k) { return (k >> 17) & 0xFFu; }
 __device__ __forceinline__ uint32_t bucket_of(uint32_t h) { return h >> (32 - NBK_LOG2); }
 __device__ __forceinline__ uint32_t want_of(uint32_t h) { return ((h >> 7) & TAG_MASK) + 1u; }  // 1 .. 16384: bit 15 stays free for zero_half
 __device__ __forceinline__ uint32_t zero_half(uint32_t x, uint32_t ww) {
@@ -214,14 +219,13 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     __syncthreads();
     // ================================================================== P1: decode, calibrate, insert
+    // The loops over a thread's four words are rolled (the kernel has to fit the instruction cache); the words' state
+    // stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is always [0].
     const bool one_seg = g0 + len <= nextB;
-    uint16_t* const o_module = c.d_module + g0 + tid; uint16_t* const o_row = c.d_row + g0 + tid; uint16_t* const o_col = c.d_col + g0 + tid;
-    int32_t* const o_charge = c.d_charge + g0 + tid; int32_t* const o_clus = c.d_clus + g0 + tid; uint8_t* const o_status = c.d_status + g0 + tid;
-    uint32_t key[NJ], chg[NJ];
-    uint32_t fl = 0u;    // per word j: bit j below threshold, bit 4 + j duplicate
-    uint32_t kpack = 0u; // per word j: its slot in the bucket (4 bits)
+    uint32_t key[NJ];  // K_* below; NOKEY: not decodable
+    uint32_t cr[NJ];   // charge | root << 16
     bool fail = false;
-#pragma unroll
+#pragma unroll 1
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, g = g0 + p;
       const bool valid = p < len;
@@ -232,28 +236,27 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         fed = sg - er * F;
       }
       uint32_t m, row, col;
-      const uint32_t st = decode_word(c.cab, w[j], fed << 11, m, row, col);
+      const uint32_t st = decode_word(c.cab, w[0], fed << 11, m, row, col);
       const bool ok = valid && st == ST_OK;
       int32_t e = 0;
-      if (ok) e = calibrate(c, w[j] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
+      if (ok) e = calibrate(c, w[0] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
       else { m = row = col = 0xFFFFu; }
       if (valid) {
-        o_module[NT * j] = (uint16_t)m; o_row[NT * j] = (uint16_t)row; o_col[NT * j] = (uint16_t)col; o_charge[NT * j] = e;
+        c.d_module[g] = (uint16_t)m; c.d_row[g] = (uint16_t)row; c.d_col[g] = (uint16_t)col; c.d_charge[g] = e;
         if (!ok) {  // undecodable words are finished here
-          o_status[NT * j] = (uint8_t)st; o_clus[NT * j] = -1;
+          c.d_status[g] = (uint8_t)st; c.d_clus[g] = -1;
           atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
         }
       }
       const uint32_t bw = s.bits[j * NWARP + warp];
       const uint32_t r = s.pre[j * NWARP + warp] + __popc(bw & le_mask) - 1u;  // a decodable word lies in a run: r >= 0
       const bool below = e < c.thr;  // S9
-      key[j] = NOKEY; chg[j] = (uint32_t)e;
+      uint32_t k0 = NOKEY;
       if (ok) {
-        key[j] = (r << 17) | (row << 9) | col;
+        k0 = (r << 17) | (row << 9) | col | (below ? K_BELOW : 0u);
         if ((bw >> lane) & 1u) { s.run_pos[r] = (uint16_t)p; s.run_mod[r] = (uint16_t)m; }
-        if (below) fl |= 1u << j;
         if (cluster_it) {
-          const uint32_t h = hash_of(key[j]), b = bucket_of(h), sh8 = (b & 3u) * 8u;
+          const uint32_t h = hash_of(k0), b = bucket_of(h), sh8 = (b & 3u) * 8u;
           const uint32_t k = (atomicAdd(&s.cnt[b >> 2], 1u << sh8) >> sh8) & 0xFFu;
           const uint32_t tag = want_of(h);
           const uint16_t idv = (uint16_t)(p | (below ? 0x8000u : 0u));
@@ -266,10 +269,12 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
             else fail = true;
             kk = 4u + (kb < 4u ? kb : 0u);
           }
-          kpack |= kk << (4 * j);
+          k0 |= kk << K_SLOT;
         }
       }
       s.label[p] = (ok && !below) ? p : MARK;
+      key[0] = k0; cr[0] = (uint32_t)e;
+      ROT4(w); ROT4(key); ROT4(cr);
     }
     if (!cluster_it) {  // a piece of a run longer than the tile: the block-per-run kernel clusters it
       if ((iflags & ITEM_LONG_HEAD) && tid == 0 && key[0] != NOKEY) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[0]);
@@ -294,20 +299,21 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the
       // edges go to the warp's list, and the list is united with all lanes busy.
       uint32_t* const el = s.edge[warp];
-      uint32_t cand = 0u;  // bit j: the pixel of word j sits in its bucket more than once (S10)
-#pragma unroll
+      bool cand = false;  // a pixel of this thread sits in its bucket more than once (S10); K_CAND marks the word
+#pragma unroll 1
       for (int j = 0; j < NJ; ++j) {
         uint32_t ne = 0u;
         {
-          const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
+          const uint32_t kj = key[0];
+          const bool live = k_live(kj);
           const uint32_t p = tid + NT * j;
-          const uint32_t h = hash_of(key[j]);
+          const uint32_t h = hash_of(kj);
           if (pass == 0) {  // the word's own bucket: more than one entry with its tag
             const uint32_t b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
             const uint2 x = s.tagsA[b];
             uint32_t nm = __popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww));
-            if (x.y >= 0x10000u && key[j] != NOKEY) nm += matches_B(s, b, want);  // rare: the first level is full
-            cand |= (nm >= 2u && key[j] != NOKEY) ? 1u << j : 0u;
+            if (x.y >= 0x10000u && kj != NOKEY) nm += matches_B(s, b, want);  // rare: the first level is full
+            if (nm >= 2u && kj != NOKEY) { cand = true; key[0] = kj | K_CAND; }
           }
           const uint32_t hn[4] = {h + D_E, h + D_S, h + D_SW, h + D_SE};
           uint32_t nb[4];
@@ -331,50 +337,51 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           }
           __syncwarp();
         }
+        ROT4(key);
       }
-      if (!__syncthreads_or(pass == 0 && cand != 0u)) break;
+      if (!__syncthreads_or(pass == 0 && cand)) break;
       // rare: some pixel appears twice.  Name the owner in every entry of the pixel, mark the other words DUPLICATE,
       // start the labels again and look up once more.
-      if (cand) {
-#pragma unroll  // (a rolled loop would index key[] at run time and put it into local memory)
-        for (int j = 0; j < NJ; ++j) {
-          if (!((cand >> j) & 1u)) continue;
-          const uint32_t h = hash_of(key[j]);
-          if (resolve_dup(s, bucket_of(h), want_of(h), tid + NT * j, (kpack >> (4 * j)) & 15u)) fl |= 16u << j;
+#pragma unroll 1
+      for (int j = 0; j < NJ; ++j) {
+        const uint32_t kj = key[0];
+        if (kj != NOKEY && (kj & K_CAND)) {
+          const uint32_t h = hash_of(kj);
+          if (resolve_dup(s, bucket_of(h), want_of(h), tid + NT * j, (kj >> K_SLOT) & 15u)) key[0] = kj | K_DUP;
         }
+        s.label[tid + NT * j] = k_live(key[0]) ? tid + NT * j : MARK;
+        ROT4(key);
       }
-#pragma unroll
-      for (int j = 0; j < NJ; ++j) s.label[tid + NT * j] = (key[j] != NOKEY && !((fl >> j) & 0x11u)) ? tid + NT * j : MARK;
       __syncthreads();
     }
     // ================================================================== P3: roots; sums
     // One pointer-jumping step first (a label only ever moves to an ancestor, so concurrent walkers stay correct).
-#pragma unroll
+#pragma unroll 1
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j;
       const uint32_t l = s.label[p];
       if (l < TILE_WORDS) { const uint32_t ll = s.label[l]; if (ll != l) s.label[p] = ll; }
     }
     __syncwarp();
-    uint32_t root[NJ];
-#pragma unroll
+#pragma unroll 1
     for (int j = 0; j < NJ; ++j) {
-      const uint32_t p = tid + NT * j;
-      const bool live = key[j] != NOKEY && !((fl >> j) & 0x11u);
+      const uint32_t p = tid + NT * j, kj = key[0], e = cr[0] & 0xFFFFu;
+      const bool live = k_live(kj);
       uint32_t r = live ? s.label[p] : 0u;
       bool done = !live;
       while (!done) { const uint32_t n = s.label[r]; done = n == r; r = n; }  // single exit: the warp reconverges
-      root[j] = live ? r : NONE;
+      cr[0] = e | ((live ? r : NONE) << 16);
       const bool is_root = live && r == p;
       if (is_root) {  // a root starts its accumulators with its own pixel (the hash is dead: nobody looks up any more)
-        const uint32_t big = s.run_big[key[j] >> 17];
-        s.sum.qn[p] = big ? chg[j] : (chg[j] | (1u << 24));  // below BIG_RUN words a cluster has at most 255 pixels and Q < 2^24
-        s.sum.sx[p] = chg[j] * (key[j] & 511u);
-        s.sum.sy[p] = chg[j] * ((key[j] >> 9) & 255u);
+        const uint32_t big = s.run_big[k_run(kj)];
+        s.sum.qn[p] = big ? e : (e | (1u << 24));  // below BIG_RUN words a cluster has at most 255 pixels and Q < 2^24
+        s.sum.sx[p] = e * (kj & 511u);
+        s.sum.sy[p] = e * ((kj >> 9) & 255u);
         s.sum.npx[p] = 1u;
       }
       const uint32_t bal = __ballot_sync(FULL, is_root);
       if (lane == 0) s.rootb[j * NWARP + warp] = bal;
+      ROT4(key); ROT4(cr);
     }
     __syncthreads();
     // every warp scans the 32 words of the root bitmap for itself: lane l holds word l and the roots before it
@@ -393,18 +400,19 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       return pos >= 1024u ? n_roots : r;
     };
     uint16_t* const rlist = reinterpret_cast<uint16_t*>(s.edge);  // the roots in word order (the edge lists are dead)
-#pragma unroll
+#pragma unroll 1
     for (int j = 0; j < NJ; ++j) {
-      const uint32_t p = tid + NT * j, r = root[j];
+      const uint32_t p = tid + NT * j, kj = key[0], e = cr[0] & 0xFFFFu, r = cr[0] >> 16;
       const uint32_t di = __shfl_sync(FULL, rt_pre, j * NWARP + warp) + __popc(__shfl_sync(FULL, rt_bits, j * NWARP + warp) & lt_mask);
       if (r == p) rlist[di] = (uint16_t)p;
       if (r != NONE && r != p) {
-        const uint32_t big = s.run_big[key[j] >> 17];
-        atomicAdd(&s.sum.qn[r], big ? chg[j] : (chg[j] | (1u << 24)));
-        atomicAdd(&s.sum.sx[r], chg[j] * (key[j] & 511u));
-        atomicAdd(&s.sum.sy[r], chg[j] * ((key[j] >> 9) & 255u));
+        const uint32_t big = s.run_big[k_run(kj)];
+        atomicAdd(&s.sum.qn[r], big ? e : (e | (1u << 24)));
+        atomicAdd(&s.sum.sx[r], e * (kj & 511u));
+        atomicAdd(&s.sum.sy[r], e * ((kj >> 9) & 255u));
         if (big) atomicAdd(&s.sum.npx[r], 1u);
       }
+      ROT4(key); ROT4(cr);
     }
     __syncthreads();
     // ================================================================== P4: cut, renumber, temp records -- one root per thread
@@ -464,20 +472,22 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     __syncthreads();
     // ================================================================== P5: final status and clus, run outputs, counters
     uint32_t cntA = 0u, cntB = 0u, cntP = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
-#pragma unroll
+#pragma unroll 1
     for (int j = 0; j < NJ; ++j) {
-      if (key[j] == NOKEY) continue;
-      if (s.run_bad[key[j] >> 17]) continue;
+      const uint32_t kj = key[0], rt = cr[0] >> 16;
+      ROT4(key); ROT4(cr);
+      if (kj == NOKEY) continue;
+      if (s.run_bad[k_run(kj)]) continue;
       const uint32_t p = tid + NT * j;
       uint32_t so; int32_t cl = -1;
-      if ((fl >> j) & 16u) { so = ST_DUP; cntA += 1u; }
-      else if ((fl >> j) & 1u) { so = ST_BELOW; cntA += 0x10000u; }
+      if (kj & K_DUP) { so = ST_DUP; cntA += 1u; }
+      else if (kj & K_BELOW) { so = ST_BELOW; cntA += 0x10000u; }
       else {
-        const uint32_t id = lid[root[j]];
+        const uint32_t id = lid[rt];
         if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
-        cntP += root[j] == p ? 1u : 0u;
+        cntP += rt == p ? 1u : 0u;
       }
-      o_status[NT * j] = (uint8_t)so; o_clus[NT * j] = cl;
+      c.d_status[g0 + p] = (uint8_t)so; c.d_clus[g0 + p] = cl;
     }
     __syncwarp();
     if (warp * 32u < R) {  // the warps that hold a run each in some lane
