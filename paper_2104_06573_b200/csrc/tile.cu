@@ -126,9 +126,12 @@ __device__ __forceinline__ void lookup4(const TileSmem& s, uint32_t sb, const ui
 #pragma unroll
   for (int i = 0; i < 4; ++i)
     if (hit[i]) asm volatile("ld.shared.u16 %0, [%1+%2];" : "=r"(res[i]) : "r"(ao[i] + k2[i]), "n"(sizeof(uint2) * NBK));  // idsA follows tagsA
+  const uint32_t full = (hit[0] ? 0u : x1[0]) | (hit[1] ? 0u : x1[1]) | (hit[2] ? 0u : x1[2]) | (hit[3] ? 0u : x1[3]);
+  if (full >= 0x10000u) {  // rare: a miss in a bucket whose first level is full (its fourth entry is taken)
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
-    if (!hit[i] && x1[i] >= 0x10000u) res[i] = lookup_B(s, bucket_of(h[i]), want_of(h[i]));  // rare: the first level is full
+    for (int i = 0; i < 4; ++i)
+      if (!hit[i] && x1[i] >= 0x10000u) res[i] = lookup_B(s, bucket_of(h[i]), want_of(h[i]));
+  }
 }
 
 // rare: the pixel of word p appears more than once in its bucket.  The lowest word owns it (S10); every entry of the
@@ -157,7 +160,9 @@ __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want,
 __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_constant__ Chunk c) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileSmem& s = *reinterpret_cast<TileSmem*>(smem_raw);
-  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  uint32_t tid;
+  asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid));  // read once: the compiler would re-read the special register all over the kernel
+  const uint32_t lane = tid & 31u, warp = tid >> 5;
   const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
   const uint32_t* __restrict__ segB = c.segB;
   const uint32_t gBeg = segB[0], gEnd = segB[S];
@@ -221,7 +226,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     // ================================================================== P1: decode, calibrate, insert
     // The loops over a thread's four words are rolled (the kernel has to fit the instruction cache); the words' state
     // stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is always [0].
-    const bool one_seg = g0 + len <= nextB;
+    const uint32_t fed_split = g0 + len <= nextB ? 0xFFFFFFFFu : nextB;  // words from here on belong to a later FED (rare)
     uint32_t key[NJ];  // K_* below; NOKEY: not decodable
     uint32_t cr[NJ];   // charge | root << 16
     bool fail = false;
@@ -230,7 +235,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t p = tid + NT * j, g = g0 + p;
       const bool valid = p < len;
       uint32_t fed = fed0;
-      if (!one_seg && valid && g >= nextB) {  // a FED boundary inside the item
+      if (g >= fed_split && valid) {  // a FED boundary inside the item
         uint32_t sg = er * F + fed0 + 1u;
         while (sg + 1u < (er + 1u) * F && segB[sg + 1u] <= g) ++sg;
         fed = sg - er * F;
