@@ -3,19 +3,20 @@
 // S13) and a5 sums / charge cut / renumber / temp records (S9, S14, S18) for one work item per block.
 //
 // A work item (runs.cu) is a stretch of at most 1024 raw words holding whole module runs.  A block of 256 threads
-// takes it with four words per thread (word p = tid + 256 j, so every access is coalesced); the word's key, charge
-// and root stay in registers through all phases, only the tables live in shared memory:
+// takes it with four words per thread (word p = tid + 256 j, so every access is coalesced); the word's key, flags,
+// charge and root stay in registers through all phases (the loops over the four words are rolled and the registers
+// turned, ROT4, so that the code fits the instruction cache), only the tables live in shared memory:
 //   P1  decode, calibrate, store module / row / col / charge; run index from the start bits; insert into the
-//       position hash: key = run | row | col -> bucket (10 bits) + tag (15 bits), exact; a bucket holds four 16-bit
-//       tags (one 64-bit load per lookup) plus four more in a second level that is only read when the first is full;
-//       slots are handed out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
-//   P2  duplicates (S10: the lowest word owns the pixel; rare path), then four forward-neighbour lookups per live
-//       pixel and lock-free hook-and-descend unions on the labels (pix_device.cuh)
-//   P3  root of every live pixel; charge | pixel count, charge*col, charge*row added into the root's accumulators
-//   P4  roots: Q >= cut survives (ballot bitmap, block scan), numbered per run in word order; temp records
+//       position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 16-bit
+//       tags (one 64-bit load per lookup) plus a second level (4 entries per 32 buckets) that is only read when the
+//       first is full; slots are handed out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
+//   P2  the word's own bucket (two entries of one pixel: S10, resolved in a rare second pass), four forward-neighbour
+//       lookups per word, edges into a per-warp list, lock-free hook-and-descend unions on the labels (pix_device.cuh)
+//   P3  root of every live pixel; roots start their accumulators (in the memory of the dead hash) and are listed in
+//       word order; the other pixels add charge | pixel count, charge*col, charge*row by shared atomics
+//   P4  one root per thread: Q >= cut survives (ballot bitmap, per-warp scan), numbered per run; temp records
 //   P5  final status and clus, per-run cluster count and temp base, per-event counters
-// Runs are separated by block barriers only (about ten per 1024 words); all warps of a block walk the same code at
-// the same time, and the whole kernel fits the instruction cache.
+// Phases are separated by block barriers (eight per item); five blocks per SM.
 // What the kernel cannot take goes to the block-per-run kernel (cluster.cu): runs longer than 1024 words (decoded
 // here, ITEM_DECODE_ONLY), items whose hash overflows a bucket (8 keys), runs with a cluster charge beyond Q_SAFE.
 // Nothing here is shared with oracle/.
