@@ -69,20 +69,27 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
         g = (g - evb > 32u) ? g - 32u : evb;
       }
     }
-    for (uint32_t ci = c0; ci < c1; ++ci) {
+    auto load_chunk = [&](uint32_t ci) {  // the four words of this lane in chunk ci (0 where there is no word)
       const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
-      const uint32_t cs = c.chunk_seg[ci];
-      const uint32_t er0 = cs >> 16, fed0 = cs & 0xFFFFu, sg0 = er0 * F + fed0;
-      const bool all_in = b >= gBeg && b + HC <= gEnd;
-      const bool one_seg = all_in && b + HC <= segB[sg0 + 1u];
       uint4 wv = make_uint4(0u, 0u, 0u, 0u);
-      if (all_in) wv = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
+      if (b >= gBeg && b + HC <= gEnd) wv = __ldg(reinterpret_cast<const uint4*>(c.words + g0));
       else {
         if (g0 >= gBeg && g0 < gEnd) wv.x = __ldg(c.words + g0);
         if (g0 + 1u >= gBeg && g0 + 1u < gEnd) wv.y = __ldg(c.words + g0 + 1u);
         if (g0 + 2u >= gBeg && g0 + 2u < gEnd) wv.z = __ldg(c.words + g0 + 2u);
         if (g0 + 3u >= gBeg && g0 + 3u < gEnd) wv.w = __ldg(c.words + g0 + 3u);
       }
+      return wv;
+    };
+    uint4 wnext = load_chunk(c0);
+    for (uint32_t ci = c0; ci < c1; ++ci) {
+      const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
+      const uint32_t cs = c.chunk_seg[ci];
+      const uint32_t er0 = cs >> 16, fed0 = cs & 0xFFFFu, sg0 = er0 * F + fed0;
+      const bool all_in = b >= gBeg && b + HC <= gEnd;
+      const bool one_seg = all_in && b + HC <= segB[sg0 + 1u];
+      const uint4 wv = wnext;
+      if (ci + 1u < c1) wnext = load_chunk(ci + 1u);  // in flight while this chunk is worked on
       const uint32_t w[4] = {wv.x, wv.y, wv.z, wv.w};
       uint32_t key[4];
       if (one_seg) {
@@ -302,7 +309,7 @@ __global__ void __launch_bounds__(PACK_WARPS * 32) pack_kernel(const __grid_cons
 void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream) {
   uint64_t nb = ((uint64_t)words_bound + 2 * HC + 8 * RANGE * HC - 1) / (8 * RANGE * HC);  // 8 warps of RANGE chunks per block
   if (nb < 1) nb = 1;
-  if (nb > (uint64_t)n_sm * 16) nb = (uint64_t)n_sm * 16;
+  if (nb > (uint64_t)n_sm * 64) nb = (uint64_t)n_sm * 64;
   runs_kernel<<<(int)nb, 256, 0, stream>>>(c);
   const uint32_t Ec = c.e1 - c.e0;
   pack_kernel<<<(int)((Ec + PACK_WARPS - 1u) / PACK_WARPS), PACK_WARPS * 32, 0, stream>>>(c);
