@@ -2,14 +2,15 @@
 // boundaries come first) as a streaming pre-pass, and the packing of module runs into work items for the tile
 // kernel (tile.cu).  DESIGN.md S11, S12.
 //
-// runs_kernel: one warp per 128 raw words, four consecutive words per lane (one 128-bit load).  A word is decoded as
+// runs_kernel: a warp walks ranges of eight 128-word chunks, four consecutive words per lane (one 128-bit load, the
+// next chunk's load in flight while a chunk is worked on).  A word is decoded as
 // far as its status and module (cabling gather only); a decodable word starts a run when its (event, module) differs
 // from the previous decodable word's.  Output: one start bit per word (bit g - T0 of sbits, T0 = first word of the
 // launch group rounded down to 128), module_first / module_end / the per-module run count (run_start, run_end).
-// The previous decodable word before a chunk is searched backwards, 32 words at a time, never beyond the start of the
+// The previous decodable word before a range is searched backwards, 32 words at a time, never beyond the start of the
 // event (an earlier event's word never continues a run; segfill_kernel closes every event's last run).
 //
-// pack_kernel: one warp per event walks the event's start bits and cuts it into items: maximal stretches of whole
+// pack_kernel: one warp per event walks the event's start bits (staged in shared memory) and cuts it into items: maximal stretches of whole
 // runs of at most ITEM_WIN words (greedy: the next item starts at the last run start inside the window), at most
 // ITEM_RUNS runs each.  A run longer than TILE_WORDS words is cut into equal pieces that the tile kernel only decodes;
 // the first piece carries ITEM_LONG_HEAD and the tile kernel hands the run to the block-per-run kernel (cluster.cu).

@@ -51,7 +51,7 @@ def _noncontiguous_events(det, rng):
     rb, cb, ab = _pixels(rng, 40)
     ev.append((np.r_[np.full(50, a), np.full(40, b), np.full(40, a)], np.r_[ra[:50], rb, ra[50:]],
                np.r_[ca[:50], cb, ca[50:]], np.r_[aa[:50], ab, aa[50:]]))
-    # a run longer than the warp window (300 words), then B, then A again, then a valid module C
+    # a run of 300 words, then B, then A again, then a valid module C
     ra, ca, aa = _pixels(rng, 420)
     rc, cc, ac = _pixels(rng, 70)
     ev.append((np.r_[np.full(300, a), np.full(40, b), np.full(120, a), np.full(70, c)], np.r_[ra[:300], rb, ra[300:], rc],

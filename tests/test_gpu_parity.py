@@ -155,7 +155,8 @@ def _hand_batch(det, events):
 
 def test_run_lengths_across_kernel_tiers(gu, full):
     """Hand-built events: one long run of n words after a filler run of k words, for n around every size at which
-    a run changes hands (findclus window 256 minus the start offset, findrun 512, block kernel's shared tier 1024)
+    something changes for a run (a work item of the tile kernel holds at most 1024 words; runs of 256 words or more count
+    their pixels differently; longer runs go to the block-per-run kernel, whose shared-memory tier ends at 2048 words)
     and k shifting the start inside the 128-word chunk.  Pixels form staircase lines, blobs and isolated pixels so
     that components span many rounds."""
     rng = np.random.default_rng(11)
