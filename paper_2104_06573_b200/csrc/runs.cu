@@ -14,7 +14,8 @@
 // runs of at most ITEM_WIN words (greedy: the next item starts at the last run start inside the window), at most
 // ITEM_RUNS runs each.  A run longer than TILE_WORDS words is cut into equal pieces that the tile kernel only decodes;
 // the first piece carries ITEM_LONG_HEAD and the tile kernel hands the run to the block-per-run kernel (cluster.cu).
-// Any two consecutive items of an event cover more than ITEM_WIN2 words, which bounds the item list.
+// An event is cut at up to seven run starts into pieces that different warps pack (the chain of a piece is short); any
+// two consecutive items of a piece cover more than ITEM_WIN2 words, which bounds the item list.
 // Nothing here is shared with oracle/.
 #include "pix_common.cuh"
 #include "pix_device.cuh"
@@ -167,6 +168,7 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
 // ---- pack_kernel: one warp per event.  The event's start bits are staged in shared memory, BUFW words at a time.
 constexpr uint32_t BUFW = 288, NEED = 34;  // a step looks at the words [s >> 5, (s >> 5) + NEED)
 constexpr int PACK_WARPS = 4;
+constexpr uint32_t PACK_SEGS = 8;  // pieces of an event that are packed by different warps
 
 struct PackWarp {
   uint32_t buf[BUFW];
@@ -245,12 +247,39 @@ __global__ void __launch_bounds__(PACK_WARPS * 32) pack_kernel(const __grid_cons
   const uint32_t nwarp = (gridDim.x * blockDim.x) >> 5;
   Stage st;
   st.sbits = c.sbits; st.buf = pw.buf; st.lane = lane; st.w_end = ((gEnd - T0 + HC - 1u) / HC) * 4u;
-  for (uint32_t er = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; er < Ec; er += nwarp) {
-    const uint32_t evb = segB[er * F], eve = segB[(er + 1u) * F];
-    uint32_t sg = er * F;
-    uint32_t s = evb;
-    uint32_t n_buf = 0u;  // items waiting in pw.items
+  for (uint32_t task = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; task < Ec * PACK_SEGS; task += nwarp) {
+    // An event is cut at PACK_SEGS - 1 run starts (the first one at or after each k/PACK_SEGS of its length) and the
+    // pieces are packed by different warps: the greedy chain of a piece is short, and the seams cost at most one short
+    // item each.
+    const uint32_t er = task / PACK_SEGS, seg = task % PACK_SEGS;
+    const uint32_t evb = segB[er * F], ev_end = segB[(er + 1u) * F];
+    if (evb >= ev_end) continue;
     st.w0 = 0xFFFFFFFFu - BUFW;  // nothing staged
+    auto first_start_from = [&](uint32_t lo, uint32_t limit) {  // first start bit in [lo, limit), or limit (bit indices; lo >= 1)
+      uint32_t p = lo - 1u, nx = NO_INDEX;
+      while (nx == NO_INDEX && p + 1u < limit) {
+        const uint32_t q = (limit - 1u - p > 992u) ? p + 992u : limit - 1u;
+        st.ensure(p >> 5);
+        nx = first_start(st, p, q);
+        p = q;
+      }
+      return nx == NO_INDEX ? limit : nx;
+    };
+    const uint32_t n_ev = ev_end - evb, rb = evb - T0, re = ev_end - T0;
+    const uint32_t q0 = rb + (uint32_t)(((uint64_t)n_ev * seg) / PACK_SEGS), q1 = rb + (uint32_t)(((uint64_t)n_ev * (seg + 1u)) / PACK_SEGS);
+    const uint32_t s_beg = T0 + ((seg == 0u || q0 == rb) ? rb : first_start_from(q0, re));
+    const uint32_t eve = T0 + ((seg + 1u == PACK_SEGS) ? re : (q1 == rb ? rb : first_start_from(q1, re)));  // this piece ends here
+    if (s_beg >= eve) continue;
+    uint32_t sg = er * F;  // FED of the piece's first word: the last FED that begins at or before it
+    for (uint32_t f0 = 0u; f0 < F; f0 += 32u) {
+      const bool in = f0 + lane < F;
+      const uint32_t v = in ? segB[er * F + f0 + lane] : 0xFFFFFFFFu;
+      const uint32_t m = __ballot_sync(FULL, in && v <= s_beg);
+      if (m) sg = er * F + f0 + 31u - (uint32_t)__clz(m);
+      if (m != FULL) break;
+    }
+    uint32_t s = s_beg;
+    uint32_t n_buf = 0u;  // items waiting in pw.items
     auto flush = [&]() {
       __syncwarp();
       uint32_t base = 0u;
@@ -260,8 +289,9 @@ __global__ void __launch_bounds__(PACK_WARPS * 32) pack_kernel(const __grid_cons
       n_buf = 0u;
       __syncwarp();
     };
+    uint32_t sg_end = segB[sg + 1u];  // first word of the next FED (kept in a register: no global load per item)
     auto emit = [&](uint32_t g, uint32_t len, uint32_t flags) {
-      while (sg + 1u < (er + 1u) * F && segB[sg + 1u] <= g) ++sg;
+      while (sg + 1u < (er + 1u) * F && sg_end <= g) { ++sg; sg_end = segB[sg + 1u]; }
       if (lane == 0) pw.items[n_buf] = make_uint4(g, len | (flags << 16), er | ((sg - er * F) << 16), 0u);
       if (++n_buf == 32u) flush();
     };
@@ -313,7 +343,7 @@ void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t st
   if (nb > (uint64_t)n_sm * 64) nb = (uint64_t)n_sm * 64;
   runs_kernel<<<(int)nb, 256, 0, stream>>>(c);
   const uint32_t Ec = c.e1 - c.e0;
-  pack_kernel<<<(int)((Ec + PACK_WARPS - 1u) / PACK_WARPS), PACK_WARPS * 32, 0, stream>>>(c);
+  pack_kernel<<<(int)((Ec * PACK_SEGS + PACK_WARPS - 1u) / PACK_WARPS), PACK_WARPS * 32, 0, stream>>>(c);
 }
 
 }  // namespace pix
