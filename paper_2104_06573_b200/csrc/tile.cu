@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     uint32_t key[NJ];  // K_* below; NOKEY: not decodable
     uint32_t cr[NJ];   // charge | root << 16
     bool fail = false;
-#pragma unroll 1
+#pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, g = g0 + p;
       const bool valid = p < len;
@@ -306,7 +306,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       // edges go to the warp's list, and the list is united with all lanes busy.
       uint32_t* const el = s.edge[warp];
       bool cand = false;  // a pixel of this thread sits in its bucket more than once (S10); K_CAND marks the word
-#pragma unroll 1
+#pragma unroll 1  // the largest loop body stays rolled (measured: unrolling it changes nothing)
       for (int j = 0; j < NJ; ++j) {
         uint32_t ne = 0u;
         {
@@ -362,14 +362,14 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     // ================================================================== P3: roots; sums
     // One pointer-jumping step first (a label only ever moves to an ancestor, so concurrent walkers stay correct).
-#pragma unroll 1
+#pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j;
       const uint32_t l = s.label[p];
       if (l < TILE_WORDS) { const uint32_t ll = s.label[l]; if (ll != l) s.label[p] = ll; }
     }
     __syncwarp();
-#pragma unroll 1
+#pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, kj = key[0], e = cr[0] & 0xFFFFu;
       const bool live = k_live(kj);
@@ -406,7 +406,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       return pos >= 1024u ? n_roots : r;
     };
     uint16_t* const rlist = reinterpret_cast<uint16_t*>(s.edge);  // the roots in word order (the edge lists are dead)
-#pragma unroll 1
+#pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, kj = key[0], e = cr[0] & 0xFFFFu, r = cr[0] >> 16;
       const uint32_t di = __shfl_sync(FULL, rt_pre, j * NWARP + warp) + __popc(__shfl_sync(FULL, rt_bits, j * NWARP + warp) & lt_mask);
@@ -478,7 +478,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     __syncthreads();
     // ================================================================== P5: final status and clus, run outputs, counters
     uint32_t cntA = 0u, cntB = 0u, cntP = 0u;  // dup | below << 16 ; ok | cut << 16 ; roots
-#pragma unroll 1
+#pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t kj = key[0], rt = cr[0] >> 16;
       ROT4(key); ROT4(cr);
