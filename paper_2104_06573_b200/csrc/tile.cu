@@ -36,6 +36,7 @@ namespace {
 #define TILE_BLOCKS 5
 #endif
 constexpr int NT = TILE_NT, NJ = TILE_WORDS / NT, BLOCKS_PER_SM = TILE_BLOCKS, NWARP = NT / 32;
+static_assert(TILE_WORDS == 1024 && NJ == 4, "the kernel is written for 1024-word items and four words per thread (ROT4, the 32-word bitmaps)");
 constexpr uint32_t FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
 constexpr uint32_t NBK = 2 * TILE_WORDS, NBK_LOG2 = TILE_WORDS == 1024 ? 11 : 10, TAG_BITS = 25 - NBK_LOG2, TAG_MASK = (1u << TAG_BITS) - 1u;        // buckets of 4 entries (load 0.5: a bucket is full for 0.2% of the lookups)
 // key: run (8) | row (8) | col (9) = 25 bits.  h = (key << 7) * HMUL mod 2^32: the top 25 bits are key * HMUL mod 2^25,
