@@ -70,7 +70,8 @@ struct __align__(16) TileSmem {
   uint32_t survb[32];                // roots that survive the cut, in root order
   uint32_t rootb[32];                // words that are roots
   uint16_t run_pos[256], run_mod[256];
-  uint8_t run_big[256], run_bad[256];
+  uint8_t run_big[256];
+  uint8_t run_bad[2][256];           // by item parity: the next item's P0 clears the other one while P5 still reads this one
   uint32_t n_runs, wbase, pad[2];
 };
 static_assert(sizeof(TileSmem) <= 233472 / BLOCKS_PER_SM - 1024, "BLOCKS_PER_SM blocks per SM");
@@ -178,6 +179,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
   const uint32_t sb_tags = (uint32_t)__cvta_generic_to_shared(s.tagsA);
   static_assert(offsetof(TileSmem, idsA) == sizeof(uint2) * NBK, "idsA follows tagsA");
 
+  uint32_t par = 0u;
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
     const uint4 item = c.items[it];
     const uint32_t g0 = item.x, len = item.y & 0xFFFFu, iflags = item.y >> 16, er = item.z & 0xFFFFu, fed0 = item.z >> 16;
@@ -198,7 +200,10 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     // the item's stretch of the temp record area, one slot per word: asked for now, needed in P4
     uint32_t wbase_t0 = 0u;
     if (tid == 0 && cluster_it) wbase_t0 = alloc_temp(c, len);
-    __syncthreads();  // the previous item is done with the shared tables
+    // No barrier here: what P0 writes (hash, counters, start bits, the run_bad of this item's parity) is not read by
+    // the previous item's P5, and nothing else is written before the barrier at the end of P0.
+    uint8_t* const rbad = s.run_bad[par];
+    par ^= 1u;
     // ================================================================== P0: clear; start bits of the item
     {
       const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
@@ -206,7 +211,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
 #pragma unroll
       for (int k = 0; k < (int)(sizeof(uint2) * NBK / 16 / NT); ++k) tA[tid + NT * k] = z4;
       if (tid < (NBK / 4 + (NBK >> BB_SHIFT) / 4) / 4) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
-      if (tid < 128) reinterpret_cast<uint32_t*>(s.run_big)[tid] = 0u;  // run_big and run_bad
+      if (tid < 64) reinterpret_cast<uint32_t*>(rbad)[tid] = 0u;
       if (tid < 32) s.survb[tid] = 0u;
       if (warp == 0) {
         const uint32_t rel = g0 - T0, wq = rel >> 5;
@@ -285,6 +290,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     if (!cluster_it) {  // a piece of a run longer than the tile: the block-per-run kernel clusters it
       if ((iflags & ITEM_LONG_HEAD) && tid == 0 && key[0] != NOKEY) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[0]);
+      __syncthreads();  // P1 read the start bits: the next item's P0 rewrites them
       continue;
     }
     if (tid == 0) s.wbase = wbase_t0;
@@ -437,7 +443,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         uint32_t p, run, Q, np;
         load_root(i, p, run, Q, np);
         sv = (int32_t)Q >= c.cut;  // S9: equality keeps (Q < 2^31)
-        if (Q > Q_SAFE) s.run_bad[run] = 1;  // 32-bit weighted sums may have wrapped
+        if (Q > Q_SAFE) rbad[run] = 1;  // 32-bit weighted sums may have wrapped
       }
       const uint32_t bal = __ballot_sync(FULL, sv);
       if (lane == 0) s.survb[i >> 5] = bal;  // the words beyond the roots stay 0 (P0)
@@ -484,7 +490,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t kj = key[0], rt = cr[0] >> 16;
       ROT4(key); ROT4(cr);
       if (kj == NOKEY) continue;
-      if (s.run_bad[k_run(kj)]) continue;
+      if (rbad[k_run(kj)]) continue;
       const uint32_t p = tid + NT * j;
       uint32_t so; int32_t cl = -1;
       if (kj & K_DUP) { so = ST_DUP; cntA += 1u; }
@@ -503,7 +509,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t b0 = rank_before(p0), b1 = rank_before(p1);  // all lanes shuffle together
       if (has) {
         const uint32_t m = s.run_mod[tid];
-        if (s.run_bad[tid]) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, m);
+        if (rbad[tid]) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, m);
         else {
           const size_t mo = (size_t)er * c.M + m;
           c.n_clus[mo] = b1 - b0; c.t_base[mo] = wbase + b0;
