@@ -257,7 +257,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
 // ------------------------------------------------------------------ kernel
 // One block per run, taken from a task list by ticket.  Runs of up to CAP digis keep all their tables in shared
 // memory; longer ones go to the next list (a larger size of this kernel) or, in the last size, use the global
-// workspace.  One size is in use: 256 threads / 2048 digis (88 KB).
+// workspace.  One size is in use: 512 threads / 2048 digis (88 KB).
 constexpr size_t SMEM_PER_DIGI = 8 + 8 + 2 * 4 + 4 * 5;  // sx, sy, 2 hash slots, pos, chg, label, q, npix
 
 __device__ __forceinline__ Tables<uint32_t> carve(unsigned char* base, uint32_t cap) {
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(THREADS) block_kernel(const __grid_constant__ 
   }
 }
 
-constexpr int T_B = 256;
+constexpr int T_B = 512;
 constexpr uint32_t CAP_B = 2048;
 
 }  // namespace
