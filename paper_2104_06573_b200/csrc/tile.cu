@@ -46,7 +46,7 @@ constexpr uint32_t HMUL = 0x9E3779B1u;
 constexpr uint32_t D_E = (1u << 7) * HMUL, D_SW = (511u << 7) * HMUL, D_S = (512u << 7) * HMUL, D_SE = (513u << 7) * HMUL;
 constexpr uint32_t MARK = 0xFFFFFFFDu;               // label of a word that is not a live pixel
 // A word's state word: key (25 bits: run | row | col) and flags.  The hash shifts the flags out (key << 7).
-constexpr uint32_t K_BELOW = 1u << 25, K_DUP = 1u << 26, K_SLOT = 27, K_CAND = 1u << 31;  // K_SLOT: 4 bits, the word's slot in its bucket
+constexpr uint32_t K_BELOW = 1u << 25, K_DUP = 1u << 26, K_SLOT = 27;  // K_SLOT: 4 bits, the word's slot in its bucket
 #define ROT4(a) do { const uint32_t t_ = a[0]; a[0] = a[1]; a[1] = a[2]; a[2] = a[3]; a[3] = t_; } while (0)
 constexpr uint32_t NONE = 0xFFFFu, NO_ID = 0xFFFFu;
 constexpr uint32_t Q_SAFE = 0xFFFFFFFFu / 415u;      // sum(e*col), sum(e*row) fit 32 bits while sum(e) <= Q_SAFE
@@ -237,6 +237,11 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     uint32_t key[NJ];  // K_* below; NOKEY: not decodable
     uint32_t cr[NJ];   // charge | root << 16
     bool fail = false;
+    // Words that are not the first entry of their bucket go to a per-warp list (bucket | slot | tag): only they can be
+    // the later copy of a pixel that appears twice (S10), and after the barrier the list is checked with all lanes busy.
+    uint32_t* const dl = s.edge[warp];  // (the edge lists are not in use yet)
+    uint32_t nd = 0u;
+    bool cand = false;  // some pixel of the item may appear twice
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, g = g0 + p;
@@ -263,7 +268,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t bw = s.bits[j * NWARP + warp];
       const uint32_t r = s.pre[j * NWARP + warp] + __popc(bw & le_mask) - 1u;  // a decodable word lies in a run: r >= 0
       const bool below = e < c.thr;  // S9
-      uint32_t k0 = NOKEY;
+      uint32_t k0 = NOKEY, chk = 0u;
       if (ok) {
         k0 = (r << 17) | (row << 9) | col | (below ? K_BELOW : 0u);
         if ((bw >> lane) & 1u) { s.run_pos[r] = (uint16_t)p; s.run_mod[r] = (uint16_t)m; }
@@ -282,7 +287,14 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
             kk = 4u + (kb < 4u ? kb : 0u);
           }
           k0 |= kk << K_SLOT;
+          if (k >= 1u) chk = b | ((k < 7u ? k : 7u) << 11) | (tag << 14);
         }
+      }
+      {
+        const uint32_t mc = __ballot_sync(FULL, chk != 0u);
+        const uint32_t at = nd + __popc(mc & lt_mask);
+        if (chk != 0u) { if (at < ECAP) dl[at] = chk; else cand = true; }  // a full list: take the exact path
+        nd += __popc(mc);
       }
       s.label[p] = (ok && !below) ? p : MARK;
       key[0] = k0; cr[0] = (uint32_t)e;
@@ -305,14 +317,38 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       s.run_big[tid] = (e1 - s.run_pos[tid] >= BIG_RUN) ? 1 : 0;
     }
     __syncwarp();
-#pragma unroll 1
-    for (int pass = 0; pass < 2; ++pass) {
-      // Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1); col 416..511 and row 160..255
-      // never occur, so no bounds checks.  When S is live, SW and SE are joined to it by their own E edges; when E is
-      // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the
-      // edges go to the warp's list, and the list is united with all lanes busy.
+    // ---- duplicates (S10).  A listed word is a candidate when a slot below its own holds its tag (or when the second
+    // level is involved).  Rare: then every word looks at its own bucket exactly, every entry of a pixel that appears
+    // twice is made to name the lowest word, and the other words become DUPLICATE before anybody looks up.
+    {
+      nd = nd < ECAP ? nd : ECAP;
+      for (uint32_t i0 = 0u; i0 < nd; i0 += 32u) {
+        if (i0 + lane < nd) {
+          const uint32_t e = dl[i0 + lane], k = (e >> 11) & 7u, tag = e >> 14;
+          const uint2 x = s.tagsA[e & (NBK - 1u)];
+          cand |= k >= 4u || (x.x & 0xFFFFu) == tag || (k > 1u && (x.x >> 16) == tag) || (k > 2u && (x.y & 0xFFFFu) == tag);
+        }
+      }
+    }
+    if (__syncthreads_or(cand)) {
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+        const uint32_t kj = key[j];
+        if (kj == NOKEY) continue;
+        const uint32_t h = hash_of(kj), b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
+        const uint2 x = s.tagsA[b];
+        uint32_t nm = __popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww));
+        if (x.y >= 0x10000u) nm += matches_B(s, b, want);
+        if (nm >= 2u && resolve_dup(s, b, want, tid + NT * j, (kj >> K_SLOT) & 15u)) { key[j] = kj | K_DUP; s.label[tid + NT * j] = MARK; }
+      }
+      __syncthreads();
+    }
+    // ---- Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1); col 416..511 and row 160..255
+    // never occur, so no bounds checks.  When S is live, SW and SE are joined to it by their own E edges; when E is
+    // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the edges
+    // go to the warp's list, and the list is united with all lanes busy.
+    {
       uint32_t* const el = s.edge[warp];
-      bool cand = false;  // a pixel of this thread sits in its bucket more than once (S10); K_CAND marks the word
 #pragma unroll 1  // the largest loop body stays rolled (measured: unrolling it changes nothing)
       for (int j = 0; j < NJ; ++j) {
         uint32_t ne = 0u;
@@ -321,13 +357,6 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           const bool live = k_live(kj);
           const uint32_t p = tid + NT * j;
           const uint32_t h = hash_of(kj);
-          if (pass == 0) {  // the word's own bucket: more than one entry with its tag
-            const uint32_t b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
-            const uint2 x = s.tagsA[b];
-            uint32_t nm = __popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww));
-            if (x.y >= 0x10000u && kj != NOKEY) nm += matches_B(s, b, want);  // rare: the first level is full
-            if (nm >= 2u && kj != NOKEY) { cand = true; key[0] = kj | K_CAND; }
-          }
           const uint32_t hn[4] = {h + D_E, h + D_S, h + D_SW, h + D_SE};
           uint32_t nb[4];
           lookup4(s, sb_tags, hn, nb);
@@ -352,21 +381,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         }
         ROT4(key);
       }
-      if (!__syncthreads_or(pass == 0 && cand)) break;
-      // rare: some pixel appears twice.  Name the owner in every entry of the pixel, mark the other words DUPLICATE,
-      // start the labels again and look up once more.
-#pragma unroll 1
-      for (int j = 0; j < NJ; ++j) {
-        const uint32_t kj = key[0];
-        if (kj != NOKEY && (kj & K_CAND)) {
-          const uint32_t h = hash_of(kj);
-          if (resolve_dup(s, bucket_of(h), want_of(h), tid + NT * j, (kj >> K_SLOT) & 15u)) key[0] = kj | K_DUP;
-        }
-        s.label[tid + NT * j] = k_live(key[0]) ? tid + NT * j : MARK;
-        ROT4(key);
-      }
-      __syncthreads();
     }
+    __syncthreads();
     // ================================================================== P3: roots; sums
     // One pointer-jumping step first (a label only ever moves to an ancestor, so concurrent walkers stay correct).
 #pragma unroll
