@@ -10,8 +10,9 @@
 //       position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 16-bit
 //       tags (one 64-bit load per lookup) plus a second level (4 entries per 32 buckets) that is only read when the
 //       first is full; slots are handed out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
-//   P2  the word's own bucket (two entries of one pixel: S10, resolved in a rare second pass), four forward-neighbour
-//       lookups per word, edges into a per-warp list, lock-free hook-and-descend unions on the labels (pix_device.cuh)
+//   P2  duplicates (S10) from the list of words that were not first in their bucket (exact pass only when a candidate
+//       turns up), four forward-neighbour lookups per word, edges into a per-warp list, lock-free hook-and-descend
+//       unions on the labels (pix_device.cuh)
 //   P3  root of every live pixel; roots start their accumulators (in the memory of the dead hash) and are listed in
 //       word order; the other pixels add charge | pixel count, charge*col, charge*row by shared atomics
 //   P4  one root per thread: Q >= cut survives (ballot bitmap, per-warp scan), numbered per run; temp records
