@@ -108,6 +108,28 @@ __device__ __noinline__ uint32_t matches_B(const TileSmem& s, uint32_t b, uint32
   return k;
 }
 
+// Union for items of long runs (long clusters: hook-and-descend walks chains that grow with the cluster).  After
+// Jaiganesh & Burtscher's ECL-CC: find the representatives with intermediate pointer jumping (plain stores are safe
+// here because a label is only ever replaced by an ancestor and only roots are hooked), hook the larger root under
+// the smaller one by compare-and-swap, go on from the winner's parent when the root was taken meanwhile.
+__device__ __forceinline__ uint32_t representative(uint32_t* L, uint32_t v) {
+  uint32_t curr = L[v];
+  if (curr != v) {
+    uint32_t prev = v, next;
+    while (curr > (next = L[curr])) { L[prev] = next; prev = curr; curr = next; }
+  }
+  return curr;
+}
+__device__ __noinline__ void unite_roots(uint32_t* L, uint32_t a, uint32_t b) {
+  uint32_t ra = representative(L, a), rb = representative(L, b);
+  while (ra != rb) {
+    const uint32_t hi = ra > rb ? ra : rb, lo = ra > rb ? rb : ra;
+    const uint32_t old = atomicCAS(L + hi, hi, lo);
+    if (old == hi) break;
+    ra = representative(L, old); rb = lo;
+  }
+}
+
 // Lookup of four pixels at once (the four loads are in flight together).  sb = shared-memory address of tagsA.  The
 // result is the word of the live pixel with hash h[i], or a value >= 0x8000 (no such pixel, or below threshold).
 __device__ __forceinline__ void lookup4(const TileSmem& s, uint32_t sb, const uint32_t (&h)[4], uint32_t (&res)[4]) {
@@ -344,6 +366,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       }
       __syncthreads();
     }
+    const bool long_item = R * 96u < len;  // long runs on average (PU200's inner modules): the other union
     // ---- Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1); col 416..511 and row 160..255
     // never occur, so no bounds checks.  When S is live, SW and SE are joined to it by their own E edges; when E is
     // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the edges
@@ -376,7 +399,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         for (uint32_t i0 = 0u; i0 < ne; i0 += 32u) {  // warp-uniform trip count: the lanes reconverge every iteration
           if (i0 + lane < ne) {
             const uint32_t e = el[i0 + lane];
-            hook(s.label, e & 0xFFFFu, e >> 16);
+            if (long_item) unite_roots(s.label, e & 0xFFFFu, e >> 16); else hook(s.label, e & 0xFFFFu, e >> 16);
           }
           __syncwarp();
         }
