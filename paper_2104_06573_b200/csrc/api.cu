@@ -86,7 +86,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.list_cap = (uint32_t)(Ec * M);
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
-  c.sbits = (uint32_t*)take((W / 32 + 16) * 4);
+  c.sbits = (uint32_t*)take((W / 32 + 64) * 4);  // the tile kernel reads 33 words from an item's first bit on
   c.item_cap = (uint32_t)(W / 64 + 16 * Ec + 64);  // runs.cu: at most W_e / 112 + 2 items per piece of an event, 8 pieces
   c.items = (uint4*)take((size_t)c.item_cap * sizeof(uint4));
   c.n_clus = (uint32_t*)take(Ec * M * 4);
