@@ -4,15 +4,16 @@
 //
 // A work item (runs.cu) is a stretch of at most 1024 raw words holding whole module runs.  A block of 256 threads
 // takes it with four words per thread (word p = tid + 256 j, so every access is coalesced); the word's key, flags,
-// charge and root stay in registers through all phases (the loops over the four words are rolled and the registers
-// turned, ROT4, so that the code fits the instruction cache), only the tables live in shared memory:
+// charge and root stay in registers through all phases (the loop of the neighbour search, the largest body, is rolled
+// and its registers turned, ROT4: fully unrolled the kernel lost 15 % to instruction fetch), only the tables live in
+// shared memory:
 //   P1  decode, calibrate, store module / row / col / charge; run index from the start bits; insert into the
 //       position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 16-bit
 //       tags (one 64-bit load per lookup) plus a second level (4 entries per 32 buckets) that is only read when the
 //       first is full; slots are handed out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
 //   P2  duplicates (S10) from the list of words that were not first in their bucket (exact pass only when a candidate
-//       turns up), four forward-neighbour lookups per word, edges into a per-warp list, lock-free hook-and-descend
-//       unions on the labels (pix_device.cuh)
+//       turns up), four forward-neighbour lookups per word, edges into a per-warp list, lock-free unions on the
+//       labels: hook-and-descend (pix_device.cuh), or by representatives (below) when the item's runs are long
 //   P3  root of every live pixel; roots start their accumulators (in the memory of the dead hash) and are listed in
 //       word order; the other pixels add charge | pixel count, charge*col, charge*row by shared atomics
 //   P4  one root per thread: Q >= cut survives (ballot bitmap, per-warp scan), numbered per run; temp records
@@ -39,7 +40,8 @@ namespace {
 constexpr int NT = TILE_NT, NJ = TILE_WORDS / NT, BLOCKS_PER_SM = TILE_BLOCKS, NWARP = NT / 32;
 static_assert(TILE_WORDS == 1024 && NJ == 4, "the kernel is written for 1024-word items and four words per thread (ROT4, the 32-word bitmaps)");
 constexpr uint32_t FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
-constexpr uint32_t NBK = 2 * TILE_WORDS, NBK_LOG2 = TILE_WORDS == 1024 ? 11 : 10, TAG_BITS = 25 - NBK_LOG2, TAG_MASK = (1u << TAG_BITS) - 1u;        // buckets of 4 entries (load 0.5: a bucket is full for 0.2% of the lookups)
+// buckets of 4 entries, 0.5 keys per bucket: a bucket is full for 0.2 % of the lookups
+constexpr uint32_t NBK = 2 * TILE_WORDS, NBK_LOG2 = 11, TAG_BITS = 25 - NBK_LOG2, TAG_MASK = (1u << TAG_BITS) - 1u;
 // key: run (8) | row (8) | col (9) = 25 bits.  h = (key << 7) * HMUL mod 2^32: the top 25 bits are key * HMUL mod 2^25,
 // a bijection of the key; bucket = top 11 bits, tag = the next 14, so (bucket, tag) names the key exactly, and the hash
 // of a neighbour is h + a constant.
@@ -62,7 +64,7 @@ struct __align__(16) TileSmem {
     struct { uint32_t qn[TILE_WORDS], sx[TILE_WORDS], sy[TILE_WORDS], npx[TILE_WORDS]; } sum;  // after P2: the roots' accumulators
   };
   uint16_t idsA[4 * NBK];    // word of the entry | below_threshold << 15; after P2: lid (local id of a root, or NO_ID)
-  uint32_t tagsB[4 * (NBK >> BB_SHIFT)];  // second level, 4 entries per 32 buckets: tag + 1 | (bucket & 31) << 15 | word << 20 | below << 30
+  uint32_t tagsB[4 * (NBK >> BB_SHIFT)];  // second level, 4 entries per 32 buckets: tag + 1 | (bucket & 31) << 16 | word << 21 | below << 31
   uint32_t cnt[NBK / 4];     // entries per bucket, one byte each
   uint32_t cntB[(NBK >> BB_SHIFT) / 4];  // entries per second-level bucket, one byte each (tagsB is never cleared)
   uint32_t edge[NT / 32][ECAP];  // per warp: the edges its words found, a | b << 16
@@ -254,8 +256,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     __syncthreads();
     // ================================================================== P1: decode, calibrate, insert
-    // The loops over a thread's four words are rolled (the kernel has to fit the instruction cache); the words' state
-    // stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is always [0].
+    // The words' state stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is
+    // always [0]: free in the unrolled loops (register renaming), three moves in the rolled one of P2.
     const uint32_t fed_split = g0 + len <= nextB ? 0xFFFFFFFFu : nextB;  // words from here on belong to a later FED (rare)
     uint32_t key[NJ];  // K_* below; NOKEY: not decodable
     uint32_t cr[NJ];   // charge | root << 16
