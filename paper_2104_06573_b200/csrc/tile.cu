@@ -8,9 +8,10 @@
 // and its registers turned, ROT4: fully unrolled the kernel lost 15 % to instruction fetch), only the tables live in
 // shared memory:
 //   P1  decode, calibrate, store module / row / col / charge; run index from the start bits; insert into the
-//       position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 16-bit
-//       tags (one 64-bit load per lookup) plus a second level (4 entries per 32 buckets) that is only read when the
-//       first is full; slots are handed out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
+//       position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 32-bit
+//       entries tag | below | word (one 128-bit load per lookup; the smallest of the four entry ^ tag is the answer)
+//       plus a second level (4 entries per 32 buckets) that is only read when the first is full; slots are handed
+//       out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
 //   P2  duplicates (S10) from the list of words that were not first in their bucket (exact pass only when a candidate
 //       turns up), four forward-neighbour lookups per word, edges into a per-warp list, lock-free unions on the
 //       labels: hook-and-descend (pix_device.cuh), or by representatives (below) when the item's runs are long
@@ -58,17 +59,21 @@ constexpr uint32_t ECAP = 3 * 32;                    // edges a warp lists befor
 constexpr uint32_t BB_SHIFT = 5, BB_MASK = (1u << BB_SHIFT) - 1u;  // first-level buckets per second-level bucket
 constexpr uint32_t B_KEY = (1u << (16 + BB_SHIFT)) - 1u, B_WORD = 16 + BB_SHIFT, B_BELOW = B_WORD + 10;  // fields of a second-level entry
 
+// A first-level entry: tag << 11 | below_threshold << 10 | word; FREE matches no tag.  x ^ tag_word(h) is below 2048
+// exactly for the entries of the pixel with hash h, and then it is below << 10 | word: the smallest of a bucket's four
+// differences is the lookup's result (live pixel: below 1024).
+constexpr uint32_t FREE = 0xFFFFFFFFu, E_TAG = TAG_MASK << 11, E_BELOW = 1u << 10;
+
 struct __align__(16) TileSmem {
   union {
-    uint2 tagsA[NBK];        // first level: 4 x (tag + 1), 0 = free
+    uint4 ent[NBK];          // first level: four entries per bucket
     struct { uint32_t qn[TILE_WORDS], sx[TILE_WORDS], sy[TILE_WORDS], npx[TILE_WORDS]; } sum;  // after P2: the roots' accumulators
   };
-  uint16_t idsA[4 * NBK];    // word of the entry | below_threshold << 15; after P2: lid (local id of a root, or NO_ID)
   uint32_t tagsB[4 * (NBK >> BB_SHIFT)];  // second level, 4 entries per 32 buckets: tag + 1 | (bucket & 31) << 16 | word << 21 | below << 31
   uint32_t cnt[NBK / 4];     // entries per bucket, one byte each
   uint32_t cntB[(NBK >> BB_SHIFT) / 4];  // entries per second-level bucket, one byte each (tagsB is never cleared)
   uint32_t edge[NT / 32][ECAP];  // per warp: the edges its words found, a | b << 16
-  uint32_t label[TILE_WORDS];
+  uint32_t label[TILE_WORDS];        // after P3: lid, 16 bits each (local id of a root, or NO_ID)
   uint32_t bits[32], pre[32];        // run-start bits of the item, run starts before each word of bits
   uint32_t survb[32];                // roots that survive the cut, in root order
   uint32_t rootb[32];                // words that are roots
@@ -78,16 +83,18 @@ struct __align__(16) TileSmem {
   uint32_t n_runs, wbase, pad[2];
 };
 static_assert(sizeof(TileSmem) <= 233472 / BLOCKS_PER_SM - 1024, "BLOCKS_PER_SM blocks per SM");
-static_assert(sizeof(uint2) * NBK == 4 * 4 * TILE_WORDS, "the accumulators take the place of the first-level tags");
 
 __device__ __forceinline__ uint32_t hash_of(uint32_t key) { return (key << 7) * HMUL; }
 __device__ __forceinline__ bool k_live(uint32_t k) { return (k & (K_BELOW | K_DUP)) == 0u; }  // NOKEY has every bit set
 __device__ __forceinline__ uint32_t k_run(uint32_t k) { return (k >> 17) & 0xFFu; }
 __device__ __forceinline__ uint32_t bucket_of(uint32_t h) { return h >> (32 - NBK_LOG2); }
-__device__ __forceinline__ uint32_t want_of(uint32_t h) { return ((h >> 7) & TAG_MASK) + 1u; }  // 1 .. 16384: bit 15 stays free for zero_half
-__device__ __forceinline__ uint32_t zero_half(uint32_t x, uint32_t ww) {
-  const uint32_t y = x ^ ww;
-  return (y - 0x00010001u) & ~y & 0x80008000u;  // bit 15 / 31 set where a half of x equals the half of ww (the lower set bit is exact)
+__device__ __forceinline__ uint32_t want_of(uint32_t h) { return ((h >> 7) & TAG_MASK) + 1u; }  // the tag in a second-level entry
+__device__ __forceinline__ uint32_t tag_word(uint32_t h) { return (h << 4) & E_TAG; }
+__device__ __forceinline__ uint32_t min4(const uint4& x, uint32_t tw) {
+  return min(min(x.x ^ tw, x.y ^ tw), min(x.z ^ tw, x.w ^ tw));
+}
+__device__ __forceinline__ uint32_t entries_of(const uint4& x, uint32_t tw) {  // how many entries of the bucket belong to the pixel
+  return ((x.x ^ tw) < 2048u ? 1u : 0u) + ((x.y ^ tw) < 2048u ? 1u : 0u) + ((x.z ^ tw) < 2048u ? 1u : 0u) + ((x.w ^ tw) < 2048u ? 1u : 0u);
 }
 __device__ __forceinline__ uint32_t countB(const TileSmem& s, uint32_t bB) {
   const uint32_t n = (s.cntB[bB >> 2] >> ((bB & 3u) * 8u)) & 0xFFu;
@@ -132,45 +139,36 @@ __device__ __noinline__ void unite_roots(uint32_t* L, uint32_t a, uint32_t b) {
   }
 }
 
-// Lookup of four pixels at once (the four loads are in flight together).  sb = shared-memory address of tagsA.  The
-// result is the word of the live pixel with hash h[i], or a value >= 0x8000 (no such pixel, or below threshold).
-__device__ __forceinline__ void lookup4(const TileSmem& s, uint32_t sb, const uint32_t (&h)[4], uint32_t (&res)[4]) {
-  uint32_t ao[4], x0[4], x1[4];
+// Lookup of four pixels at once (the four loads are in flight together).  The result is the word of the live pixel
+// with hash h[i], or a value >= 1024 (no such pixel, or below threshold).
+__device__ __forceinline__ void lookup4(const TileSmem& s, const uint32_t (&h)[4], uint32_t (&res)[4]) {
+  uint4 x[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) x[i] = s.ent[bucket_of(h[i])];
+  bool rare = false;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    ao[i] = sb + ((h[i] >> (32 - NBK_LOG2 - 3)) & ((NBK - 1u) << 3));  // address of the bucket
-    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x0[i]), "=r"(x1[i]) : "r"(ao[i]));
+    res[i] = min4(x[i], tag_word(h[i]));
+    rare |= res[i] >= 2048u && x[i].w != FREE;
   }
-  uint32_t k2[4];
-  bool hit[4];
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const uint32_t ww = ((h[i] >> 7) & TAG_MASK) * 0x00010001u + 0x00010001u;  // tag + 1 in both halves
-    const uint32_t z0 = zero_half(x0[i], ww), z1 = zero_half(x1[i], ww);
-    hit[i] = (z0 | z1) != 0u;
-    k2[i] = z0 ? ((z0 & 0x8000u) ? 0u : 2u) : ((z1 & 0x8000u) ? 4u : 6u);
-    res[i] = 0xFFFFu;
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-    if (hit[i]) asm volatile("ld.shared.u16 %0, [%1+%2];" : "=r"(res[i]) : "r"(ao[i] + k2[i]), "n"(sizeof(uint2) * NBK));  // idsA follows tagsA
-  const uint32_t full = (hit[0] ? 0u : x1[0]) | (hit[1] ? 0u : x1[1]) | (hit[2] ? 0u : x1[2]) | (hit[3] ? 0u : x1[3]);
-  if (full >= 0x10000u) {  // rare: a miss in a bucket whose first level is full (its fourth entry is taken)
+  if (rare) {  // a miss in a bucket whose first level is full
 #pragma unroll
     for (int i = 0; i < 4; ++i)
-      if (!hit[i] && x1[i] >= 0x10000u) res[i] = lookup_B(s, bucket_of(h[i]), want_of(h[i]));
+      if (res[i] >= 2048u && x[i].w != FREE) res[i] = lookup_B(s, bucket_of(h[i]), want_of(h[i]));
   }
 }
 
 // rare: the pixel of word p appears more than once in its bucket.  The lowest word owns it (S10); every entry of the
 // pixel is made to name the owner, so a lookup may take any of them.  Returns true when p is not the owner.
-__device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want, uint32_t p, uint32_t k_own) {
-  const uint16_t* tA = reinterpret_cast<const uint16_t*>(s.tagsA) + b * 4u;
-  const uint32_t bB = b >> BB_SHIFT, nB = tA[3] ? countB(s, bB) : 0u, w19 = want | ((b & BB_MASK) << 16);
+__device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t h, uint32_t p, uint32_t k_own) {
+  uint32_t* const eA = reinterpret_cast<uint32_t*>(s.ent + b);
+  const uint32_t tw = tag_word(h), want = want_of(h);
+  const uint32_t bB = b >> BB_SHIFT, nB = eA[3] != FREE ? countB(s, bB) : 0u, w19 = want | ((b & BB_MASK) << 16);
   uint32_t best = 0xFFFFFFFFu;  // word << 1 | below
   for (uint32_t i = 0; i < 4u; ++i) {
-    if (tA[i] != want) continue;
-    const uint32_t idv = s.idsA[b * 4u + i], v = ((idv & 0x3FFu) << 1) | (idv >> 15);
+    const uint32_t d = eA[i] ^ tw;
+    if (d >= 2048u) continue;
+    const uint32_t v = ((d & 0x3FFu) << 1) | (d >> 10);
     best = v < best ? v : best;
   }
   for (uint32_t i = 0; i < nB; ++i) {
@@ -180,7 +178,7 @@ __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t want,
     best = v < best ? v : best;
   }
   if ((best >> 1) == p) return false;
-  if (k_own < 4u) s.idsA[b * 4u + k_own] = (uint16_t)((best >> 1) | ((best & 1u) << 15));
+  if (k_own < 4u) eA[k_own] = tw | (best >> 1) | ((best & 1u) ? E_BELOW : 0u);
   else s.tagsB[bB * 4u + k_own - 4u] = w19 | ((best >> 1) << B_WORD) | ((best & 1u) << B_BELOW);
   return true;
 }
@@ -199,10 +197,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
   uint32_t n_items = c.ctl[CTL_ITEM_COUNT];
   n_items = n_items < c.item_cap ? n_items : c.item_cap;
   const uint32_t lt_mask = (1u << lane) - 1u, le_mask = lt_mask | (1u << lane);
-  uint16_t* const tagA16 = reinterpret_cast<uint16_t*>(s.tagsA);
-  uint16_t* const lid = s.idsA;
-  const uint32_t sb_tags = (uint32_t)__cvta_generic_to_shared(s.tagsA);
-  static_assert(offsetof(TileSmem, idsA) == sizeof(uint2) * NBK, "idsA follows tagsA");
+  uint32_t* const ent32 = reinterpret_cast<uint32_t*>(s.ent);
+  uint16_t* const lid = reinterpret_cast<uint16_t*>(s.label);  // not in the hash: the next item's P0 clears that while P5 still reads lid
 
   uint32_t par = 0u;
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
@@ -231,10 +227,9 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     par ^= 1u;
     // ================================================================== P0: clear; start bits of the item
     {
-      const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
-      uint4* tA = reinterpret_cast<uint4*>(s.tagsA);
+      const uint4 z4 = make_uint4(0u, 0u, 0u, 0u), f4 = make_uint4(FREE, FREE, FREE, FREE);
 #pragma unroll
-      for (int k = 0; k < (int)(sizeof(uint2) * NBK / 16 / NT); ++k) tA[tid + NT * k] = z4;
+      for (int k = 0; k < (int)(NBK / NT); ++k) s.ent[tid + NT * k] = f4;
       if (tid < (NBK / 4 + (NBK >> BB_SHIFT) / 4) / 4) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
       if (tid < 64) reinterpret_cast<uint32_t*>(rbad)[tid] = 0u;
       if (tid < 32) s.survb[tid] = 0u;
@@ -301,9 +296,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           const uint32_t h = hash_of(k0), b = bucket_of(h), sh8 = (b & 3u) * 8u;
           const uint32_t k = (atomicAdd(&s.cnt[b >> 2], 1u << sh8) >> sh8) & 0xFFu;
           const uint32_t tag = want_of(h);
-          const uint16_t idv = (uint16_t)(p | (below ? 0x8000u : 0u));
           uint32_t kk = k;
-          if (k < 4u) { tagA16[b * 4u + k] = (uint16_t)tag; s.idsA[b * 4u + k] = idv; }
+          if (k < 4u) ent32[b * 4u + k] = tag_word(h) | (below ? E_BELOW : 0u) | p;
           else {  // rare: the bucket's first level is full
             const uint32_t bB = b >> BB_SHIFT, shB = (bB & 3u) * 8u;
             const uint32_t kb = (atomicAdd(&s.cntB[bB >> 2], 1u << shB) >> shB) & 0xFFu;
@@ -350,8 +344,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       for (uint32_t i0 = 0u; i0 < nd; i0 += 32u) {
         if (i0 + lane < nd) {
           const uint32_t e = dl[i0 + lane], k = (e >> 11) & 7u, tag = e >> 14;
-          const uint2 x = s.tagsA[e & (NBK - 1u)];
-          cand |= k >= 4u || (x.x & 0xFFFFu) == tag || (k > 1u && (x.x >> 16) == tag) || (k > 2u && (x.y & 0xFFFFu) == tag);
+          cand |= k >= 4u || entries_of(s.ent[e & (NBK - 1u)], (tag - 1u) << 11) >= 2u;
         }
       }
     }
@@ -360,11 +353,11 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       for (int j = 0; j < NJ; ++j) {
         const uint32_t kj = key[j];
         if (kj == NOKEY) continue;
-        const uint32_t h = hash_of(kj), b = bucket_of(h), want = want_of(h), ww = want * 0x00010001u;
-        const uint2 x = s.tagsA[b];
-        uint32_t nm = __popc(zero_half(x.x, ww)) + __popc(zero_half(x.y, ww));
-        if (x.y >= 0x10000u) nm += matches_B(s, b, want);
-        if (nm >= 2u && resolve_dup(s, b, want, tid + NT * j, (kj >> K_SLOT) & 15u)) { key[j] = kj | K_DUP; s.label[tid + NT * j] = MARK; }
+        const uint32_t h = hash_of(kj), b = bucket_of(h);
+        const uint4 x = s.ent[b];
+        uint32_t nm = entries_of(x, tag_word(h));
+        if (x.w != FREE) nm += matches_B(s, b, want_of(h));
+        if (nm >= 2u && resolve_dup(s, b, h, tid + NT * j, (kj >> K_SLOT) & 15u)) { key[j] = kj | K_DUP; s.label[tid + NT * j] = MARK; }
       }
       __syncthreads();
     }
@@ -385,10 +378,10 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           const uint32_t h = hash_of(kj);
           const uint32_t hn[4] = {h + D_E, h + D_S, h + D_SW, h + D_SE};
           uint32_t nb[4];
-          lookup4(s, sb_tags, hn, nb);
-          const uint32_t nE = nb[0], nS = nb[1], nSW = nb[2], nSE = nb[3];  // >= 0x8000: no live pixel there
-          const uint32_t t1 = nS < 0x8000u ? nS : nSW;
-          const bool f0 = live && nE < 0x8000u, f1 = live && t1 < 0x8000u, f2 = live && nS >= 0x8000u && nE >= 0x8000u && nSE < 0x8000u;
+          lookup4(s, hn, nb);
+          const uint32_t nE = nb[0], nS = nb[1], nSW = nb[2], nSE = nb[3];  // >= 1024: no live pixel there
+          const uint32_t t1 = nS < 1024u ? nS : nSW;
+          const bool f0 = live && nE < 1024u, f1 = live && t1 < 1024u, f2 = live && nS >= 1024u && nE >= 1024u && nSE < 1024u;
           const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
           if (f0) el[ne + __popc(m0 & lt_mask)] = p | (nE << 16);
           ne += __popc(m0);
