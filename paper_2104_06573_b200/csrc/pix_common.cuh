@@ -37,7 +37,7 @@ constexpr uint32_t CHUNK_WORDS = 128;  // words per warp in decode and findclus;
 enum { EC_EMPTY = 0, EC_ERR_LINK, EC_ERR_ROC, EC_ERR_DCOL, EC_ERR_PXID, EC_FLAGS, EC_DUP, EC_BELOW, EC_OK, EC_CUT,
        EC_PRECUT, EC_PUSHED /* runs the event has put on the task lists (at most M) */, EC_STRIDE = 16 };
 // ctl words
-enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_TEMP_COUNT = 8, CTL_ITEM_COUNT = 9, CTL_WORDS = 16 };
+enum { CTL_OVF_COUNT = 0, CTL_OVF_TICKET = 1, CTL_SLICE_COUNT = 2, CTL_TEMP_COUNT = 8, CTL_ITEM_COUNT = 9, CTL_ITEM_NEXT = 10, CTL_WORDS = 16 };
 // work items of the tile kernel (runs.cu packs them, tile.cu takes them): x = global index of the first word,
 // y = words | flags << 16, z = event (launch-group relative) | FED of the first word << 16
 #ifndef PIX_TILE_WORDS

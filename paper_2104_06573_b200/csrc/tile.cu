@@ -80,7 +80,7 @@ struct __align__(16) TileSmem {
   uint16_t run_pos[256], run_mod[256];
   uint8_t run_big[256];
   uint8_t run_bad[2][256];           // by item parity: the next item's P0 clears the other one while P5 still reads this one
-  uint32_t n_runs, wbase, pad[2];
+  uint32_t n_runs, wbase, next_item, pad[1];
 };
 static_assert(sizeof(TileSmem) <= 233472 / BLOCKS_PER_SM - 1024, "BLOCKS_PER_SM blocks per SM");
 
@@ -201,7 +201,12 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
   uint16_t* const lid = reinterpret_cast<uint16_t*>(s.label);  // not in the hash: the next item's P0 clears that while P5 still reads lid
 
   uint32_t par = 0u;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+  uint32_t nxt;
+  for (uint32_t it = blockIdx.x; it < n_items; it = nxt) {
+    // The block's first item is its own index, the others come from a counter: asked for now, handed to the block with
+    // the barrier after P1 (blocks that drew cheap items go on drawing, so the grid ends together).
+    uint32_t nxt_t0 = 0u;
+    if (tid == 0) nxt_t0 = gridDim.x + atomicAdd(c.ctl + CTL_ITEM_NEXT, 1u);
     const uint4 item = c.items[it];
     const uint32_t g0 = item.x, len = item.y & 0xFFFFu, iflags = item.y >> 16, er = item.z & 0xFFFFu, fed0 = item.z >> 16;
     const bool cluster_it = !(iflags & ITEM_DECODE_ONLY);
@@ -213,11 +218,6 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     const uint32_t ebase = segB[er * F];
     const uint32_t nextB = segB[er * F + fed0 + 1u];        // first word of the next FED
-    if (it + gridDim.x < n_items) {  // the next item of this block: its words on their way into L2 / L1 while this one is clustered
-      const uint4 nx = c.items[it + gridDim.x];
-      const uint32_t* q = c.words + nx.x + 32u * tid;  // one 128-byte line per thread covers up to 8192 words
-      if (32u * tid < (nx.y & 0xFFFFu)) asm volatile("prefetch.global.L2 [%0];" :: "l"(q));
-    }
     // the item's stretch of the temp record area, one slot per word: asked for now, needed in P4
     uint32_t wbase_t0 = 0u;
     if (tid == 0 && cluster_it) wbase_t0 = alloc_temp(c, len);
@@ -321,14 +321,23 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     }
     if (!cluster_it) {  // a piece of a run longer than the tile: the block-per-run kernel clusters it
       if ((iflags & ITEM_LONG_HEAD) && tid == 0 && key[0] != NOKEY) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[0]);
+      if (tid == 0) s.next_item = nxt_t0;
       __syncthreads();  // P1 read the start bits: the next item's P0 rewrites them
+      nxt = s.next_item;
       continue;
     }
-    if (tid == 0) s.wbase = wbase_t0;
+    if (tid == 0) { s.wbase = wbase_t0; s.next_item = nxt_t0; }
     const uint32_t R = s.n_runs;
-    if (__syncthreads_or(fail)) {  // a bucket with more than 8 keys: the block-per-run kernel takes the runs of the item
+    const bool failed = __syncthreads_or(fail);
+    nxt = s.next_item;
+    if (failed) {  // a bucket with more than 8 keys: the block-per-run kernel takes the runs of the item
       if (tid < R) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[tid]);
       continue;
+    }
+    if (nxt < n_items) {  // the next item: its words on their way into L2 while this one is clustered
+      const uint4 nx = c.items[nxt];
+      const uint32_t* q = c.words + nx.x + 32u * tid;  // one 128-byte line per thread covers up to 8192 words
+      if (32u * tid < (nx.y & 0xFFFFu)) asm volatile("prefetch.global.L2 [%0];" :: "l"(q));
     }
     // ================================================================== P2: neighbours -> edges -> unions; duplicates
     if (tid < R) {
