@@ -34,7 +34,7 @@ __device__ __forceinline__ uint32_t run_key(const CabEntry* __restrict__ cab, ui
   return ok ? ((er << 16) | (ex & 0xFFFFu)) : NOKEY;
 }
 
-__global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk c) {
+__global__ void __launch_bounds__(256, 8) runs_kernel(const __grid_constant__ Chunk c) {
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
   const uint32_t* __restrict__ segB = c.segB;
@@ -112,24 +112,43 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
         }
       }
       // a word starts a run when its (event, module) differs from the previous decodable word's
-      uint32_t tkey = NOKEY, tj = 0u;  // the lane's last decodable word
-#pragma unroll
-      for (int j = 0; j < 4; ++j) if (key[j] != NOKEY) { tkey = key[j]; tj = j; }
-      const uint32_t has = __ballot_sync(FULL, tkey != NOKEY);
-      const uint32_t below_l = has & lt_mask;
-      const int src = below_l ? 31 - __clz(below_l) : 0;
-      uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = b + 4u * (uint32_t)src + __shfl_sync(FULL, tj, src);
-      if (!below_l) { pkey = carry_key; pg = carry_g; }
       uint32_t startmask = 0u;
       uint32_t s_key = NOKEY, s_g = 0u, s_pkey = NOKEY, s_pg = 0u;  // the lane's first run start and its predecessor
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        if (key[j] == NOKEY) continue;
-        if (key[j] != pkey) {
-          if (!startmask) { s_key = key[j]; s_g = g0 + j; s_pkey = pkey; s_pg = pg; }
-          startmask |= 1u << j;
+      const uint32_t kmax = max(max(key[0], key[1]), max(key[2], key[3]));
+      if (__all_sync(FULL, kmax != NOKEY)) {  // the usual chunk: every word decodable, the previous word is the neighbour
+        uint32_t pkey = __shfl_up_sync(FULL, key[3], 1), pg = g0 - 1u;
+        if (lane == 0) { pkey = carry_key; pg = carry_g; }
+        startmask = (key[0] != pkey ? 1u : 0u) | (key[1] != key[0] ? 2u : 0u) | (key[2] != key[1] ? 4u : 0u) | (key[3] != key[2] ? 8u : 0u);
+        if (startmask) {
+          const uint32_t j0 = (uint32_t)__ffs((int)startmask) - 1u;
+          s_key = j0 == 0u ? key[0] : j0 == 1u ? key[1] : j0 == 2u ? key[2] : key[3];
+          s_pkey = j0 == 0u ? pkey : j0 == 1u ? key[0] : j0 == 2u ? key[1] : key[2];
+          s_g = g0 + j0;
+          s_pg = j0 == 0u ? pg : s_g - 1u;
         }
-        pkey = key[j]; pg = g0 + j;
+        carry_key = __shfl_sync(FULL, key[3], 31); carry_g = b + HC - 1u;
+      } else {
+        uint32_t tkey = NOKEY, tj = 0u;  // the lane's last decodable word
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (key[j] != NOKEY) { tkey = key[j]; tj = j; }
+        const uint32_t has = __ballot_sync(FULL, tkey != NOKEY);
+        const uint32_t below_l = has & lt_mask;
+        const int src = below_l ? 31 - __clz(below_l) : 0;
+        uint32_t pkey = __shfl_sync(FULL, tkey, src), pg = b + 4u * (uint32_t)src + __shfl_sync(FULL, tj, src);
+        if (!below_l) { pkey = carry_key; pg = carry_g; }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (key[j] == NOKEY) continue;
+          if (key[j] != pkey) {
+            if (!startmask) { s_key = key[j]; s_g = g0 + j; s_pkey = pkey; s_pg = pg; }
+            startmask |= 1u << j;
+          }
+          pkey = key[j]; pg = g0 + j;
+        }
+        if (has) {
+          const int top = 31 - __clz(has);
+          carry_key = __shfl_sync(FULL, tkey, top); carry_g = b + 4u * (uint32_t)top + __shfl_sync(FULL, tj, top);
+        }
       }
       if (s_key != NOKEY) {  // one copy of the atomics for the usual case of at most one start per lane
         run_start(c, s_key, s_g);
@@ -150,17 +169,13 @@ __global__ void __launch_bounds__(256) runs_kernel(const __grid_constant__ Chunk
           pk = kj; pgg = g0 + j;
         }
       }
-      if (has) {
-        const int top = 31 - __clz(has);
-        carry_key = __shfl_sync(FULL, tkey, top); carry_g = b + 4u * (uint32_t)top + __shfl_sync(FULL, tj, top);
-      }
       // start bits of the chunk: lane l's nibble sits at bit 4 l of the 128-bit row
-      const uint32_t nib = startmask << (4u * (lane & 7u));
-#pragma unroll
-      for (uint32_t k = 0; k < 4u; ++k) {
-        const uint32_t v = __reduce_or_sync(FULL, (lane >> 3) == k ? nib : 0u);
-        if (lane == k) c.sbits[ci * 4u + k] = v;
-      }
+      // (three folding shuffles: lanes 0, 8, 16, 24 end up with the words of their eight lanes)
+      uint32_t v = startmask;
+      v |= __shfl_down_sync(FULL, v, 1) << 4;
+      v |= __shfl_down_sync(FULL, v, 2) << 8;
+      v |= __shfl_down_sync(FULL, v, 4) << 16;
+      if ((lane & 7u) == 0u) c.sbits[ci * 4u + (lane >> 3)] = v;
     }
   }
 }
