@@ -5,8 +5,10 @@
 // runs_kernel: a warp walks ranges of eight 128-word chunks, four consecutive words per lane (one 128-bit load, the
 // next chunk's load in flight while a chunk is worked on).  A word is decoded as
 // far as its status and module (cabling gather only); a decodable word starts a run when its (event, module) differs
-// from the previous decodable word's.  Output: one start bit per word (bit g - T0 of sbits, T0 = first word of the
-// launch group rounded down to 128), module_first / module_end / the per-module run count (run_start, run_end).
+// from the previous decodable word's (when all 128 words of the chunk are decodable, the usual case, that is the
+// word before it: one shuffle; otherwise a ballot / find-last-set scan).  Output: one start bit per word (bit g - T0
+// of sbits, T0 = first word of the launch group rounded down to 128; the lanes' nibbles are folded into four words by
+// three shuffles), module_first / module_end / the per-module run count (run_start, run_end).
 // The previous decodable word before a range is searched backwards, 32 words at a time, never beyond the start of the
 // event (an earlier event's word never continues a run; segfill_kernel closes every event's last run).
 //
