@@ -19,7 +19,8 @@
 //       word order; the other pixels add charge | pixel count, charge*col, charge*row by shared atomics
 //   P4  one root per thread: Q >= cut survives (ballot bitmap, per-warp scan), numbered per run; temp records
 //   P5  final status and clus, per-run cluster count and temp base, per-event counters
-// Phases are separated by block barriers (seven per item); five blocks per SM.
+// Phases are separated by block barriers (seven per item); five blocks per SM; a block's first item is its own index,
+// the following ones come from a counter (so that the blocks of the grid end together).
 // What the kernel cannot take goes to the block-per-run kernel (cluster.cu): runs longer than 1024 words (decoded
 // here, ITEM_DECODE_ONLY), items whose hash overflows a bucket (8 keys), runs with a cluster charge beyond Q_SAFE.
 // Nothing here is shared with oracle/.
