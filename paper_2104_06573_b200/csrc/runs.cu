@@ -2,8 +2,9 @@
 // boundaries come first) as a streaming pre-pass, and the packing of module runs into work items for the tile
 // kernel (tile.cu).  DESIGN.md S11, S12.
 //
-// runs_kernel: a warp walks ranges of eight 128-word chunks, four consecutive words per lane (one 128-bit load, the
-// next chunk's load in flight while a chunk is worked on).  A word is decoded as
+// runs_kernel: a warp walks ranges of sixteen 128-word chunks, two chunks at a time with eight consecutive words per
+// lane (two 128-bit loads, the next pair's loads in flight meanwhile) while they lie in one (event, FED) segment and
+// every word is decodable, else one chunk with four words per lane.  A word is decoded as
 // far as its status and module (cabling gather only); a decodable word starts a run when its (event, module) differs
 // from the previous decodable word's (when all 128 words of the chunk are decodable, the usual case, that is the
 // word before it: one shuffle; otherwise a ballot / find-last-set scan).  Output: one start bit per word (bit g - T0
@@ -27,7 +28,7 @@ namespace pix {
 namespace {
 
 constexpr uint32_t HC = CHUNK_WORDS, FULL = 0xFFFFFFFFu, NOKEY = 0xFFFFFFFFu;
-constexpr uint32_t RANGE = 8;  // chunks a warp walks in one go (the look-back is done once per range)
+constexpr uint32_t RANGE = 16;  // chunks a warp walks in one go (the look-back is done once per range)
 
 // (event, module) of a decodable word, NOKEY otherwise (S4-S6: the same checks as decode_word, without the position)
 __device__ __forceinline__ uint32_t run_key(const CabEntry* __restrict__ cab, uint32_t w, uint32_t fedbase, uint32_t er) {
@@ -36,7 +37,7 @@ __device__ __forceinline__ uint32_t run_key(const CabEntry* __restrict__ cab, ui
   return ok ? ((er << 16) | (ex & 0xFFFFu)) : NOKEY;
 }
 
-__global__ void __launch_bounds__(256, 8) runs_kernel(const __grid_constant__ Chunk c) {
+__global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Chunk c) {
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
   const uint32_t* __restrict__ segB = c.segB;
@@ -85,15 +86,66 @@ __global__ void __launch_bounds__(256, 8) runs_kernel(const __grid_constant__ Ch
       }
       return wv;
     };
-    uint4 wnext = load_chunk(c0);
+    // Two chunks at a time, eight consecutive words per lane, while they lie inside one (event, FED) segment and every
+    // word is decodable (nearly always); the words of the next pair are in flight meanwhile.  Otherwise one chunk.
+    bool pre = false;
+    uint4 pa = make_uint4(0u, 0u, 0u, 0u), pb = pa;
     for (uint32_t ci = c0; ci < c1; ++ci) {
       const uint32_t b = T0 + ci * HC, g0 = b + 4u * lane;
       const uint32_t cs = c.chunk_seg[ci];
       const uint32_t er0 = cs >> 16, fed0 = cs & 0xFFFFu, sg0 = er0 * F + fed0;
+      const uint32_t seg_end = segB[sg0 + 1u];
+      if (ci + 1u < c1 && b >= gBeg && b + 2u * HC <= gEnd && b + 2u * HC <= seg_end) {
+        const uint4* wp = reinterpret_cast<const uint4*>(c.words + b + 8u * lane);
+        const uint4 wa = pre ? pa : __ldg(wp), wb = pre ? pb : __ldg(wp + 1);
+        pre = ci + 3u < c1 && b + 4u * HC <= gEnd;
+        if (pre) { pa = __ldg(wp + 64); pb = __ldg(wp + 65); }  // the pair after this one (2 x 128 words = 64 uint4 on)
+        const uint32_t w8[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+        uint32_t k[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) k[i] = run_key(c.cab, w8[i], fed0 << 11, er0);
+        const uint32_t kmx = max(max(max(k[0], k[1]), max(k[2], k[3])), max(max(k[4], k[5]), max(k[6], k[7])));
+        if (__all_sync(FULL, kmx != NOKEY)) {
+          const uint32_t g8 = b + 8u * lane;
+          uint32_t pkey = __shfl_up_sync(FULL, k[7], 1), pg = g8 - 1u;
+          if (lane == 0) { pkey = carry_key; pg = carry_g; }
+          uint32_t sm = k[0] != pkey ? 1u : 0u;
+#pragma unroll
+          for (int i = 1; i < 8; ++i) sm |= k[i] != k[i - 1] ? 1u << i : 0u;
+          if (sm) {  // (one copy of the atomics for the usual case of one start per lane)
+            const uint32_t j0 = (uint32_t)__ffs((int)sm) - 1u;
+            uint32_t sk = k[0], sp = pkey;
+#pragma unroll
+            for (int i = 1; i < 8; ++i) if (j0 == (uint32_t)i) { sk = k[i]; sp = k[i - 1]; }
+            run_start(c, sk, g8 + j0);
+            if (sp != NOKEY) run_end(c, sp, j0 ? g8 + j0 - 1u : pg);
+            if (sm & (sm - 1u)) {  // rare: more runs start inside the lane's eight words
+              uint32_t pk = NOKEY;
+#pragma unroll 1
+              for (uint32_t i = 0; i < 8u; ++i) {
+                const uint32_t ki = k[0];
+#pragma unroll
+                for (int t = 0; t < 7; ++t) k[t] = k[t + 1];
+                k[7] = ki;  // rotate: ki is word i's key
+                if (i > j0 && ((sm >> i) & 1u)) { run_start(c, ki, g8 + i); run_end(c, pk, g8 + i - 1u); }
+                pk = ki;
+              }
+            }
+          }
+          carry_key = __shfl_sync(FULL, k[7], 31); carry_g = b + 2u * HC - 1u;
+          // start bits: lane l's byte sits at bit 8 l of the 256-bit row; lanes 0, 4, 8 ... end up with the eight words
+          uint32_t v = sm;
+          v |= __shfl_down_sync(FULL, v, 1) << 8;
+          v |= __shfl_down_sync(FULL, v, 2) << 16;
+          if ((lane & 3u) == 0u) c.sbits[ci * 4u + (lane >> 2)] = v;
+          ++ci;  // two chunks done
+          continue;
+        }
+      }
+      pre = false;
       const bool all_in = b >= gBeg && b + HC <= gEnd;
-      const bool one_seg = all_in && b + HC <= segB[sg0 + 1u];
-      const uint4 wv = wnext;
-      if (ci + 1u < c1) wnext = load_chunk(ci + 1u);  // in flight while this chunk is worked on
+      const bool one_seg = all_in && b + HC <= seg_end;
+      const uint4 wv = load_chunk(ci);
       const uint32_t w[4] = {wv.x, wv.y, wv.z, wv.w};
       uint32_t key[4];
       if (one_seg) {
