@@ -194,6 +194,29 @@ def test_random_recipes(gu, full):
     check(gu, full, b, chunk_events=int(rng.integers(3, 9)))
 
 
+def test_prepass_chunk_and_pair_boundaries(gu, full):
+    """The run-start pre-pass (runs.cu) works on 128-word chunks, two at a time when a pair lies inside one (event, FED)
+    segment and holds decodable words only.  Events of many small sizes put event and FED boundaries at every
+    alignment; all-zero words (EMPTY, transparent to runs) and words with an impossible double column are written at
+    and next to chunk and pair boundaries, so that pairs, single chunks and the scan over undecodable words meet in
+    every order.  One launch group and ragged ones."""
+    rng = np.random.default_rng(77)
+    recipes = [dict(n_clusters=int(rng.integers(3, 900)), inner_modules=int(rng.choice([0, 16])), inner_weight=4,
+                    long_permille=int(rng.choice([0, 20])), shuffle_order=int(rng.integers(0, 2)), edge_class=0)
+               for _ in range(48)]
+    b = pixgen.events(full, recipes, 7700 + np.arange(len(recipes)))
+    words = b.words.copy()
+    n = len(words)
+    for base in range(0, n - 600, 512 * int(rng.integers(1, 4))):
+        for off in (0, 1, 126, 127, 128, 129, 255, 256, 257, 383, 384):
+            if rng.random() < 0.35:
+                g = base + off
+                words[g] = 0 if rng.random() < 0.5 else (words[g] & ~np.uint32(31 << 16)) | np.uint32(int(rng.integers(26, 32)) << 16)
+    b2 = pixgen.Batch(words, b.event_offsets, b.fed_offsets, b.tally)
+    check(gu, full, b2)
+    check(gu, full, b2, chunk_events=7)
+
+
 def test_rechits_lite(gu, full):
     """pix_rechits (S25-S28) against the oracle's rechits on PU50, edge, duplicate, dense and PU200 events:
     boxes and flags bit-exact, local positions within 1e-5 relative (they inherit the centroid's tolerance)."""
