@@ -87,6 +87,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
   c.sbits = (uint32_t*)take((W / 32 + 64) * 4);  // the tile kernel reads 33 words from an item's first bit on
+  c.cbad = (uint8_t*)take(W / 128 + 2);
   c.item_cap = (uint32_t)(W / 64 + 16 * Ec + 64);  // runs.cu: at most W_e / 112 + 2 items per piece of an event, 8 pieces
   c.items = (uint4*)take((size_t)c.item_cap * sizeof(uint4));
   c.n_clus = (uint32_t*)take(Ec * M * 4);
@@ -212,10 +213,18 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   for (size_t i = 0; i < ngp; ++i) gp[i] = make_float2(gains->gain[i], gains->pedestal[i]);
   // cabling re-laid out so that a decode is one 8-byte gather and two multiply-adds (pix_common.cuh; reading S3)
   std::vector<pix::CabEntry> cab(ncab);
+  // Words of a run that ascend strictly in (link, roc, dcol, pxid) are different pixels (the tile kernel then skips its
+  // search for duplicates) unless two valid entries of the table name the same ROC position of a module.
+  std::vector<unsigned char> roc_seen((size_t)M * 16, 0);
+  bool geom_unique = true;
   for (size_t i = 0; i < ncab; ++i) {
     const uint32_t e = cabling->entry[i];
     const uint32_t bad = !(e & 1u) ? PIX_ST_ERR_LINK : (!(e & 2u) ? PIX_ST_ERR_ROC : 0u);
     const uint32_t rocx = (e >> 18) & 7u, rocy = (e >> 21) & 1u, flip_r = (e >> 22) & 1u, flip_c = (e >> 23) & 1u;
+    if (!bad) {
+      const size_t pos = (size_t)((e >> 2) & 0xFFFFu) * 16 + rocy * 8 + rocx;
+      if (pos >= roc_seen.size() || roc_seen[pos]) geom_unique = false; else roc_seen[pos] = 1;
+    }
     const uint32_t row0 = rocy * 80u + (flip_r ? 79u : 0u), col0 = rocx * 52u + (flip_c ? 51u : 0u);
     cab[i].x = ((e >> 2) & 0xFFFFu) | (bad << 16) | ((flip_c ? 0xFFu : 0x01u) << 24);
     cab[i].y = row0 | (col0 << 8) | ((flip_r ? 0xFFu : 0x01u) << 24);
@@ -226,7 +235,7 @@ int pix_create(const pix_cabling_map* cabling, const pix_gain_table* gains, cons
   if (!ok) { cudaGetLastError(); release_tables(t); delete h; return PIX_ERR_ALLOC; }
 
   pix::Chunk& c = h->proto;
-  c.F = F; c.M = M; c.cab = t->cab; c.gp = t->gp;
+  c.F = F; c.M = M; c.cab = t->cab; c.gp = t->gp; c.geom_unique = geom_unique ? 1u : 0u;
   c.F_shift = 0xFFFFFFFFu;
   for (uint32_t sh = 0; sh < 17; ++sh) if ((1u << sh) == F) c.F_shift = sh;
   c.vcal_gain = params->vcal_gain; c.vcal_offset = params->vcal_offset; c.max_e_f = (float)params->max_electrons;

@@ -86,6 +86,9 @@ struct Chunk {
   uint32_t* chunk_seg;      // [cap_words/128 + 2] event_rel << 16 | fed of the chunk's first word
   uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
   uint32_t* sbits;          // [cap_words/32 + 64] run-start bits, bit (g - T0) (runs.cu)
+  uint8_t* cbad;            // [cap_words/128 + 2] per 128-word chunk: 0 when every word is decodable and the words of a
+                            // run ascend strictly in (link, roc, dcol, pxid), the detector's read-out order (runs.cu)
+  uint32_t geom_unique;     // 1 when no two valid cabling entries name the same ROC position of a module
   uint4* items;             // [item_cap] work items of the tile kernel
   uint32_t item_cap;
   uint32_t* n_clus;         // [(e1-e0)*M] clusters surviving the cut, per module

@@ -9,7 +9,9 @@
 // from the previous decodable word's (when all 128 words of the chunk are decodable, the usual case, that is the
 // word before it: one shuffle; otherwise a ballot / find-last-set scan).  Output: one start bit per word (bit g - T0
 // of sbits, T0 = first word of the launch group rounded down to 128; the lanes' nibbles are folded into four words by
-// three shuffles), module_first / module_end / the per-module run count (run_start, run_end).
+// three shuffles), module_first / module_end / the per-module run count (run_start, run_end), and one flag per chunk:
+// every word decodable and the words of a run strictly ascending in (link, roc, dcol, pxid) -- read-out order, in which
+// no pixel comes twice (tile.cu then skips its search for duplicates).
 // The previous decodable word before a range is searched backwards, 32 words at a time, never beyond the start of the
 // event (an earlier event's word never continues a run; segfill_kernel closes every event's last run).
 //
@@ -50,7 +52,7 @@ __global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Ch
   for (uint32_t c0 = ((blockIdx.x * blockDim.x + threadIdx.x) >> 5) * RANGE; c0 < n_chunks; c0 += nwarp * RANGE) {
     const uint32_t c1 = c0 + RANGE < n_chunks ? c0 + RANGE : n_chunks;
     // ---- the last decodable word before the range, inside the event of the range's first word
-    uint32_t carry_key = NOKEY, carry_g = 0u;
+    uint32_t carry_key = NOKEY, carry_g = 0u, carry_w = 0xFFFFFFFFu;  // carry_w: its raw word (all ones: unknown)
     {
       const uint32_t b = T0 + c0 * HC, cs = c.chunk_seg[c0], er0 = cs >> 16, sg0 = er0 * F + (cs & 0xFFFFu);
       const uint32_t gw = b < gBeg ? gBeg : b, evb = segB[er0 * F];
@@ -58,16 +60,18 @@ __global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Ch
       while (g > evb) {
         const bool in = lane < g - evb;
         const uint32_t gi = g - 1u - lane;
-        uint32_t key = NOKEY;
+        uint32_t key = NOKEY, wi = 0u;
         if (in) {
           uint32_t sg = sg0;
           while (segB[sg] > gi) --sg;
-          key = run_key(c.cab, __ldg(c.words + gi), (sg - er0 * F) << 11, er0);
+          wi = __ldg(c.words + gi);
+          key = run_key(c.cab, wi, (sg - er0 * F) << 11, er0);
         }
         const uint32_t bal = __ballot_sync(FULL, key != NOKEY);
         if (bal) {
           const int src = __ffs(bal) - 1;
           carry_key = __shfl_sync(FULL, key, src);
+          carry_w = __shfl_sync(FULL, wi, src);
           carry_g = g - 1u - (uint32_t)src;
           break;
         }
@@ -107,11 +111,18 @@ __global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Ch
         const uint32_t kmx = max(max(max(k[0], k[1]), max(k[2], k[3])), max(max(k[4], k[5]), max(k[6], k[7])));
         if (__all_sync(FULL, kmx != NOKEY)) {
           const uint32_t g8 = b + 8u * lane;
-          uint32_t pkey = __shfl_up_sync(FULL, k[7], 1), pg = g8 - 1u;
-          if (lane == 0) { pkey = carry_key; pg = carry_g; }
+          uint32_t pkey = __shfl_up_sync(FULL, k[7], 1), pg = g8 - 1u, pw = __shfl_up_sync(FULL, w8[7], 1);
+          if (lane == 0) { pkey = carry_key; pg = carry_g; pw = carry_w; }
           uint32_t sm = k[0] != pkey ? 1u : 0u;
+          bool viol = k[0] == pkey && (w8[0] >> 8) <= (pw >> 8);  // words of a run that do not ascend (read-out order)
 #pragma unroll
-          for (int i = 1; i < 8; ++i) sm |= k[i] != k[i - 1] ? 1u << i : 0u;
+          for (int i = 1; i < 8; ++i) {
+            sm |= k[i] != k[i - 1] ? 1u << i : 0u;
+            viol |= k[i] == k[i - 1] && (w8[i] >> 8) <= (w8[i - 1] >> 8);
+          }
+          const bool pair_bad = __any_sync(FULL, viol);
+          if (lane < 2) c.cbad[ci + lane] = pair_bad ? 1 : 0;
+          carry_w = __shfl_sync(FULL, w8[7], 31);
           if (sm) {  // (one copy of the atomics for the usual case of one start per lane)
             const uint32_t j0 = (uint32_t)__ffs((int)sm) - 1u;
             uint32_t sk = k[0], sp = pkey;
@@ -169,9 +180,14 @@ __global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Ch
       uint32_t startmask = 0u;
       uint32_t s_key = NOKEY, s_g = 0u, s_pkey = NOKEY, s_pg = 0u;  // the lane's first run start and its predecessor
       const uint32_t kmax = max(max(key[0], key[1]), max(key[2], key[3]));
+      bool chunk_bad = true;  // an undecodable word, or words of a run that do not ascend
       if (__all_sync(FULL, kmax != NOKEY)) {  // the usual chunk: every word decodable, the previous word is the neighbour
-        uint32_t pkey = __shfl_up_sync(FULL, key[3], 1), pg = g0 - 1u;
-        if (lane == 0) { pkey = carry_key; pg = carry_g; }
+        uint32_t pkey = __shfl_up_sync(FULL, key[3], 1), pg = g0 - 1u, pw = __shfl_up_sync(FULL, w[3], 1);
+        if (lane == 0) { pkey = carry_key; pg = carry_g; pw = carry_w; }
+        const bool viol = (key[0] == pkey && (w[0] >> 8) <= (pw >> 8)) || (key[1] == key[0] && (w[1] >> 8) <= (w[0] >> 8)) ||
+                          (key[2] == key[1] && (w[2] >> 8) <= (w[1] >> 8)) || (key[3] == key[2] && (w[3] >> 8) <= (w[2] >> 8));
+        chunk_bad = __any_sync(FULL, viol);
+        carry_w = __shfl_sync(FULL, w[3], 31);
         startmask = (key[0] != pkey ? 1u : 0u) | (key[1] != key[0] ? 2u : 0u) | (key[2] != key[1] ? 4u : 0u) | (key[3] != key[2] ? 8u : 0u);
         if (startmask) {
           const uint32_t j0 = (uint32_t)__ffs((int)startmask) - 1u;
@@ -203,7 +219,9 @@ __global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Ch
           const int top = 31 - __clz(has);
           carry_key = __shfl_sync(FULL, tkey, top); carry_g = b + 4u * (uint32_t)top + __shfl_sync(FULL, tj, top);
         }
+        carry_w = 0xFFFFFFFFu;
       }
+      if (lane == 0) c.cbad[ci] = chunk_bad ? 1 : 0;
       if (s_key != NOKEY) {  // one copy of the atomics for the usual case of at most one start per lane
         run_start(c, s_key, s_g);
         if (s_pkey != NOKEY) run_end(c, s_pkey, s_pg);

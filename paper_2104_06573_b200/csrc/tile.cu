@@ -13,7 +13,9 @@
 //       plus a second level (4 entries per 32 buckets) that is only read when the first is full; slots are handed
 //       out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
 //   P2  duplicates (S10) from the list of words that were not first in their bucket (exact pass only when a candidate
-//       turns up), four forward-neighbour lookups per word, edges into a per-warp list, lock-free unions on the
+//       turns up; list and pass are skipped for an item whose words come in the detector's read-out order, which the
+//       pre-pass certifies per 128-word chunk: such words are all different pixels), four forward-neighbour lookups
+//       per word, edges into a per-warp list, lock-free unions on the
 //       labels: hook-and-descend (pix_device.cuh), or by representatives (below) when the item's runs are long
 //   P3  root of every live pixel; roots start their accumulators (in the memory of the dead hash) and are listed in
 //       word order; the other pixels add charge | pixel count, charge*col, charge*row by shared atomics
@@ -222,6 +224,9 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     // the item's stretch of the temp record area, one slot per word: asked for now, needed in P4
     uint32_t wbase_t0 = 0u;
     if (tid == 0 && cluster_it) wbase_t0 = alloc_temp(c, len);
+    // Words in read-out order (every 128-word chunk the item touches is clean, runs.cu) are all different pixels
+    bool off_t = false;
+    if (tid <= ((g0 + len - 1u - T0) >> 7) - ((g0 - T0) >> 7)) off_t = c.cbad[((g0 - T0) >> 7) + tid] != 0;
     // No barrier here: what P0 writes (hash, counters, start bits, the run_bad of this item's parity) is not read by
     // the previous item's P5, and nothing else is written before the barrier at the end of P0.
     uint8_t* const rbad = s.run_bad[par];
@@ -250,7 +255,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         if (lane == 31) s.n_runs = inc;
       }
     }
-    __syncthreads();
+    const bool ordered = !__syncthreads_or(off_t) && c.geom_unique != 0u;
     // ================================================================== P1: decode, calibrate, insert
     // The words' state stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is
     // always [0]: free in the unrolled loops (register renaming), three moves in the rolled one of P2.
@@ -307,10 +312,10 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
             kk = 4u + (kb < 4u ? kb : 0u);
           }
           k0 |= kk << K_SLOT;
-          if (k >= 1u) chk = b | ((k < 7u ? k : 7u) << 11) | (tag << 14);
+          if (k >= 1u && !ordered) chk = b | ((k < 7u ? k : 7u) << 11) | (tag << 14);
         }
       }
-      {
+      if (!ordered) {
         const uint32_t mc = __ballot_sync(FULL, chk != 0u);
         const uint32_t at = nd + __popc(mc & lt_mask);
         if (chk != 0u) { if (at < ECAP) dl[at] = chk; else cand = true; }  // a full list: take the exact path
@@ -358,7 +363,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         }
       }
     }
-    if (__syncthreads_or(cand)) {
+    if (!ordered && __syncthreads_or(cand)) {  // (words in read-out order are all different)
 #pragma unroll
       for (int j = 0; j < NJ; ++j) {
         const uint32_t kj = key[j];

@@ -220,6 +220,53 @@ def test_undecodable_stretch_is_linear(gu, full):
     assert dt < 20.0, dt
 
 
+def test_two_cabling_entries_for_one_roc(gu, full):
+    """A cabling table in which two (link, ROC) entries name the same ROC position of a module: the same pixel can then
+    arrive twice in words that ascend in (link, roc, dcol, pxid) like ordinary read-out order.  The later word is a
+    DUPLICATE (S10) all the same; the tile kernel's short cut for ordered words must be off for such a table."""
+    import dataclasses
+    inv = full.inverse()
+    m = 700
+    f, l = int(inv["fed"][m]), int(inv["link"][m])
+    ent = full.cabling.reshape(full.n_feds, 64, 32).copy()
+    r1 = int(inv["roc"][m, 3])                                  # the ROC at position 3 (rocy 0, rocx 3)
+    r2 = int(np.nonzero((ent[f, l] & 2) == 0)[0][-1])           # an unused ROC number of the link, above the used ones
+    assert r2 > int(inv["roc"][m].max())
+    ent[f, l, r2] = ent[f, l, r1]
+    det = dataclasses.replace(full, cabling=ent.reshape(-1), _inv={})
+    rng = np.random.default_rng(31)
+    rows = np.r_[10, 10, 11, 11, 40, 41, 60]; cols = np.r_[160, 161, 160, 161, 170, 170, 200]   # inside ROC position 3
+    adc = rng.integers(60, 250, size=len(rows))
+    w, _ = full.encode(np.full(len(rows), m), rows, cols, adc)
+    again = (w[[1, 2, 4]] & ~np.uint32(31 << 21)) | np.uint32(r2 << 21)  # the same pixels through the second entry
+    again = (again & ~np.uint32(255)) | np.uint32(200)
+    other, _ = full.encode(np.full(3, m), np.r_[100, 100, 101], np.r_[20, 21, 21], np.r_[90, 90, 90])
+    mine = np.sort(np.concatenate([w, again, other])).astype(np.uint32)
+    assert np.all(np.diff(mine >> 8) > 0)                       # read-out order, every (link, roc, dcol, pxid) once
+    # forty other modules around it, each in read-out order, so that the module sits in the middle of a work item made of
+    # whole, clean 128-word chunks (the short cut is decided per chunk; the chunks at the ends of an event never take it)
+    per_fed = [[] for _ in range(full.n_feds)]
+    before, after = np.nonzero(inv["fed"] < f)[0], np.nonzero(inv["fed"] > f)[0]
+    for mo in np.r_[rng.choice(before, size=20, replace=False), rng.choice(after, size=20, replace=False)]:
+        r, c, a = _pixels(rng, 45)
+        wo, _ = full.encode(np.full(45, mo), r, c, a)
+        per_fed[int(inv["fed"][mo])].append((int(inv["link"][mo]), np.sort(wo)))
+    per_fed[f].append((l, mine))
+    chunks, fo = [], [0]
+    for lst in per_fed:
+        for _, wo in sorted(lst, key=lambda t: t[0]):
+            chunks.append(wo)
+        fo.append(sum(len(x) for x in chunks))
+    words = np.concatenate(chunks).astype(np.uint32)
+    at = int(np.nonzero(words == mine[0])[0][0])
+    assert 256 <= at and at + len(mine) + 256 <= len(words)
+    b = pixgen.Batch(words, np.array([0, len(words)], np.uint32), np.array(fo, np.uint32).reshape(1, -1), np.zeros((1, 5), np.uint32))
+    got = gu.run_batch(det, b, P)
+    exp = gu.oracle_events(det, b, P)
+    gu.assert_event_equal(got[0], exp[0], tag="two entries for one ROC")
+    assert int(exp[0]["summary"][7]) == 3                       # three DUPLICATE words
+
+
 def _full_size(gu, full, b, n_sample, seed, tag):
     """One pix_process_batch call with library-default launch groups; identities on every event, n_sample events
     compared element by element with the oracle."""
