@@ -84,7 +84,7 @@ size_t carve_workspace(pix_handle* h, unsigned char* base) {
   c.ctl = (uint32_t*)take(pix::CTL_WORDS * 4);
   c.ovf_list = (uint32_t*)take(Ec * M * 4);
   c.list_cap = (uint32_t)(Ec * M);
-  c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 4);
+  c.slice_list = (uint32_t*)take((W / 1024 + Ec + 1) * 8);  // two words per slice
   c.chunk_seg = (uint32_t*)take((W / 128 + 2) * 4);
   c.sbits = (uint32_t*)take((W / 32 + 64) * 4);  // the tile kernel reads 33 words from an item's first bit on
   c.cbad = (uint8_t*)take(W / 128 + 2);

@@ -3,9 +3,10 @@
 // cluster records to their final place clus_module_start[module] + local id (S14), and the summary (S20).
 //
 // Two kernels.  offsets: one block per event computes the event's M-entry scan (warp-shuffle scan), writes the
-// offsets and the summary, and appends the event's record slices (SLICE records each) to a work list.
-// scatter: a persistent grid takes slices from the list; a block stages the event's offsets in shared memory
-// and copies its records, one thread per output record, module found by binary search in the shared offsets.
+// offsets and the summary, and appends the event's record slices (SLICE records each, with the modules of the first
+// and the last record) to a work list.  scatter: a persistent grid takes slices from the list; a block stages the
+// offsets of the slice's modules in shared memory and copies its records, one thread per output record, module found
+// by binary search among those offsets.
 #include "pix_common.cuh"
 #include "pix_device.cuh"
 
@@ -106,11 +107,24 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
     s[10] = skip ? s_red[3] : ec[EC_CUT];
     s[11] = s_red[0]; s[12] = skip ? 0u : ec[EC_PRECUT]; s[13] = s_red[1]; s[14] = n_emit;
     s[15] = flags | (total > c.cap_ev ? FLAG_CAPACITY : 0u);
-    const uint32_t nsl = (n_emit + SLICE - 1u) / SLICE;
-    if (nsl) {
-      const uint32_t at = atomicAdd(c.ctl + CTL_SLICE_COUNT, nsl);
-      for (uint32_t q = 0; q < nsl; ++q) c.slice_list[at + q] = (er << 16) | q;  // cap_ev <= 2^26 records (pix_create)
+  }
+  // work items of the scatter: slices of SLICE records, each with the modules its first and last record belong to
+  const uint32_t nsl = (n_emit + SLICE - 1u) / SLICE;
+  if (tid == 0 && nsl) s_red[4] = atomicAdd(c.ctl + CTL_SLICE_COUNT, nsl);
+  __syncthreads();
+  auto module_of = [&](uint32_t g) {  // last m with s_start[m] <= g
+    uint32_t lo = 0, hi = M;
+    while (lo < hi) {
+      const uint32_t mid = (lo + hi + 1u) >> 1;
+      if (s_start[mid] <= g) lo = mid; else hi = mid - 1u;
     }
+    return lo;
+  };
+  for (uint32_t q = tid; q < nsl; q += FIN_THREADS) {
+    const uint32_t g_first = q * SLICE, g_last = (g_first + SLICE < n_emit ? g_first + SLICE : n_emit) - 1u;
+    const uint32_t at = s_red[4] + q;
+    c.slice_list[2u * at] = (er << 16) | q;  // cap_ev <= 2^26 records (pix_create)
+    c.slice_list[2u * at + 1u] = module_of(g_first) | (module_of(g_last) << 16);  // (module ids stay below 16384)
   }
 }
 
@@ -120,20 +134,21 @@ __global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_const
   const uint32_t M = c.M, tid = threadIdx.x;
   const uint32_t count = c.ctl[CTL_SLICE_COUNT];
   for (uint32_t it = blockIdx.x; it < count; it += gridDim.x) {
-    const uint32_t item = c.slice_list[it];
+    const uint32_t item = c.slice_list[2u * it], mods = c.slice_list[2u * it + 1u];
     const uint32_t er = item >> 16, e = c.e0 + er, g0 = (item & 0xFFFFu) * SLICE;
+    const uint32_t m_first = mods & 0xFFFFu, m_last = mods >> 16;  // the slice's records lie in these modules
     const uint32_t* cms = c.clus_module_start + (size_t)e * (M + 1);
     __syncthreads();  // the previous item is done with s_start
-    for (uint32_t m = tid; m <= M; m += FIN_THREADS) s_start[m] = cms[m];
+    for (uint32_t m = m_first + tid; m <= m_last + 1u; m += FIN_THREADS) s_start[m] = cms[m];
+    const uint32_t total = cms[M];
     __syncthreads();
-    const uint32_t total = s_start[M];
     const uint32_t n_emit = total < c.cap_ev ? total : c.cap_ev;
     const uint32_t* tbase = c.t_base + (size_t)er * M;
 #pragma unroll
     for (uint32_t j = 0; j < SLICE / FIN_THREADS; ++j) {
       const uint32_t g = g0 + j * FIN_THREADS + tid;
       if (g >= n_emit) continue;
-      uint32_t lo = 0, hi = M;  // last m with s_start[m] <= g
+      uint32_t lo = m_first, hi = m_last;  // last m with s_start[m] <= g
       while (lo < hi) {
         const uint32_t mid = (lo + hi + 1u) >> 1;
         if (s_start[mid] <= g) lo = mid; else hi = mid - 1u;

@@ -84,7 +84,7 @@ struct Chunk {
   uint32_t* ovf_list;       // [(e1-e0)*M] task ids (event_rel*M + module) left to the overflow kernel
   uint32_t list_cap;        // (e1-e0)*M: every event lists at most M runs (push_run)
   uint32_t* chunk_seg;      // [cap_words/128 + 2] event_rel << 16 | fed of the chunk's first word
-  uint32_t* slice_list;     // [cap_words/1024 + (e1-e0)] scatter work items: event_rel << 16 | slice
+  uint32_t* slice_list;     // [2 * (cap_words/1024 + (e1-e0))] scatter work items: event_rel << 16 | slice, first | last << 16 module
   uint32_t* sbits;          // [cap_words/32 + 64] run-start bits, bit (g - T0) (runs.cu)
   uint8_t* cbad;            // [cap_words/128 + 2] per 128-word chunk: 0 when every word is decodable and the words of a
                             // run ascend strictly in (link, roc, dcol, pxid), the detector's read-out order (runs.cu)
