@@ -11,9 +11,11 @@
 //      row*416+col; equal keys keep the MIN digi index (S10: first index wins)
 //   2  a digi that is not the owner of its position is a DUPLICATE
 //   3  every live digi (owner, charge >= threshold) looks up its 4 forward neighbours
-//      (r,c+1) (r+1,c-1) (r+1,c) (r+1,c+1) and unites with live owners: hook-and-descend with atomicMin
-//      (larger index under smaller) => the root is the component's min digi index
-//   4  flatten labels; add charge, pixel count and charge-weighted col/row into the root's accumulators
+//      (r,c+1) (r+1,c-1) (r+1,c) (r+1,c+1) and unites with live owners: representatives with pointer jumping, the
+//      larger root hooked under the smaller by compare-and-swap (unite_roots, pix_device.cuh) => the root is the
+//      component's min digi index
+//   4  flatten labels; add charge, pixel count and charge-weighted col/row into the root's accumulators (the 64-bit
+//      sums in shared memory as two 32-bit halves: add_weighted)
 //   5  roots in digi order: Q >= cut survives and takes the next local id (ballot/popc scan); the root
 //      writes the temp record at (run first + id)
 //   6  per digi: final status and clus; per task: counts
@@ -73,7 +75,7 @@ __device__ __forceinline__ uint32_t hash_find(const SlotT* tab, uint32_t size, u
   }
 }
 
-// ------------------------------------------------------------------ unions: hook() of pix_device.cuh
+// ------------------------------------------------------------------ unions: unite_roots() of pix_device.cuh
 // read-only walk to the root (step 4: own entries are being flattened concurrently, nobody else's may be written)
 __device__ __forceinline__ uint32_t uf_root(const volatile uint32_t* L, uint32_t x) {
   uint32_t p = L[x];
@@ -124,6 +126,27 @@ struct Tables {
   unsigned long long* sx;     // [n] sum charge*col
   unsigned long long* sy;     // [n] sum charge*row
 };
+
+// Charge-weighted sums (64 bits).  In shared memory a 64-bit atomicAdd is a compare-and-swap loop, and the hundreds of
+// pixels of a long cluster all add to one root: there the two halves of the word take the low 16 bits and the rest of
+// every addend (< 2^25) by 32-bit atomics, exact for up to 65536 addends.  In the global workspace: one 64-bit atomic.
+template <bool SPLIT>
+__device__ __forceinline__ void add_weighted(unsigned long long* a, uint32_t v) {
+  if (SPLIT) {
+    uint32_t* h = reinterpret_cast<uint32_t*>(a);
+    atomicAdd(h, v & 0xFFFFu); atomicAdd(h + 1, v >> 16);
+  } else {
+    atomicAdd(a, (unsigned long long)v);
+  }
+}
+template <bool SPLIT>
+__device__ __forceinline__ unsigned long long weighted_sum(const unsigned long long* a) {
+  if (SPLIT) {
+    const uint32_t* h = reinterpret_cast<const uint32_t*>(a);
+    return (unsigned long long)h[0] + ((unsigned long long)h[1] << 16);
+  }
+  return *a;
+}
 
 // ------------------------------------------------------------------ the task
 template <typename G, typename SlotT, bool STAGE_CHARGE>
@@ -180,7 +203,7 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
       const uint32_t j = hash_find(T.tab, size, nkey);
       if (j == NO_INDEX) continue;
       if (!(((volatile uint32_t*)T.pos)[j] & LIVE)) continue;
-      hook(T.label, k, j);
+      unite_roots(T.label, k, j);  // (long clusters are why a run ends up here: not hook-and-descend)
     }
   }
   g.sync();
@@ -195,8 +218,8 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     const uint32_t e = (uint32_t)(STAGE_CHARGE ? T.chg[k] : c.d_charge[gb + k]);
     atomicAdd(T.q + r, e);
     atomicAdd(T.npix + r, 1u);
-    atomicAdd(T.sx + r, (unsigned long long)e * col);
-    atomicAdd(T.sy + r, (unsigned long long)e * row);
+    add_weighted<STAGE_CHARGE>(T.sx + r, e * col);
+    add_weighted<STAGE_CHARGE>(T.sy + r, e * row);
   }
   g.sync();
   // 5: roots in digi order -> local ids (S14), temp records (S18) in a stretch of n slots of the temp area
@@ -218,8 +241,8 @@ __device__ __forceinline__ void cluster_task(const Chunk& c, const G& g, const T
     const uint32_t id = n_post + g.scan_flag(surv, tot_post);
     if (root) {
       if (surv) {
-        put_temp(c, tbase + id, first + k, T.npix[k], Q, (float)((double)T.sx[k] / (double)Q),
-                 (float)((double)T.sy[k] / (double)Q));
+        put_temp(c, tbase + id, first + k, T.npix[k], Q, (float)((double)weighted_sum<STAGE_CHARGE>(T.sx + k) / (double)Q),
+                 (float)((double)weighted_sum<STAGE_CHARGE>(T.sy + k) / (double)Q));
       }
       T.q[k] = surv ? id : NO_INDEX;
     }

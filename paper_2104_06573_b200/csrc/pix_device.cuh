@@ -85,4 +85,26 @@ __device__ __forceinline__ void hook(uint32_t* L, uint32_t a, uint32_t b) {
   }
 }
 
+// Union for long clusters (hook-and-descend walks chains that grow with the cluster): tile.cu's items of long runs, cluster.cu.  After
+// Jaiganesh & Burtscher's ECL-CC: find the representatives with intermediate pointer jumping (plain stores are safe
+// here because a label is only ever replaced by an ancestor and only roots are hooked), hook the larger root under
+// the smaller one by compare-and-swap, go on from the winner's parent when the root was taken meanwhile.
+__device__ __forceinline__ uint32_t representative(uint32_t* L, uint32_t v) {
+  uint32_t curr = L[v];
+  if (curr != v) {
+    uint32_t prev = v, next;
+    while (curr > (next = L[curr])) { L[prev] = next; prev = curr; curr = next; }
+  }
+  return curr;
+}
+static __device__ __noinline__ void unite_roots(uint32_t* L, uint32_t a, uint32_t b) {
+  uint32_t ra = representative(L, a), rb = representative(L, b);
+  while (ra != rb) {
+    const uint32_t hi = ra > rb ? ra : rb, lo = ra > rb ? rb : ra;
+    const uint32_t old = atomicCAS(L + hi, hi, lo);
+    if (old == hi) break;
+    ra = representative(L, old); rb = lo;
+  }
+}
+
 }  // namespace pix
