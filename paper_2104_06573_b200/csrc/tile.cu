@@ -233,19 +233,15 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         if (lane == 31) s.n_runs = inc;
       }
     }
-    const bool ordered = !__syncthreads_or(off_t) && c.geom_unique != 0u;
     // ================================================================== P1: decode, calibrate, insert
     // The words' state stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is
     // always [0]: free in the unrolled loops (register renaming), three moves in the rolled one of P2.
+    // First what needs neither the cleared tables nor the start bits -- decode, calibration, the four stores -- so that
+    // nobody waits at P0's barrier for the warp that fetches the start bits; the module waits in cr's upper half.
     const uint32_t fed_split = g0 + len <= nextB ? 0xFFFFFFFFu : nextB;  // words from here on belong to a later FED (rare)
     uint32_t key[NJ];  // K_* below; NOKEY: not decodable
     uint32_t cr[NJ];   // charge | root << 16
     bool fail = false;
-    // Words that are not the first entry of their bucket go to a per-warp list (bucket | slot | tag): only they can be
-    // the later copy of a pixel that appears twice (S10), and after the barrier the list is checked with all lanes busy.
-    uint32_t* const dl = s.edge[warp];  // (the edge lists are not in use yet)
-    uint32_t nd = 0u;
-    bool cand = false;  // some pixel of the item may appear twice
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
       const uint32_t p = tid + NT * j, g = g0 + p;
@@ -269,13 +265,27 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
         }
       }
+      key[0] = ok ? ((row << 9) | col | (e < c.thr ? K_BELOW : 0u)) : NOKEY;  // S9; the run comes after the barrier
+      cr[0] = (uint32_t)e | (m << 16);
+      ROT4(w); ROT4(key); ROT4(cr);
+    }
+    const bool ordered = !__syncthreads_or(off_t) && c.geom_unique != 0u;  // P0 is done
+    // Words that are not the first entry of their bucket go to a per-warp list (bucket | slot | tag): only they can be
+    // the later copy of a pixel that appears twice (S10), and after the barrier the list is checked with all lanes busy.
+    uint32_t* const dl = s.edge[warp];  // (the edge lists are not in use yet)
+    uint32_t nd = 0u;
+    bool cand = false;  // some pixel of the item may appear twice
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const uint32_t p = tid + NT * j;
+      const uint32_t kj = key[0];
+      const bool ok = kj != NOKEY, below = (kj & K_BELOW) != 0u;
       const uint32_t bw = s.bits[j * NWARP + warp];
       const uint32_t r = s.pre[j * NWARP + warp] + __popc(bw & le_mask) - 1u;  // a decodable word lies in a run: r >= 0
-      const bool below = e < c.thr;  // S9
       uint32_t k0 = NOKEY, chk = 0u;
       if (ok) {
-        k0 = (r << 17) | (row << 9) | col | (below ? K_BELOW : 0u);
-        if ((bw >> lane) & 1u) { s.run_pos[r] = (uint16_t)p; s.run_mod[r] = (uint16_t)m; }
+        k0 = kj | (r << 17);
+        if ((bw >> lane) & 1u) { s.run_pos[r] = (uint16_t)p; s.run_mod[r] = (uint16_t)(cr[0] >> 16); }
         if (cluster_it) {
           const uint32_t h = hash_of(k0), b = bucket_of(h), sh8 = (b & 3u) * 8u;
           const uint32_t k = (atomicAdd(&s.cnt[b >> 2], 1u << sh8) >> sh8) & 0xFFu;
@@ -300,8 +310,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         nd += __popc(mc);
       }
       s.label[p] = (ok && !below) ? p : MARK;
-      key[0] = k0; cr[0] = (uint32_t)e;
-      ROT4(w); ROT4(key); ROT4(cr);
+      key[0] = k0; cr[0] &= 0xFFFFu;
+      ROT4(key); ROT4(cr);
     }
     if (!cluster_it) {  // a piece of a run longer than the tile: the block-per-run kernel clusters it
       if ((iflags & ITEM_LONG_HEAD) && tid == 0 && key[0] != NOKEY) push_run(c, c.ovf_list, CTL_OVF_COUNT, er, s.run_mod[0]);
