@@ -300,6 +300,7 @@ template <int THREADS, uint32_t CAP>
 __global__ void __launch_bounds__(THREADS) block_kernel(const __grid_constant__ Chunk c, const uint32_t* __restrict__ in_list,
                                                         uint32_t ctl_count, uint32_t ctl_ticket, uint32_t* __restrict__ long_list,
                                                         uint32_t ctl_long) {
+  chain_begin();
   extern __shared__ __align__(16) unsigned char ovf_smem[];
   __shared__ uint32_t s_scan[THREADS / 32 + 1];
   __shared__ uint32_t s_task;
@@ -350,7 +351,7 @@ cudaError_t configure_overflow_kernel() {
 
 // the runs the tile kernel left: longer than 1024 digis, hash overflow, or with 64-bit charge sums
 void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
-  block_kernel<T_B, CAP_B><<<n_sm * 2, T_B, CAP_B * SMEM_PER_DIGI, stream>>>(c, c.ovf_list, CTL_OVF_COUNT, CTL_OVF_TICKET, nullptr, 0u);
+  launch_chained(false, block_kernel<T_B, CAP_B>, n_sm * 2, T_B, CAP_B * SMEM_PER_DIGI, stream, c, (const uint32_t*)c.ovf_list, (uint32_t)CTL_OVF_COUNT, (uint32_t)CTL_OVF_TICKET, (uint32_t*)nullptr, 0u);
 }
 
 }  // namespace pix

@@ -15,6 +15,7 @@ namespace {
 // whatever the caller's offset arrays hold, every index derived later stays inside the buffers.
 // Other threads initialise the per-(event,module) range sentinels and zero the counters.
 __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk c, uint32_t n_total) {
+  chain_begin();
   const uint32_t Ec = c.e1 - c.e0;
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
   uint32_t lo = ev_offset(c, c.e0);
@@ -59,6 +60,7 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ Chunk
 // last run: module_end of the module of the event's last decodable word (the runs kernel closes a run when it
 // sees the next run start of the same event, and never looks back beyond the start of an event).
 __global__ void __launch_bounds__(256) segfill_kernel(const __grid_constant__ Chunk c) {
+  chain_begin();
   const uint32_t F = c.F, Ec = c.e1 - c.e0, S = Ec * F;
   const uint32_t gBeg = c.segB[0], gEnd = c.segB[S];
   if (gBeg >= gEnd) return;
@@ -107,8 +109,8 @@ static inline int grid_for(uint32_t work_items, uint32_t per_block, int cap_bloc
 
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream) {
   const uint32_t Ec = c.e1 - c.e0;
-  init_kernel<<<grid_for(Ec * c.M, 256, n_sm * 8), 256, 0, stream>>>(c, n_total);
-  segfill_kernel<<<grid_for(Ec * (c.F > 32u ? c.F : 32u), 256, n_sm * 8), 256, 0, stream>>>(c);
+  launch_chained(true, init_kernel, grid_for(Ec * c.M, 256, n_sm * 8), 256, 0, stream, c, n_total);
+  launch_chained(true, segfill_kernel, grid_for(Ec * (c.F > 32u ? c.F : 32u), 256, n_sm * 8), 256, 0, stream, c);
 }
 
 }  // namespace pix

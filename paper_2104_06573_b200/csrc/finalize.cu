@@ -28,6 +28,7 @@ __device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, uint32_t lan
 constexpr uint32_t SLICE = 1024;  // records per scatter work item
 
 __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_constant__ Chunk c) {
+  chain_begin();
   extern __shared__ uint32_t s_start[];  // [M+1]
   __shared__ uint32_t s_warp[FIN_THREADS / 32];
   __shared__ uint32_t s_red[8];
@@ -130,6 +131,7 @@ __global__ void __launch_bounds__(FIN_THREADS) offsets_kernel(const __grid_const
 
 // ---- records: output record g of the event <- temp record (run first + local id)
 __global__ void __launch_bounds__(FIN_THREADS) scatter_kernel(const __grid_constant__ Chunk c) {
+  chain_begin();
   extern __shared__ uint32_t s_start[];  // [M+1]
   const uint32_t M = c.M, tid = threadIdx.x;
   const uint32_t count = c.ctl[CTL_SLICE_COUNT];
@@ -174,8 +176,8 @@ cudaError_t configure_finalize_kernel() {
 void launch_finalize(const Chunk& c, int n_sm, cudaStream_t stream) {
   const uint32_t Ec = c.e1 - c.e0;
   const size_t smem = (size_t)(c.M + 1) * sizeof(uint32_t);
-  offsets_kernel<<<Ec, FIN_THREADS, smem, stream>>>(c);
-  scatter_kernel<<<n_sm * 8, FIN_THREADS, smem, stream>>>(c);
+  launch_chained(true, offsets_kernel, Ec, FIN_THREADS, smem, stream, c);
+  launch_chained(false, scatter_kernel, n_sm * 8, FIN_THREADS, smem, stream, c);
 }
 
 }  // namespace pix

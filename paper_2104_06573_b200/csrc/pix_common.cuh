@@ -113,6 +113,26 @@ __device__ __forceinline__ void put_temp(const Chunk& c, uint32_t i, uint32_t fi
   c.t_a[i] = make_uint4(first, npix, charge, __float_as_uint(x)); c.t_y[i] = y;
 }
 
+// The kernels of a launch group are chained by programmatic dependent launch: each one lets its successor's blocks
+// be placed as soon as all of its own blocks have started, and each one waits for its predecessor to finish (and its
+// writes to be visible) before it touches memory.  That hides the launch and ramp-up latency between the eight
+// kernels (one event per call: 74 -> 66 us); the order of the work is that of the stream.  Two launches stay plain
+// (`chained` false), measured: the overflow kernel and the scatter, whose early blocks cost the large batch 0.5-4 %.
+__device__ __forceinline__ void chain_begin() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+template <typename... KArgs, typename... Args>
+inline void launch_chained(bool chained, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = chained ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 // launchers (host), one per kernel; all asynchronous on `stream`
 void launch_init(const Chunk& c, uint32_t n_total, int n_sm, cudaStream_t stream);
 void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t stream);

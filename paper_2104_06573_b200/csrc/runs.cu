@@ -40,6 +40,7 @@ __device__ __forceinline__ uint32_t run_key(const CabEntry* __restrict__ cab, ui
 }
 
 __global__ void __launch_bounds__(256, 4) runs_kernel(const __grid_constant__ Chunk c) {
+  chain_begin();
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t F = c.F, S = (c.e1 - c.e0) * F;
   const uint32_t* __restrict__ segB = c.segB;
@@ -323,6 +324,7 @@ __device__ __forceinline__ uint32_t count_starts(const Stage& st, uint32_t lo, u
 }
 
 __global__ void __launch_bounds__(PACK_WARPS * 32) pack_kernel(const __grid_constant__ Chunk c) {
+  chain_begin();
   __shared__ PackWarp sm[PACK_WARPS];
   const uint32_t lane = threadIdx.x & 31u;
   PackWarp& pw = sm[threadIdx.x >> 5];
@@ -428,9 +430,9 @@ void launch_runs(const Chunk& c, uint32_t words_bound, int n_sm, cudaStream_t st
   uint64_t nb = ((uint64_t)words_bound + 2 * HC + 8 * RANGE * HC - 1) / (8 * RANGE * HC);  // 8 warps of RANGE chunks per block
   if (nb < 1) nb = 1;
   if (nb > (uint64_t)n_sm * 64) nb = (uint64_t)n_sm * 64;
-  runs_kernel<<<(int)nb, 256, 0, stream>>>(c);
+  launch_chained(true, runs_kernel, (unsigned)nb, 256, 0, stream, c);
   const uint32_t Ec = c.e1 - c.e0;
-  pack_kernel<<<(int)((Ec * PACK_SEGS + PACK_WARPS - 1u) / PACK_WARPS), PACK_WARPS * 32, 0, stream>>>(c);
+  launch_chained(true, pack_kernel, (Ec * PACK_SEGS + PACK_WARPS - 1u) / PACK_WARPS, PACK_WARPS * 32, 0, stream, c);
 }
 
 }  // namespace pix

@@ -165,6 +165,7 @@ __device__ __noinline__ bool resolve_dup(TileSmem& s, uint32_t b, uint32_t h, ui
 }
 
 __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_constant__ Chunk c) {
+  chain_begin();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileSmem& s = *reinterpret_cast<TileSmem*>(smem_raw);
   uint32_t tid;
@@ -575,7 +576,7 @@ cudaError_t configure_tile_kernel() {
 }
 
 void launch_tile(const Chunk& c, int n_sm, cudaStream_t stream) {
-  tile_kernel<<<n_sm * BLOCKS_PER_SM, NT, sizeof(TileSmem), stream>>>(c);
+  launch_chained(true, tile_kernel, n_sm * BLOCKS_PER_SM, NT, sizeof(TileSmem), stream, c);
 }
 
 }  // namespace pix
