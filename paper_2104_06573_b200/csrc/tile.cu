@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       if (ok) e = calibrate(c, w[0] & 255u, __ldg(c.gp + (m * (uint32_t)COLS + col)));  // S8: one pair per (module, col)
       else { m = row = col = 0xFFFFu; }
       if (valid) {
-        c.d_module[g] = (uint16_t)m; c.d_row[g] = (uint16_t)row; c.d_col[g] = (uint16_t)col; c.d_charge[g] = e;
+        __stcs(c.d_module + g, (uint16_t)m); __stcs(c.d_row + g, (uint16_t)row); __stcs(c.d_col + g, (uint16_t)col); __stcs(c.d_charge + g, e);
         if (!ok) {  // undecodable words are finished here
           c.d_status[g] = (uint8_t)st; c.d_clus[g] = -1;
           atomicAdd(c.ev_cnt + (size_t)er * EC_STRIDE + (st - ST_EMPTY), 1u);
@@ -539,7 +539,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         if (id != NO_ID) { so = ST_OK; cl = (int32_t)id; cntB += 1u; } else { so = ST_CUT; cntB += 0x10000u; }
         cntP += rt == p ? 1u : 0u;
       }
-      c.d_status[g0 + p] = (uint8_t)so; c.d_clus[g0 + p] = cl;
+      __stcs(c.d_status + g0 + p, (uint8_t)so); __stcs(c.d_clus + g0 + p, cl);
     }
     __syncwarp();
     if (warp * 32u < R) {  // the warps that hold a run each in some lane
