@@ -221,6 +221,36 @@ int pix_overflow_runs(pix_handle* h, uint32_t* out);
 int pix_set_profiling(pix_handle* h, int enable);
 int pix_read_profile(pix_handle* h, float* ms_out, uint32_t* n_chunks_out);
 
+/* Clustering of ONE module's decoded digis without any allocation (for callers that cannot call cudaMalloc: code under
+ * CUDA graph capture, tight serving loops; pix_create allocates, so this entry point takes no handle).
+ * "clusters the pixels on each detector module"; the same readings as pix_process (S9 threshold and charge cut, S10
+ * first digi of a pixel wins, S13 8-connectivity, S14 clusters numbered by their lowest digi, S18 records), run by the
+ * block-per-run kernel with its tables in a static device array of 1 MiB + 256 B (64 B per digi) that every GPU
+ * holds from the moment it loads the library.
+ *   n_digis <= PIX_NOALLOC_MAX_DIGIS, else PIX_ERR_CAPACITY (nothing is launched).
+ *   row, col, charge [n_digis]  DEVICE, inputs (the digi arrays pix_process wrote for the module's words, in word
+ *                    order): row < 160 and col < 416, or row == 0xFFFF for a word that is not a pixel.
+ *   clus, status [n_digis]      DEVICE, outputs as in pix_digis; a word with row == 0xFFFF gets clus = -1 and its
+ *                    status is left untouched.
+ *   c_first_digi .. c_y_row [max_clusters]  DEVICE, outputs: the module's cluster records in local-id order
+ *                    (first_digi = index into the module's digis); records at and beyond counts[1] are untouched.
+ *   counts [8]       DEVICE, output: clusters surviving the cut, records emitted (min with max_clusters), clusters
+ *                    before the cut, digis DUPLICATE / BELOW_THRESHOLD / OK / CUT, 0.
+ * One 512-thread block on the caller's stream; asynchronous; calls no cudaMalloc / cudaFree or allocating routine.
+ * Every call shares the static array (it keeps the last call's contents; the kernel clears what must start at zero),
+ * so two calls that overlap on one GPU (two streams, two host threads) race: serialise them.
+ * pix_noalloc_setup looks the array's device address up (cudaGetSymbolAddress) for the current device; call it once
+ * per device, with that device current, before a region where even that is unwelcome (stream capture);
+ * pix_cluster_module_noalloc does it itself on first use otherwise.  Errors: the codes above; the text comes from
+ * pix_noalloc_last_error (per host thread, "" if the last call succeeded). */
+#define PIX_NOALLOC_MAX_DIGIS 16384u
+int pix_noalloc_setup(void);
+int pix_cluster_module_noalloc(void* cuda_stream, uint32_t n_digis, const uint16_t* row, const uint16_t* col,
+                               const int32_t* charge, int32_t pixel_threshold_e, int32_t cluster_charge_cut_e,
+                               uint32_t max_clusters, int32_t* clus, uint8_t* status, uint32_t* c_first_digi,
+                               uint32_t* c_n_pix, uint32_t* c_charge, float* c_x_col, float* c_y_row, uint32_t* counts);
+const char* pix_noalloc_last_error(void);
+
 /* Text of the last error on this handle ("" if none).  Valid until the next call on the handle. */
 const char* pix_last_error(const pix_handle* h);
 

@@ -25,7 +25,9 @@ SUMMARY = ("n_words", "n_decoded", "n_empty", "n_err_link", "n_err_roc", "n_err_
 FLAG_NONCONTIGUOUS, FLAG_CLUSTER_CAPACITY_OVERFLOW, FLAG_EVENT_TOO_LARGE = 1, 2, 4
 EXPORTS = ("pix_create", "pix_clone", "pix_destroy", "pix_process", "pix_process_batch", "pix_process_batch_host",
            "pix_rechits", "pix_kernel_launches", "pix_last_error", "pix_set_profiling", "pix_read_profile",
-           "pix_overflow_runs", "pix_host_bytes_out", "pix_legacy_format")
+           "pix_overflow_runs", "pix_host_bytes_out", "pix_legacy_format", "pix_noalloc_setup",
+           "pix_cluster_module_noalloc", "pix_noalloc_last_error")
+NOALLOC_MAX_DIGIS = 16384  # PIX_NOALLOC_MAX_DIGIS of include/pixclus.h
 
 _vp, _u32 = ctypes.c_void_p, ctypes.c_uint32
 
@@ -272,6 +274,37 @@ def pix_legacy_format(h: Handle, stream, n_events: int, raw_words, n_words_total
     rc = lib.pix_legacy_format(h.ptr, _stream_ptr(stream), n_events, _ptr(raw_words), n_words_total, _ptr(event_word_offsets),
                                _ptr(fed_offsets), ctypes.byref(d), _ptr(module_raw_id), max_errors_per_event, ctypes.byref(o))
     return _check(h, rc, raise_on_error)
+
+
+def pix_noalloc_last_error() -> str:
+    lib = load()
+    lib.pix_noalloc_last_error.restype = ctypes.c_char_p
+    return (lib.pix_noalloc_last_error() or b"").decode()
+
+
+def pix_noalloc_setup() -> None:
+    """Looks up the static scratch array's address for the current device (allocates nothing)."""
+    lib = load()
+    lib.pix_noalloc_setup.restype = ctypes.c_int
+    rc = lib.pix_noalloc_setup()
+    if rc != 0:
+        raise PixError(rc, pix_noalloc_last_error())
+
+
+def pix_cluster_module_noalloc(stream, n_digis: int, row, col, charge, pixel_threshold_e: int, cluster_charge_cut_e: int,
+                               max_clusters: int, out: dict, raise_on_error: bool = True) -> int:
+    """One module's decoded digis -> clus, status, cluster records, counts, with no allocation anywhere (device
+    pointers, asynchronous).  out: clus, status, first_digi, n_pix, charge, x_col, y_row, counts."""
+    lib = load()
+    lib.pix_cluster_module_noalloc.argtypes = [_vp, _u32, _vp, _vp, _vp, ctypes.c_int32, ctypes.c_int32, _u32] + [_vp] * 8
+    lib.pix_cluster_module_noalloc.restype = ctypes.c_int
+    rc = lib.pix_cluster_module_noalloc(_stream_ptr(stream), n_digis, _ptr(row), _ptr(col), _ptr(charge), pixel_threshold_e,
+                                        cluster_charge_cut_e, max_clusters,
+                                        *[_ptr(out.get(k)) for k in ("clus", "status", "first_digi", "n_pix", "charge",
+                                                                     "x_col", "y_row", "counts")])
+    if rc != 0 and raise_on_error:
+        raise PixError(rc, pix_noalloc_last_error())
+    return rc
 
 
 def alloc_legacy(n_words: int, n_events: int, max_errors_per_event: int, device="cuda", fill: int | None = None):

@@ -20,6 +20,10 @@
 //      writes the temp record at (run first + id)
 //   6  per digi: final status and clus; per task: counts
 // The digi fields (row, col, charge) are read back from the output arrays the decode kernel has written.
+#include <cstdio>
+#include <mutex>
+
+#include "../../include/pixclus.h"
 #include "pix_common.cuh"
 #include "pix_device.cuh"
 
@@ -354,4 +358,139 @@ void launch_overflow(const Chunk& c, int n_sm, cudaStream_t stream) {
   launch_chained(false, block_kernel<T_B, CAP_B>, n_sm * 2, T_B, CAP_B * SMEM_PER_DIGI, stream, c, (const uint32_t*)c.ovf_list, (uint32_t)CTL_OVF_COUNT, (uint32_t)CTL_OVF_TICKET, (uint32_t*)nullptr, 0u);
 }
 
+
+// ------------------------------------------------------------------ the entry point that allocates nothing
+// pix_cluster_module_noalloc (include/pixclus.h): the global-workspace path of the kernel above for ONE module's
+// decoded digis, for callers that cannot call cudaMalloc (no handle: pix_create allocates).  Its tables live in a
+// file-scope device array of fixed size, which every GPU that loads the library holds until the process exits:
+//   header (256 B) + per digi 16 B hash + 4 B position + 4 B charge sum + 4 B pixel count + 8 + 8 B weighted sums
+//   + 20 B temp record = 256 B + 64 B x PIX_NOALLOC_MAX_DIGIS (16384) = 1 MiB + 256 B.
+// In host code the array's name is a host-side stand-in, not a device address: pix_noalloc_setup asks
+// cudaGetSymbolAddress for the address once per device and the launch passes pointers made from it.
+// Every call uses the same array: the kernel clears what has to start at zero, and calls that overlap on the GPU
+// (two streams, two threads) race.
+namespace {
+
+constexpr uint32_t NA_MAX = PIX_NOALLOC_MAX_DIGIS;
+constexpr size_t NA_HDR = 256, NA_BYTES = NA_HDR + (size_t)NA_MAX * 64;
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NA_BYTES];
+
+// header words (uint32)
+enum { NH_FIRST = 0, NH_END = 1, NH_SEG = 2 /* 2 words */, NH_NCLUS = 4, NH_TBASE = 5, NH_EVCNT = 16 /* 16 */, NH_CTL = 32 /* 16 */ };
+
+struct NoallocOut {
+  uint32_t* first_digi; uint32_t* n_pix; uint32_t* charge; float* x_col; float* y_row; uint32_t* counts;
+};
+
+__global__ void __launch_bounds__(T_B) noalloc_kernel(const __grid_constant__ Chunk c, uint32_t* hdr, uint32_t n,
+                                                      uint32_t max_clusters, NoallocOut o) {
+  __shared__ uint32_t s_scan[T_B / 32 + 1];
+  const BlockGroup<T_B> g{s_scan};
+  // the array keeps the last call's contents: the header (run bounds, counters) is written afresh, the tables are
+  // cleared or overwritten by the task itself (steps 0 and 1)
+  if (threadIdx.x < NA_HDR / 4) hdr[threadIdx.x] = (threadIdx.x == NH_END || threadIdx.x == NH_SEG + 1) ? n : 0u;
+  __syncthreads();
+  Tables<unsigned long long> T;
+  T.tab = c.g_hash; T.pos = c.g_pos; T.chg = nullptr;
+  T.label = reinterpret_cast<uint32_t*>(c.d_clus);  // clus is written last, per digi
+  T.q = c.g_q; T.npix = c.g_npix; T.sx = c.g_sx; T.sy = c.g_sy;
+  cluster_task<BlockGroup<T_B>, unsigned long long, false>(c, g, T, 0u);
+  __syncthreads();
+  const uint32_t total = hdr[NH_NCLUS], tb = hdr[NH_TBASE];
+  const uint32_t emit = total < max_clusters ? total : max_clusters;
+  for (uint32_t i = threadIdx.x; i < emit; i += T_B) {  // temp records (in local-id order) -> the caller's arrays
+    const uint4 a = c.t_a[tb + i];
+    o.first_digi[i] = a.x; o.n_pix[i] = a.y; o.charge[i] = a.z; o.x_col[i] = __uint_as_float(a.w); o.y_row[i] = c.t_y[tb + i];
+  }
+  if (threadIdx.x == 0) {
+    const uint32_t* ec = hdr + NH_EVCNT;
+    o.counts[0] = total; o.counts[1] = emit; o.counts[2] = ec[EC_PRECUT]; o.counts[3] = ec[EC_DUP];
+    o.counts[4] = ec[EC_BELOW]; o.counts[5] = ec[EC_OK]; o.counts[6] = ec[EC_CUT]; o.counts[7] = 0u;
+  }
+}
+
+constexpr int NA_MAX_DEVICES = 64;
+std::mutex g_noalloc_mu;
+unsigned char* g_noalloc_addr[NA_MAX_DEVICES];  // device address of g_noalloc_scratch, per device ordinal
+thread_local char g_noalloc_err[192];
+
+int noalloc_fail(int code, const char* fmt, unsigned long long a, unsigned long long b) {
+  snprintf(g_noalloc_err, sizeof(g_noalloc_err), fmt, a, b);
+  return code;
+}
+int noalloc_fail(int code, const char* msg) {
+  snprintf(g_noalloc_err, sizeof(g_noalloc_err), "%s", msg);
+  return code;
+}
+
+// the scratch array's address on the current device (looked up on first use, with that device current)
+int noalloc_address(unsigned char** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return noalloc_fail(PIX_ERR_CUDA, cudaGetErrorString(e));
+  if (dev < 0 || dev >= NA_MAX_DEVICES) return noalloc_fail(PIX_ERR_INVALID_ARG, "device ordinal %llu beyond %llu", (unsigned long long)dev, NA_MAX_DEVICES);
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p) { cudaGetLastError(); return noalloc_fail(PIX_ERR_CUDA, e != cudaSuccess ? cudaGetErrorString(e) : "cudaGetSymbolAddress returned NULL"); }
+    g_noalloc_addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return PIX_OK;
+}
+
+}  // namespace
+
 }  // namespace pix
+
+extern "C" {
+
+int pix_noalloc_setup(void) {
+  pix::g_noalloc_err[0] = 0;
+  unsigned char* p = nullptr;
+  return pix::noalloc_address(&p);
+}
+
+const char* pix_noalloc_last_error(void) { return pix::g_noalloc_err; }
+
+int pix_cluster_module_noalloc(void* cuda_stream, uint32_t n_digis, const uint16_t* row, const uint16_t* col, const int32_t* charge,
+                               int32_t pixel_threshold_e, int32_t cluster_charge_cut_e, uint32_t max_clusters, int32_t* clus,
+                               uint8_t* status, uint32_t* c_first_digi, uint32_t* c_n_pix, uint32_t* c_charge, float* c_x_col,
+                               float* c_y_row, uint32_t* counts) {
+  using namespace pix;
+  g_noalloc_err[0] = 0;
+  if (n_digis > NA_MAX)
+    return noalloc_fail(PIX_ERR_CAPACITY, "n_digis %llu is beyond PIX_NOALLOC_MAX_DIGIS = %llu (the static scratch array)", n_digis, NA_MAX);
+  if (!counts || (n_digis && (!row || !col || !charge || !clus || !status)))
+    return noalloc_fail(PIX_ERR_INVALID_ARG, "NULL argument");
+  if (max_clusters && (!c_first_digi || !c_n_pix || !c_charge || !c_x_col || !c_y_row))
+    return noalloc_fail(PIX_ERR_INVALID_ARG, "NULL record array with max_clusters > 0");
+  unsigned char* base = nullptr;
+  if (int rc = noalloc_address(&base)) return rc;
+  // the task's view of the scratch array: one event, one module, one run [0, n_digis)
+  uint32_t* hdr = reinterpret_cast<uint32_t*>(base);
+  unsigned char* q = base + NA_HDR;
+  Chunk c = {};
+  c.e0 = 0; c.e1 = 1; c.F = 1; c.M = 1; c.F_shift = 0;
+  c.thr = pixel_threshold_e; c.cut = cluster_charge_cut_e;
+  c.d_row = const_cast<uint16_t*>(row); c.d_col = const_cast<uint16_t*>(col); c.d_charge = const_cast<int32_t*>(charge);  // read only
+  c.d_clus = clus; c.d_status = status;
+  c.module_first = hdr + NH_FIRST; c.module_end = hdr + NH_END; c.segB = hdr + NH_SEG;
+  c.n_clus = hdr + NH_NCLUS; c.t_base = hdr + NH_TBASE; c.ev_cnt = hdr + NH_EVCNT; c.ctl = hdr + NH_CTL;
+  c.g_hash = reinterpret_cast<unsigned long long*>(q); q += (size_t)NA_MAX * 16;
+  c.t_a = reinterpret_cast<uint4*>(q); q += (size_t)NA_MAX * 16;
+  c.g_sx = reinterpret_cast<unsigned long long*>(q); q += (size_t)NA_MAX * 8;
+  c.g_sy = reinterpret_cast<unsigned long long*>(q); q += (size_t)NA_MAX * 8;
+  c.g_pos = reinterpret_cast<uint32_t*>(q); q += (size_t)NA_MAX * 4;
+  c.g_q = reinterpret_cast<uint32_t*>(q); q += (size_t)NA_MAX * 4;
+  c.g_npix = reinterpret_cast<uint32_t*>(q); q += (size_t)NA_MAX * 4;
+  c.t_y = reinterpret_cast<float*>(q); q += (size_t)NA_MAX * 4;
+  NoallocOut o{c_first_digi, c_n_pix, c_charge, c_x_col, c_y_row, counts};
+  noalloc_kernel<<<1, T_B, 0, (cudaStream_t)cuda_stream>>>(c, hdr, n_digis, max_clusters, o);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return noalloc_fail(PIX_ERR_CUDA, cudaGetErrorString(e));
+  return PIX_OK;
+}
+
+}  // extern "C"
