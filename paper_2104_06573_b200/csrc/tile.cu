@@ -218,9 +218,14 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       if (tid < (NBK / 4 + (NBK >> BB_SHIFT) / 4) / 4) reinterpret_cast<uint4*>(s.cnt)[tid] = z4;  // cnt and cntB
       if (tid < 64) reinterpret_cast<uint32_t*>(rbad)[tid] = 0u;
       if (tid < 32) s.survb[tid] = 0u;
-      if (warp == 0) {
-        const uint32_t rel = g0 - T0, wq = rel >> 5;
-        uint32_t v = __funnelshift_r(c.sbits[wq + lane], c.sbits[wq + lane + 1u], rel & 31u);
+    }
+    // the item's start bits: warp NWARP - 1 (its fourth word lies beyond every item: it has the least to do) fetches
+    // them now and works them up after its share of the decoding, just before the barrier
+    uint32_t sb_lo = 0u, sb_hi = 0u;
+    if (warp == NWARP - 1u) { const uint32_t wq = (g0 - T0) >> 5; sb_lo = c.sbits[wq + lane]; sb_hi = c.sbits[wq + lane + 1u]; }
+    auto start_bits = [&]() {
+      {
+        uint32_t v = __funnelshift_r(sb_lo, sb_hi, (g0 - T0) & 31u);
         const uint32_t nb = len > 32u * lane ? len - 32u * lane : 0u;
         v &= nb >= 32u ? FULL : ((1u << nb) - 1u);
         s.bits[lane] = v;
@@ -233,7 +238,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
         s.pre[lane] = inc - pc;
         if (lane == 31) s.n_runs = inc;
       }
-    }
+    };
     // ================================================================== P1: decode, calibrate, insert
     // The words' state stays in registers and is turned by one place per iteration (ROT4), so that the word at hand is
     // always [0]: free in the unrolled loops (register renaming), three moves in the rolled one of P2.
@@ -270,6 +275,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       cr[0] = (uint32_t)e | (m << 16);
       ROT4(w); ROT4(key); ROT4(cr);
     }
+    if (warp == NWARP - 1u) start_bits();
     const bool ordered = !__syncthreads_or(off_t) && c.geom_unique != 0u;  // P0 is done
     // Words that are not the first entry of their bucket go to a per-warp list (bucket | slot | tag): only they can be
     // the later copy of a pixel that appears twice (S10), and after the barrier the list is checked with all lanes busy.
