@@ -374,7 +374,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     const bool long_item = R * 96u < len;  // long runs on average (PU200's inner modules): the other union
     // ---- Forward neighbours (S13): E (r, c+1), SW (r+1, c-1), S (r+1, c), SE (r+1, c+1); col 416..511 and row 160..255
     // never occur, so no bounds checks.  When S is live, SW and SE are joined to it by their own E edges; when E is
-    // live, SE is E's S neighbour.  Every lane looks up (a word that is no live pixel drops what it finds), the edges
+    // live, SE is E's S neighbour; when E, S and SE are all live, S is reached through E - SE - S (E's own S edge, or by
+    // the same argument further along the row, and S's E edge).  Every lane looks up (a word that is no live pixel drops what it finds), the edges
     // go to the warp's list, and the list is united with all lanes busy.
     {
       uint32_t* const el = s.edge[warp];
@@ -391,7 +392,7 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
           lookup4(s, hn, nb);
           const uint32_t nE = nb[0], nS = nb[1], nSW = nb[2], nSE = nb[3];  // >= 1024: no live pixel there
           const uint32_t t1 = nS < 1024u ? nS : nSW;
-          const bool f0 = live && nE < 1024u, f1 = live && t1 < 1024u, f2 = live && nS >= 1024u && nE >= 1024u && nSE < 1024u;
+          const bool f0 = live && nE < 1024u, f1 = live && t1 < 1024u && (nS | nE | nSE) >= 1024u, f2 = live && nS >= 1024u && nE >= 1024u && nSE < 1024u;
           const uint32_t m0 = __ballot_sync(FULL, f0), m1 = __ballot_sync(FULL, f1), m2 = __ballot_sync(FULL, f2);
           if (f0) el[ne + __popc(m0 & lt_mask)] = p | (nE << 16);
           ne += __popc(m0);
