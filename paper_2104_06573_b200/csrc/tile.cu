@@ -482,12 +482,14 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
       const uint32_t big = s.run_big[run], a = s.sum.qn[p];
       Q = big ? a : (a & 0xFFFFFFu); np = big ? s.sum.npx[p] : (a >> 24);
     };
+    uint32_t p_0 = 0u, run_0 = 0u, Q_0 = 0u, np_0 = 0u;  // the root of the first round stays in registers for the second loop
     for (uint32_t i0 = 0u; i0 < n_roots; i0 += NT) {  // block-uniform trip count (one round unless the item is all single pixels)
       const uint32_t i = i0 + tid;
       bool sv = false;
       if (i < n_roots) {
         uint32_t p, run, Q, np;
         load_root(i, p, run, Q, np);
+        if (i0 == 0u) { p_0 = p; run_0 = run; Q_0 = Q; np_0 = np; }
         sv = (int32_t)Q >= c.cut;  // S9: equality keeps (Q < 2^31)
         if (Q > Q_SAFE) rbad[run] = 1;  // 32-bit weighted sums may have wrapped
       }
@@ -515,8 +517,8 @@ __global__ void __launch_bounds__(NT, BLOCKS_PER_SM) tile_kernel(const __grid_co
     for (uint32_t i0 = 0u; i0 < n_roots; i0 += NT) {
       const uint32_t i = i0 + tid;
       const bool valid = i < n_roots;
-      uint32_t p = 0u, run = 0u, Q = 0u, np = 0u;
-      if (valid) load_root(i, p, run, Q, np);
+      uint32_t p = p_0, run = run_0, Q = Q_0, np = np_0;
+      if (valid && i0 != 0u) load_root(i, p, run, Q, np);
       const uint32_t rank = surv_before_root(i), base = rank_before(valid ? (uint32_t)s.run_pos[run] : 0u);
       if (valid) {
         uint32_t id = NO_ID;
