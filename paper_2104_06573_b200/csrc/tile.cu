@@ -7,16 +7,18 @@
 // charge and root stay in registers through all phases (the loop of the neighbour search, the largest body, is rolled
 // and its registers turned, ROT4: fully unrolled the kernel lost 15 % to instruction fetch), only the tables live in
 // shared memory:
-//   P1  decode, calibrate, store module / row / col / charge; run index from the start bits; insert into the
-//       position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 32-bit
+//   P0  clear the tables; the item's run-start bits (fetched at the top of the item by the last warp, whose fourth
+//       word lies beyond every item, and worked up after its share of the decoding)
+//   P1  decode, calibrate, store module / row / col / charge (in front of P0's barrier: none of it needs the tables);
+//       then run index from the start bits; insert into the position hash: key = run | row | col -> bucket (11 bits) + tag (14 bits), exact; a bucket holds four 32-bit
 //       entries tag | below | word (one 128-bit load per lookup; the smallest of the four entry ^ tag is the answer)
 //       plus a second level (4 entries per 32 buckets) that is only read when the first is full; slots are handed
 //       out by a per-bucket counter (one shared atomicAdd, no probing, no CAS)
 //   P2  duplicates (S10) from the list of words that were not first in their bucket (exact pass only when a candidate
 //       turns up; list and pass are skipped for an item whose words come in the detector's read-out order, which the
 //       pre-pass certifies per 128-word chunk: such words are all different pixels), four forward-neighbour lookups
-//       per word, edges into a per-warp list, lock-free unions on the
-//       labels: hook-and-descend (pix_device.cuh), or by representatives (below) when the item's runs are long
+//       per word, at most two edges per pixel and none that other pixels' edges imply, into a per-warp list, lock-free
+//       unions on the labels: hook-and-descend, or by representatives when the item's runs are long (pix_device.cuh)
 //   P3  root of every live pixel; roots start their accumulators (in the memory of the dead hash) and are listed in
 //       word order; the other pixels add charge | pixel count, charge*col, charge*row by shared atomics
 //   P4  one root per thread: Q >= cut survives (ballot bitmap, per-warp scan), numbered per run; temp records
